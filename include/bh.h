@@ -1,0 +1,147 @@
+/*
+ * bh.h — C ABI of libbh: fp64 Barnes-Hut mutual gravity on one NVIDIA B200 (sm_100a).
+ *
+ * The library implements the data-parallel hot path of arxiv/paper_1912_04197 (Ferrari, Lavagna &
+ * Blazquez): the gravity module of PAPER.md §2.1 (lines 45-118).  Every step runs in hand-written
+ * CUDA kernels; there is no CPU fallback.  Citations are PAPER.md:<line>; "R<k>" are the readings
+ * of the paper listed in DESIGN.md §3.
+ *
+ * Conventions
+ *   - Pointers named *_dev are CUDA device pointers, *_host are host pointers.  fp64 throughout
+ *     ("full double precision").  Arrays are dense, row-major: pos/vel/acc are [n][3].
+ *   - Every call enqueues its work on the context's stream and returns without waiting for the
+ *     GPU, except the calls documented as synchronising (bh_synchronize, bh_eval_host and the
+ *     bh_get_* / bh_measure_* calls marked so below).  A context is not thread-safe.
+ *   - Return value: BH_OK (0) or a negative bh_status.  No exceptions, no abort().  Data errors that
+ *     only the GPU can see (non-finite coordinates, node capacity) are sticky: they are reported by
+ *     the next synchronising call.  bh_last_error() gives a human-readable message.
+ *   - Ownership: the caller owns every buffer it passes, including the workspace; the library
+ *     allocates no device memory except a few bytes of pinned host memory at bh_create.
+ *   - Preconditions that are not checked: masses finite and > 0 (R15); |coordinate| < 2^1000 and the
+ *     largest extent either 0 or >= 2^-900.
+ */
+#ifndef BH_H_
+#define BH_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct bh_ctx bh_ctx; /* opaque */
+
+typedef enum {
+    BH_OK = 0,
+    BH_ERR_INVALID_ARG = -1, /* null pointer, n < 1, n > max_n, leaf_cap < 1, theta < 0, eps < 0, ... */
+    BH_ERR_CAPACITY = -2,    /* workspace too small / node array overflow */
+    BH_ERR_NONFINITE = -3,   /* a coordinate is NaN or infinite (found by the bounding-box reduction) */
+    BH_ERR_STATE = -4,       /* call order: accel/direct before build, kdk_step before bind_state */
+    BH_ERR_CUDA = -5         /* a CUDA runtime call or an earlier asynchronous launch failed */
+} bh_status;
+
+#define BH_MAX_LEVEL 21    /* 63-bit Morton keys, 3 bits per level (R9) */
+#define BH_GROUP_CELL 512  /* Gc: walk groups never straddle a tree cell holding <= Gc bodies (R6) */
+
+/* Bytes of device workspace a context for up to max_n bodies needs.  0 if the arguments are invalid
+ * (max_n < 1 or > 2^30, leaf_cap < 1 or > 1024, group_size not 0 or 32). */
+size_t bh_workspace_bytes(int64_t max_n, int leaf_cap, int group_size);
+
+/* Create a context.  leaf_cap = C: a node is a leaf iff it holds <= C bodies or sits at level 21
+ * (PAPER.md:62 subdivides "until each node ... contains zero or one particle" = C 1; R8).
+ * group_size = W, the most bodies that walk the tree together (0 or 32; R6).  workspace_dev must hold
+ * bh_workspace_bytes() bytes, be 256-byte aligned and stay valid until bh_destroy.  cuda_stream is a
+ * cudaStream_t (NULL = the legacy default stream). */
+bh_status bh_create(bh_ctx **out, int64_t max_n, int leaf_cap, int group_size, void *workspace_dev,
+                    size_t workspace_bytes, void *cuda_stream);
+bh_status bh_destroy(bh_ctx *ctx);
+bh_status bh_set_stream(bh_ctx *ctx, void *cuda_stream);
+
+/* Build the octree of the n bodies ("re-built at each time step"):
+ * bounding cube -> 63-bit Morton keys -> stable LSD radix sort -> sorted (x,y,z,m) bodies and group
+ * boxes -> nodes (level, begin, count, first_child, child_mask, parent) in level/Morton order ->
+ * monopoles, Eq. (2) PAPER.md:76.  pos_dev [n][3] and mass_dev [n] are read only and need not outlive
+ * the call's execution on the stream. */
+bh_status bh_build(bh_ctx *ctx, const double *pos_dev, const double *mass_dev, int64_t n);
+
+/* Barnes-Hut accelerations of all bodies of the last build, Eqs. (3)-(6) PAPER.md:84-106, written
+ * to acc_dev [n][3] in the body order given to bh_build.  theta >= 0 is the opening parameter
+ * (cell edge / distance, R4; strict <, R5), eps >= 0 the Plummer softening of Eq. (6), G the
+ * gravitational constant.  Output is acceleration, not force (R1). */
+bh_status bh_accel(bh_ctx *ctx, double theta, double eps, double G, double *acc_dev);
+
+/* Direct N^2 sum, Eq. (1), over the bodies of the last build; same softened kernel. */
+bh_status bh_direct(bh_ctx *ctx, double eps, double G, double *acc_dev);
+
+/* Direct sum for nt target bodies tgt_dev[k] (indices in bh_build order) against all n sources;
+ * acc_dev is [nt][3].  For sampled checks at sizes where N^2 is too long. */
+bh_status bh_direct_targets(bh_ctx *ctx, const int32_t *tgt_dev, int64_t nt, double eps, double G,
+                            double *acc_dev);
+
+/* Leapfrog kick-drift-kick (PAPER.md:148 lists leapfrog among the symplectic steppers; R18).
+ * bh_bind_state borrows pos_dev/vel_dev [n][3] (updated IN PLACE by every step) and mass_dev [n].
+ * bh_kdk_step(dt):  v += a dt/2;  x += v dt;  rebuild tree;  a = accel(x);  v += a dt/2, with
+ * v = fma(a, dt/2, v) and x = fma(v, dt, x).  The first step after bind evaluates a(x0) once. */
+bh_status bh_bind_state(bh_ctx *ctx, double *pos_dev, double *vel_dev, const double *mass_dev,
+                        int64_t n, double theta, double eps, double G);
+bh_status bh_kdk_step(bh_ctx *ctx, double dt);
+/* Device pointer to the accelerations [n][3] held by the bound state (valid after a step). */
+bh_status bh_get_state_acc(bh_ctx *ctx, const double **acc_dev);
+
+/* End-to-end evaluation from HOST buffers: copies pos_host [n][3] and mass_host [n] to the GPU,
+ * builds, walks, copies acc_host [n][3] back and waits.  Pinned host memory makes the copies
+ * asynchronous; pageable memory works too. */
+bh_status bh_eval_host(bh_ctx *ctx, const double *pos_host, const double *mass_host, int64_t n,
+                       double theta, double eps, double G, double *acc_host);
+
+/* Wait for the stream and report sticky errors (BH_ERR_NONFINITE, BH_ERR_CAPACITY, BH_ERR_CUDA). */
+bh_status bh_synchronize(bh_ctx *ctx);
+
+/* ---- inspection of the last build (parity tests, metrics) ---- */
+/* Synchronising. Cube corner lo[3] and side L (a power of two, R11). */
+bh_status bh_get_cube(bh_ctx *ctx, double lo_host[3], double *side_host);
+/* Sorted keys [n] and the sort permutation perm [n] (sorted position -> bh_build index). */
+bh_status bh_get_keys(bh_ctx *ctx, uint64_t *sorted_key_dev, uint32_t *perm_dev);
+/* Synchronising. Node count M and depth (deepest level). */
+bh_status bh_get_node_count(bh_ctx *ctx, int64_t *m_host, int32_t *depth_host);
+/* Node arrays, each [M] (mono [M][4] = cx,cy,cz,m); any pointer may be NULL. Caller sizes them
+ * with bh_get_node_count. */
+bh_status bh_get_nodes(bh_ctx *ctx, uint8_t *level_dev, uint32_t *begin_dev, uint32_t *count_dev,
+                       int32_t *first_child_dev, uint8_t *child_mask_dev, int32_t *parent_dev,
+                       double *mono_dev);
+/* Synchronising. Walk groups (R6): a group cell is a tree node with <= BH_GROUP_CELL bodies (or a
+ * leaf) whose parent has more; each group cell is cut into runs of W consecutive sorted bodies;
+ * groups are numbered in sorted-body order.  *ng_host = number of groups Ng; gstart_dev (may be
+ * NULL, else room for Ng+1 <= n+1 entries) receives the first sorted body of each group, then n. */
+bh_status bh_get_groups(bh_ctx *ctx, int64_t *ng_host, uint32_t *gstart_dev);
+/* Synchronising. Sorted bodies [n][4] (x,y,z,m) and group boxes [Ng][3] each; any pointer may be NULL. */
+bh_status bh_get_bodies(bh_ctx *ctx, double *sbody_dev, double *glo_dev, double *ghi_dev);
+/* Synchronising. Per-group interaction-list lengths of the last bh_accel, each [Ng]. */
+bh_status bh_get_counts(bh_ctx *ctx, uint32_t *n_mono_per_group_dev, uint32_t *n_direct_per_group_dev);
+
+/* Synchronising. Totals of the last bh_accel: stats[0] = sum over groups of n_mono, stats[1] = sum
+ * of n_direct, stats[2] = body-source interactions evaluated (sum of group bodies x list length),
+ * stats[3] = nodes tested by the opening criterion. */
+bh_status bh_get_stats(bh_ctx *ctx, uint64_t stats_host[4]);
+
+/* Phase timing with CUDA events on the context's stream.  After bh_set_timing(ctx, 1) every
+ * bh_build/bh_accel/bh_direct records events; bh_get_phase_ms (synchronising) returns the last
+ * durations in ms: [0] cube, [1] keys+histogram, [2] sort, [3] gather+boxes, [4] tree,
+ * [5] monopoles, [6] walk, [7] direct, [8] kick/drift kernels of the last bh_kdk_step. */
+#define BH_NUM_PHASES 9
+bh_status bh_set_timing(bh_ctx *ctx, int enable);
+bh_status bh_get_phase_ms(bh_ctx *ctx, float ms_host[BH_NUM_PHASES]);
+
+/* fp64 FMA throughput microbenchmark (register-resident DFMA chains on every SM): returns the
+ * measured TFLOP/s (2 flops per FMA) in *tflops_host.  The roofline denominator of the walk and
+ * direct kernels.  Synchronising. */
+bh_status bh_measure_fp64_peak(bh_ctx *ctx, double *tflops_host);
+
+const char *bh_last_error(const bh_ctx *ctx);
+const char *bh_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* BH_H_ */

@@ -251,12 +251,41 @@ void orc_monopoles(const double *sbody, int64_t M, const uint32_t *begin, const 
     }
 }
 
-/* O7  Walk groups: W consecutive sorted bodies and their axis-aligned bounding box (exact). */
-void orc_groups(const double *sbody, int64_t n, int32_t W, double *glo, double *ghi)
+/* ---------------------------------------------------------------------------------------------
+ * O7  Walk groups (reading R6).  PAPER.md:118: "Each body is assigned to a thread ... Thanks to
+ * sorting, neighbor bodies require the traversal of a similar sub-part of the octree": bodies that
+ * are neighbours in the sorted order walk together.  A group must be spatially compact, so groups
+ * never straddle a GROUP CELL: a tree node holding <= Gc bodies whose parent holds more than Gc
+ * (the root if n <= Gc; a level-21 leaf is a group cell whatever it holds).  Group cells partition
+ * the sorted bodies; each is cut into runs of W consecutive bodies (the last run may be shorter).
+ * Groups are numbered in sorted-body order.  gstart must have room for n + 1 entries; returns the
+ * number of groups Ng, group g = sorted bodies [gstart[g], gstart[g+1]).
+ * ------------------------------------------------------------------------------------------- */
+int64_t orc_group_starts(int64_t n, int64_t M, int32_t W, int32_t Gc, const uint32_t *begin,
+                         const uint32_t *count, const int32_t *first_child, const int32_t *parent,
+                         uint32_t *gstart)
 {
-    int64_t ng = (n + W - 1) / W;
+    /* mark the first body of every run */
+    uint8_t *flag = (uint8_t *)calloc((size_t)n + 1, 1);
+    for (int64_t t = 0; t < M; ++t) {
+        int small = (int64_t)count[t] <= Gc || first_child[t] < 0;
+        int parent_big = parent[t] < 0 || (int64_t)count[parent[t]] > Gc;
+        if (small && parent_big)
+            for (int64_t j = begin[t]; j < (int64_t)begin[t] + count[t]; j += W) flag[j] = 1;
+    }
+    int64_t ng = 0;
+    for (int64_t j = 0; j < n; ++j)
+        if (flag[j]) gstart[ng++] = (uint32_t)j;
+    gstart[ng] = (uint32_t)n;
+    free(flag);
+    return ng;
+}
+
+/* bounding boxes of the groups (exact min / max of the sorted coordinates) */
+void orc_group_boxes(const double *sbody, const uint32_t *gstart, int64_t ng, double *glo, double *ghi)
+{
     for (int64_t g = 0; g < ng; ++g) {
-        int64_t b = g * W, e = b + W < n ? b + W : n;
+        int64_t b = gstart[g], e = gstart[g + 1];
         for (int a = 0; a < 3; ++a) {
             double l = sbody[4 * b + a], h = l;
             for (int64_t j = b + 1; j < e; ++j) {
@@ -357,14 +386,15 @@ static inline void orc_term(const long double p[3], const double *src, long doub
 
 /* Lists of one group (for tests of the walk structure). Returns 0; lists are malloc'ed here and
  * must be released with orc_free. */
-int orc_walk_lists(double L, int64_t n, int32_t W, const uint8_t *level, const uint32_t *begin,
-                   const uint32_t *count, const int32_t *first_child, const uint8_t *child_mask,
-                   const double *mono, const double *glo, const double *ghi, int64_t g, double theta,
-                   int32_t **list_mono, int64_t *n_mono, int32_t **list_direct, int64_t *n_direct)
+int orc_walk_lists(double L, int64_t n, const uint32_t *gstart, const uint8_t *level,
+                   const uint32_t *begin, const uint32_t *count, const int32_t *first_child,
+                   const uint8_t *child_mask, const double *mono, const double *glo, const double *ghi,
+                   int64_t g, double theta, int32_t **list_mono, int64_t *n_mono,
+                   int32_t **list_direct, int64_t *n_direct)
 {
     orc_tree_view T = {L, n, level, begin, count, first_child, child_mask, mono};
     orc_ivec lm = {0, 0, 0}, ld = {0, 0, 0};
-    int64_t gb = g * W, ge = gb + W < n ? gb + W : n;
+    int64_t gb = gstart[g], ge = gstart[g + 1];
     orc_visit(&T, 0, gb, ge, &glo[3 * g], &ghi[3 * g], theta * theta, &lm, &ld);
     *list_mono = lm.v;
     *n_mono = lm.n;
@@ -381,7 +411,7 @@ void orc_free(void *p) { free(p); }
  * store at the body's ORIGINAL index.  n_mono / n_direct (per group, indexed g - g0) and kappa
  * (per body, original index; sum of term norms over norm of the sum) may be NULL.
  * ------------------------------------------------------------------------------------------- */
-void orc_accel(double L, int64_t n, int32_t W, const uint8_t *level, const uint32_t *begin,
+void orc_accel(double L, int64_t n, const uint32_t *gstart, const uint8_t *level, const uint32_t *begin,
                const uint32_t *count, const int32_t *first_child, const uint8_t *child_mask,
                const double *mono, const double *sbody, const uint32_t *perm, const double *glo,
                const double *ghi, double theta, double eps, double G, int64_t g0, int64_t g1,
@@ -394,7 +424,7 @@ void orc_accel(double L, int64_t n, int32_t W, const uint8_t *level, const uint3
         orc_ivec lm = {0, 0, 0}, ld = {0, 0, 0};
 #pragma omp for schedule(dynamic, 4)
         for (int64_t g = g0; g < g1; ++g) {
-            int64_t gb = g * W, ge = gb + W < n ? gb + W : n;
+            int64_t gb = gstart[g], ge = gstart[g + 1];
             lm.n = 0;
             ld.n = 0;
             orc_visit(&T, 0, gb, ge, &glo[3 * g], &ghi[3 * g], theta * theta, &lm, &ld);

@@ -97,12 +97,14 @@ class Tree:
     child_mask: np.ndarray   # [M] u8
     parent: np.ndarray       # [M] i32
     mono: np.ndarray         # [M,4] (cx,cy,cz,m)
+    Gc: int                  # group-cell capacity
+    gstart: np.ndarray       # [Ng+1] u32: group g = sorted bodies [gstart[g], gstart[g+1])
     glo: np.ndarray          # [Ng,3]
     ghi: np.ndarray          # [Ng,3]
 
     @property
     def ngroups(self) -> int:
-        return (self.n + self.W - 1) // self.W
+        return self.gstart.shape[0] - 1
 
 
 def tree_from_keys(skey: np.ndarray, leaf_cap: int):
@@ -134,17 +136,29 @@ def monopoles(sbody, begin, count, first_child, child_mask) -> np.ndarray:
     return mono
 
 
-def groups(sbody, W):
-    n = sbody.shape[0]
-    ng = (n + W - 1) // W
+def group_starts(n, W, Gc, begin, count, first_child, parent) -> np.ndarray:
+    """O7: group start indices [Ng+1] (last entry n)."""
+    gstart = np.zeros(n + 1, dtype=np.uint32)
+    lib().orc_group_starts.restype = C.c_int64
+    ng = lib().orc_group_starts(C.c_int64(n), C.c_int64(begin.shape[0]), C.c_int32(W), C.c_int32(Gc),
+                                _p(begin), _p(count), _p(first_child), _p(parent), _p(gstart))
+    return gstart[:ng + 1].copy()
+
+
+def group_boxes(sbody, gstart):
+    ng = gstart.shape[0] - 1
     glo = np.zeros((ng, 3))
     ghi = np.zeros((ng, 3))
-    lib().orc_groups(_p(sbody), C.c_int64(n), C.c_int32(W), _p(glo), _p(ghi))
+    lib().orc_group_boxes(_p(sbody), _p(gstart), C.c_int64(ng), _p(glo), _p(ghi))
     return glo, ghi
 
 
-def build(pos, mass, leaf_cap: int, W: int = 32) -> Tree:
-    """O1..O7 in order: cube, keys, sort, gather, tree, monopoles, groups."""
+DEFAULT_GC = 512   # group-cell capacity used by the CUDA path (DESIGN.md R6)
+
+
+def build(pos, mass, leaf_cap: int, W: int = 32, Gc: int | None = None, gstart=None) -> Tree:
+    """O1..O7 in order: cube, keys, sort, gather, tree, monopoles, groups.  Gc defaults to
+    max(DEFAULT_GC, W); W = 1 with any Gc is the paper's per-body walk."""
     pos = np.ascontiguousarray(pos, dtype=np.float64)
     mass = np.ascontiguousarray(mass, dtype=np.float64)
     n = pos.shape[0]
@@ -155,9 +169,14 @@ def build(pos, mass, leaf_cap: int, W: int = 32) -> Tree:
     lib().orc_gather(_p(pos), _p(mass), _p(perm), C.c_int64(n), _p(sbody))
     M, depth, level, begin, count, first_child, child_mask, parent = tree_from_keys(skey, leaf_cap)
     mono = monopoles(sbody, begin, count, first_child, child_mask)
-    glo, ghi = groups(sbody, W)
+    if Gc is None:
+        Gc = max(DEFAULT_GC, W)
+    if gstart is None:
+        gstart = group_starts(n, W, Gc, begin, count, first_child, parent)
+    gstart = np.ascontiguousarray(gstart, dtype=np.uint32)
+    glo, ghi = group_boxes(sbody, gstart)
     return Tree(n, leaf_cap, W, lo, L, e, key, perm, skey, sbody, M, depth, level, begin, count,
-                first_child, child_mask, parent, mono, glo, ghi)
+                first_child, child_mask, parent, mono, Gc, gstart, glo, ghi)
 
 
 def walk_lists(t: Tree, g: int, theta: float):
@@ -166,7 +185,7 @@ def walk_lists(t: Tree, g: int, theta: float):
     ld = C.POINTER(C.c_int32)()
     nm = C.c_int64()
     nd = C.c_int64()
-    lib().orc_walk_lists(C.c_double(t.L), C.c_int64(t.n), C.c_int32(t.W), _p(t.level), _p(t.begin),
+    lib().orc_walk_lists(C.c_double(t.L), C.c_int64(t.n), _p(t.gstart), _p(t.level), _p(t.begin),
                          _p(t.count), _p(t.first_child), _p(t.child_mask), _p(t.mono), _p(t.glo),
                          _p(t.ghi), C.c_int64(g), C.c_double(theta), C.byref(lm), C.byref(nm),
                          C.byref(ld), C.byref(nd))
@@ -187,7 +206,7 @@ def accel(t: Tree, theta: float, eps: float, G: float, g0: int = 0, g1: int | No
     n_mono = np.zeros(g1 - g0, dtype=np.uint32)
     n_direct = np.zeros(g1 - g0, dtype=np.uint32)
     kappa = np.full(t.n, np.nan) if want_kappa else None
-    lib().orc_accel(C.c_double(t.L), C.c_int64(t.n), C.c_int32(t.W), _p(t.level), _p(t.begin),
+    lib().orc_accel(C.c_double(t.L), C.c_int64(t.n), _p(t.gstart), _p(t.level), _p(t.begin),
                     _p(t.count), _p(t.first_child), _p(t.child_mask), _p(t.mono), _p(t.sbody),
                     _p(t.perm), _p(t.glo), _p(t.ghi), C.c_double(theta), C.c_double(eps),
                     C.c_double(G), C.c_int64(g0), C.c_int64(g1), _p(acc), _p(n_mono), _p(n_direct),

@@ -1,0 +1,304 @@
+"""Thin ctypes binding of libbh (include/bh.h): same call names, argument marshalling only.
+
+Every step of the path runs in the CUDA kernels of the library; torch is used for device memory
+and streams.  There is no fallback: if libbh.so is missing, or a call returns a negative status,
+this module raises.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import torch
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libbh.so")
+NUM_PHASES = 9
+PHASE_NAMES = ("cube", "keys", "sort", "gather", "tree", "monopoles", "walk", "direct", "kick_drift")
+
+BH_OK, BH_ERR_INVALID_ARG, BH_ERR_CAPACITY, BH_ERR_NONFINITE, BH_ERR_STATE, BH_ERR_CUDA = 0, -1, -2, -3, -4, -5
+
+_lib = None
+
+
+class BhError(RuntimeError):
+    def __init__(self, status: int, message: str):
+        super().__init__(f"libbh status {status}: {message}")
+        self.status = status
+
+
+def lib() -> C.CDLL:
+    """Load libbh.so (built in-tree by paper_1912_04197_b200.build). Fails loudly if absent."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise RuntimeError(f"{LIB_PATH} is missing: run `python -m paper_1912_04197_b200.build` "
+                               "(there is no CPU fallback)")
+        L = C.CDLL(LIB_PATH)
+        vp, i64, dbl, i32 = C.c_void_p, C.c_int64, C.c_double, C.c_int
+        L.bh_workspace_bytes.restype = C.c_size_t
+        L.bh_workspace_bytes.argtypes = [i64, i32, i32]
+        L.bh_last_error.restype = C.c_char_p
+        L.bh_last_error.argtypes = [vp]
+        L.bh_version.restype = C.c_char_p
+        sigs = {
+            "bh_create": [C.POINTER(vp), i64, i32, i32, vp, C.c_size_t, vp],
+            "bh_destroy": [vp], "bh_set_stream": [vp, vp],
+            "bh_build": [vp, vp, vp, i64],
+            "bh_accel": [vp, dbl, dbl, dbl, vp],
+            "bh_direct": [vp, dbl, dbl, vp],
+            "bh_direct_targets": [vp, vp, i64, dbl, dbl, vp],
+            "bh_bind_state": [vp, vp, vp, vp, i64, dbl, dbl, dbl],
+            "bh_kdk_step": [vp, dbl],
+            "bh_get_state_acc": [vp, C.POINTER(vp)],
+            "bh_eval_host": [vp, vp, vp, i64, dbl, dbl, dbl, vp],
+            "bh_synchronize": [vp],
+            "bh_get_cube": [vp, C.POINTER(dbl), C.POINTER(dbl)],
+            "bh_get_keys": [vp, vp, vp],
+            "bh_get_node_count": [vp, C.POINTER(i64), C.POINTER(C.c_int32)],
+            "bh_get_nodes": [vp, vp, vp, vp, vp, vp, vp, vp],
+            "bh_get_groups": [vp, C.POINTER(i64), vp],
+            "bh_get_bodies": [vp, vp, vp, vp],
+            "bh_get_counts": [vp, vp, vp],
+            "bh_get_stats": [vp, C.POINTER(C.c_uint64)],
+            "bh_set_timing": [vp, i32],
+            "bh_get_phase_ms": [vp, C.POINTER(C.c_float)],
+            "bh_measure_fp64_peak": [vp, C.POINTER(dbl)],
+        }
+        for name, args in sigs.items():
+            f = getattr(L, name)
+            f.restype = C.c_int
+            f.argtypes = args
+        _lib = L
+    return _lib
+
+
+EXPORTS = ("bh_workspace_bytes", "bh_create", "bh_destroy", "bh_set_stream", "bh_build", "bh_accel",
+           "bh_direct", "bh_direct_targets", "bh_bind_state", "bh_kdk_step", "bh_get_state_acc",
+           "bh_eval_host", "bh_synchronize", "bh_get_cube", "bh_get_keys", "bh_get_node_count",
+           "bh_get_nodes", "bh_get_groups", "bh_get_bodies", "bh_get_counts", "bh_get_stats", "bh_set_timing",
+           "bh_get_phase_ms", "bh_measure_fp64_peak", "bh_last_error", "bh_version")
+
+
+def _check(ctx, status: int):
+    if status != BH_OK:
+        raise BhError(status, lib().bh_last_error(ctx).decode())
+
+
+def _dev(t: torch.Tensor | None, dtype, what: str):
+    if t is None:
+        return None
+    if not (t.is_cuda and t.dtype == dtype and t.is_contiguous()):
+        raise TypeError(f"{what}: expected a contiguous CUDA tensor of {dtype}")
+    return t.data_ptr()
+
+
+def _host(t: torch.Tensor, what: str):
+    if t.is_cuda or t.dtype != torch.float64 or not t.is_contiguous():
+        raise TypeError(f"{what}: expected a contiguous CPU float64 tensor")
+    return t.data_ptr()
+
+
+def _stream_ptr(stream):
+    if stream is None:
+        stream = torch.cuda.current_stream()
+    return stream.cuda_stream
+
+
+# ---- the C calls, one to one ----
+def bh_workspace_bytes(max_n: int, leaf_cap: int, group_size: int = 0) -> int:
+    return int(lib().bh_workspace_bytes(max_n, leaf_cap, group_size))
+
+
+def bh_create(max_n: int, leaf_cap: int, group_size: int, workspace: torch.Tensor, stream=None):
+    ctx = C.c_void_p()
+    st = lib().bh_create(C.byref(ctx), max_n, leaf_cap, group_size, workspace.data_ptr(),
+                         workspace.numel() * workspace.element_size(), _stream_ptr(stream))
+    _check(None, st)
+    return ctx
+
+
+def bh_destroy(ctx):
+    _check(ctx, lib().bh_destroy(ctx))
+
+
+def bh_set_stream(ctx, stream):
+    _check(ctx, lib().bh_set_stream(ctx, _stream_ptr(stream)))
+
+
+def bh_build(ctx, pos: torch.Tensor, mass: torch.Tensor):
+    n = pos.shape[0]
+    if pos.dim() != 2 or pos.shape[1] != 3 or mass.shape != (n,):
+        raise TypeError("bh_build: pos must be [n,3] and mass [n]")
+    _check(ctx, lib().bh_build(ctx, _dev(pos, torch.float64, "pos"), _dev(mass, torch.float64, "mass"), n))
+
+
+def bh_accel(ctx, theta: float, eps: float, G: float, acc: torch.Tensor):
+    _check(ctx, lib().bh_accel(ctx, theta, eps, G, _dev(acc, torch.float64, "acc")))
+
+
+def bh_direct(ctx, eps: float, G: float, acc: torch.Tensor):
+    _check(ctx, lib().bh_direct(ctx, eps, G, _dev(acc, torch.float64, "acc")))
+
+
+def bh_direct_targets(ctx, targets: torch.Tensor, eps: float, G: float, acc: torch.Tensor):
+    _check(ctx, lib().bh_direct_targets(ctx, _dev(targets, torch.int32, "targets"), targets.numel(), eps, G,
+                                        _dev(acc, torch.float64, "acc")))
+
+
+def bh_bind_state(ctx, pos, vel, mass, theta: float, eps: float, G: float):
+    _check(ctx, lib().bh_bind_state(ctx, _dev(pos, torch.float64, "pos"), _dev(vel, torch.float64, "vel"),
+                                    _dev(mass, torch.float64, "mass"), pos.shape[0], theta, eps, G))
+
+
+def bh_kdk_step(ctx, dt: float):
+    _check(ctx, lib().bh_kdk_step(ctx, dt))
+
+
+def bh_eval_host(ctx, pos_host, mass_host, theta, eps, G, acc_host):
+    _check(ctx, lib().bh_eval_host(ctx, _host(pos_host, "pos"), _host(mass_host, "mass"), pos_host.shape[0],
+                                   theta, eps, G, _host(acc_host, "acc")))
+
+
+def bh_synchronize(ctx):
+    _check(ctx, lib().bh_synchronize(ctx))
+
+
+def bh_get_cube(ctx):
+    lo = (C.c_double * 3)()
+    side = C.c_double()
+    _check(ctx, lib().bh_get_cube(ctx, lo, C.byref(side)))
+    return [lo[0], lo[1], lo[2]], side.value
+
+
+def bh_get_keys(ctx, sorted_key: torch.Tensor | None, perm: torch.Tensor | None):
+    _check(ctx, lib().bh_get_keys(ctx, _dev(sorted_key, torch.int64, "sorted_key"), _dev(perm, torch.int32, "perm")))
+
+
+def bh_get_node_count(ctx):
+    m = C.c_int64()
+    d = C.c_int32()
+    _check(ctx, lib().bh_get_node_count(ctx, C.byref(m), C.byref(d)))
+    return m.value, d.value
+
+
+def bh_get_nodes(ctx, level=None, begin=None, count=None, first_child=None, child_mask=None, parent=None, mono=None):
+    _check(ctx, lib().bh_get_nodes(ctx, _dev(level, torch.uint8, "level"), _dev(begin, torch.int32, "begin"),
+                                   _dev(count, torch.int32, "count"), _dev(first_child, torch.int32, "first_child"),
+                                   _dev(child_mask, torch.uint8, "child_mask"), _dev(parent, torch.int32, "parent"),
+                                   _dev(mono, torch.float64, "mono")))
+
+
+def bh_get_groups(ctx, gstart: torch.Tensor | None = None) -> int:
+    ng = C.c_int64()
+    _check(ctx, lib().bh_get_groups(ctx, C.byref(ng), _dev(gstart, torch.int32, "gstart")))
+    return ng.value
+
+
+def bh_get_bodies(ctx, sbody=None, glo=None, ghi=None):
+    _check(ctx, lib().bh_get_bodies(ctx, _dev(sbody, torch.float64, "sbody"), _dev(glo, torch.float64, "glo"),
+                                    _dev(ghi, torch.float64, "ghi")))
+
+
+def bh_get_counts(ctx, n_mono=None, n_direct=None):
+    _check(ctx, lib().bh_get_counts(ctx, _dev(n_mono, torch.int32, "n_mono"), _dev(n_direct, torch.int32, "n_direct")))
+
+
+def bh_get_stats(ctx):
+    s = (C.c_uint64 * 4)()
+    _check(ctx, lib().bh_get_stats(ctx, s))
+    return {"n_mono": s[0], "n_direct": s[1], "interactions": s[2], "nodes_tested": s[3]}
+
+
+def bh_set_timing(ctx, enable: bool):
+    _check(ctx, lib().bh_set_timing(ctx, int(enable)))
+
+
+def bh_get_phase_ms(ctx):
+    ms = (C.c_float * NUM_PHASES)()
+    _check(ctx, lib().bh_get_phase_ms(ctx, ms))
+    return {PHASE_NAMES[i]: ms[i] for i in range(NUM_PHASES)}
+
+
+def bh_measure_fp64_peak(ctx) -> float:
+    v = C.c_double()
+    _check(ctx, lib().bh_measure_fp64_peak(ctx, C.byref(v)))
+    return v.value
+
+
+# ---- convenience owner of a context and its torch-allocated workspace (no arithmetic) ----
+class Context:
+    def __init__(self, max_n: int, leaf_cap: int, group_size: int = 0, device="cuda:0", stream=None):
+        if not torch.cuda.is_available():
+            raise RuntimeError("libbh needs a CUDA device; there is no CPU fallback")
+        self.device = torch.device(device)
+        self.max_n, self.leaf_cap, self.W = max_n, leaf_cap, 32
+        nbytes = bh_workspace_bytes(max_n, leaf_cap, group_size)
+        if nbytes == 0:
+            raise BhError(BH_ERR_INVALID_ARG, "max_n, leaf_cap or group_size out of range")
+        with torch.cuda.device(self.device):
+            self.workspace = torch.empty(nbytes + 256, dtype=torch.uint8, device=self.device)
+            off = (-self.workspace.data_ptr()) % 256
+            self._ws = self.workspace[off:off + nbytes]
+            self.ctx = bh_create(max_n, leaf_cap, group_size, self._ws, stream)
+        self.n = 0
+
+    def close(self):
+        if self.ctx is not None:
+            bh_destroy(self.ctx)
+            self.ctx = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def build(self, pos, mass):
+        bh_build(self.ctx, pos, mass)
+        self.n = pos.shape[0]
+
+    def accel(self, theta, eps, G, out=None):
+        out = torch.empty((self.n, 3), dtype=torch.float64, device=self.device) if out is None else out
+        bh_accel(self.ctx, theta, eps, G, out)
+        return out
+
+    def direct(self, eps, G, targets=None, out=None):
+        if targets is None:
+            out = torch.empty((self.n, 3), dtype=torch.float64, device=self.device) if out is None else out
+            bh_direct(self.ctx, eps, G, out)
+        else:
+            out = torch.empty((targets.numel(), 3), dtype=torch.float64, device=self.device) if out is None else out
+            bh_direct_targets(self.ctx, targets, eps, G, out)
+        return out
+
+    def tree(self):
+        """Copies of the last build's arrays (torch tensors on the device), for inspection."""
+        M, depth = bh_get_node_count(self.ctx)
+        d, n = self.device, self.n
+        ng = bh_get_groups(self.ctx)
+        out = dict(M=M, depth=depth, ng=ng, gstart=torch.empty(ng + 1, dtype=torch.int32, device=d),
+                   skey=torch.empty(n, dtype=torch.int64, device=d), perm=torch.empty(n, dtype=torch.int32, device=d),
+                   level=torch.empty(M, dtype=torch.uint8, device=d), begin=torch.empty(M, dtype=torch.int32, device=d),
+                   count=torch.empty(M, dtype=torch.int32, device=d),
+                   first_child=torch.empty(M, dtype=torch.int32, device=d),
+                   child_mask=torch.empty(M, dtype=torch.uint8, device=d),
+                   parent=torch.empty(M, dtype=torch.int32, device=d),
+                   mono=torch.empty((M, 4), dtype=torch.float64, device=d),
+                   sbody=torch.empty((n, 4), dtype=torch.float64, device=d),
+                   glo=torch.empty((ng, 3), dtype=torch.float64, device=d),
+                   ghi=torch.empty((ng, 3), dtype=torch.float64, device=d))
+        bh_get_keys(self.ctx, out["skey"], out["perm"])
+        bh_get_nodes(self.ctx, out["level"], out["begin"], out["count"], out["first_child"], out["child_mask"],
+                     out["parent"], out["mono"])
+        bh_get_groups(self.ctx, out["gstart"])
+        bh_get_bodies(self.ctx, out["sbody"], out["glo"], out["ghi"])
+        out["lo"], out["L"] = bh_get_cube(self.ctx)
+        return out
+
+    def counts(self):
+        ng = bh_get_groups(self.ctx)
+        a = torch.empty(ng, dtype=torch.int32, device=self.device)
+        b = torch.empty(ng, dtype=torch.int32, device=self.device)
+        bh_get_counts(self.ctx, a, b)
+        return a, b

@@ -1,0 +1,532 @@
+// bh_api.cu — the C ABI declared in include/bh.h: context, workspace carving, call sequencing.
+#include <cstdio>
+#include <cstring>
+#include <new>
+
+#include "bh_common.cuh"
+
+using namespace bh;
+
+struct bh_ctx {
+    int64_t max_n = 0;
+    int leaf_cap = 0;
+    int group = kGroup;
+    cudaStream_t stream = nullptr;
+    Workspace ws{};
+    int64_t n = 0;          // bodies of the last build
+    bool built = false;
+    bool walked = false;
+    // bound leapfrog state
+    double *pos = nullptr, *vel = nullptr;
+    const double *mass = nullptr;
+    int64_t bound_n = 0;
+    double theta = 0, eps = 0, G = 0;
+    bool bound = false, have_acc = false;
+    // timing
+    bool timing = false;
+    cudaEvent_t ev[BH_NUM_PHASES][2]{};
+    bool ev_set[BH_NUM_PHASES]{};
+    DevState *host_state = nullptr;   // pinned mirror for synchronising getters
+    char err[256] = "";
+};
+
+namespace {
+
+thread_local char g_err[256] = "";
+
+bh_status fail(bh_ctx *c, bh_status s, const char *msg)
+{
+    snprintf(c ? c->err : g_err, 256, "%s", msg);
+    return s;
+}
+
+bh_status cuda_check(bh_ctx *c, cudaError_t e, const char *what)
+{
+    if (e == cudaSuccess) return BH_OK;
+    snprintf(c->err, 256, "%s: %s", what, cudaGetErrorString(e));
+    return BH_ERR_CUDA;
+}
+
+inline size_t align_up(size_t x) { return (x + 255) & ~(size_t)255; }
+
+struct Carver {
+    char *base;
+    size_t off = 0;
+    template <typename T>
+    T *take(size_t count)
+    {
+        size_t at = off;
+        off = align_up(off + count * sizeof(T));
+        return base ? reinterpret_cast<T *>(base + at) : nullptr;
+    }
+};
+
+struct Phase {   // records events around a phase when timing is on
+    bh_ctx *c;
+    int id;
+    Phase(bh_ctx *ctx, int phase) : c(ctx), id(phase)
+    {
+        if (c->timing) cudaEventRecord(c->ev[id][0], c->stream);
+    }
+    ~Phase()
+    {
+        if (c->timing) {
+            cudaEventRecord(c->ev[id][1], c->stream);
+            c->ev_set[id] = true;
+        }
+    }
+};
+
+bh_status fetch_state(bh_ctx *c)   // synchronising
+{
+    cudaError_t e = cudaMemcpyAsync(c->host_state, c->ws.st, sizeof(DevState), cudaMemcpyDeviceToHost, c->stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
+    if (e != cudaSuccess) return cuda_check(c, e, "state readback");
+    const int s = c->host_state->status;
+    if (s & kStatNonFinite) return fail(c, BH_ERR_NONFINITE, "a body coordinate is NaN or infinite");
+    if (s & kStatCapacity) return fail(c, BH_ERR_CAPACITY, "node array overflow");
+    if (s & kStatStack) return fail(c, BH_ERR_CAPACITY, "walk stack overflow");
+    return BH_OK;
+}
+
+bh_status do_build(bh_ctx *c, const double *pos, const double *mass, int64_t n)
+{
+    const Workspace &w = c->ws;
+    cudaStream_t s = c->stream;
+    c->built = false;
+    c->walked = false;
+    cudaMemsetAsync(w.zero_begin, 0, w.zero_bytes, s);
+    {
+        Phase p(c, 0);
+        launch_cube(w, pos, n, s);
+    }
+    {
+        Phase p(c, 1);
+        launch_keys(w, pos, n, s);
+    }
+    {
+        Phase p(c, 2);
+        launch_sort(w, n, s);
+    }
+    {
+        Phase p(c, 3);
+        launch_gather(w, pos, mass, n, s);
+    }
+    {
+        Phase p(c, 4);
+        launch_tree(w, n, c->leaf_cap, s);
+    }
+    {
+        Phase p(c, 5);
+        launch_monopoles(w, n, s);
+    }
+    bh_status st = cuda_check(c, cudaGetLastError(), "bh_build launch");
+    if (st != BH_OK) return st;
+    c->n = n;
+    c->built = true;
+    return BH_OK;
+}
+
+bh_status do_accel(bh_ctx *c, double theta, double eps, double G, double *acc)
+{
+    const Workspace &w = c->ws;
+    // reset the group queue and the counters of this evaluation
+    cudaMemsetAsync(&w.st->walk_queue, 0, sizeof(unsigned), c->stream);
+    cudaMemsetAsync(&w.st->stats[0], 0, 4 * sizeof(unsigned long long), c->stream);
+    {
+        Phase p(c, 6);
+        launch_walk(w, c->n, theta, eps, G, acc, c->stream);
+    }
+    bh_status st = cuda_check(c, cudaGetLastError(), "bh_accel launch");
+    if (st == BH_OK) c->walked = true;
+    return st;
+}
+
+}  // namespace
+
+namespace bh {
+
+Workspace carve(char *base, int64_t max_n, int leaf_cap)
+{
+    Workspace w{};
+    Carver cv{base};
+    const int64_t n = max_n;
+    w.node_cap = node_capacity(n, leaf_cap);
+    w.sort_tiles = (n + kSortTile - 1) / kSortTile;
+    w.tree_tiles = (n + kTreeTile - 1) / kTreeTile;
+    w.walk_warps = WalkConfig::kSMs * WalkConfig::kBlocksPerSM * WalkConfig::kWarpsPerBlock;
+    const int64_t groups = n;   // capacity: a group holds at least one body
+    w.st = cv.take<DevState>(1);
+    w.bbox_part = cv.take<double>(148 * 4 * 8);
+    // --- region cleared by one memset at every build ---
+    size_t z0 = cv.off;
+    w.hist = cv.take<unsigned>(kSortPasses * kRadix);
+    w.zero_begin = w.hist;
+    w.sort_ticket = cv.take<unsigned>(kSortPasses);
+    w.lookback = cv.take<unsigned>((size_t)kSortPasses * w.sort_tiles * kRadix);
+    w.node_meta = cv.take<unsigned>(w.node_cap);
+    w.zero_bytes = cv.off - z0;
+    // ---
+    w.key[0] = cv.take<unsigned long long>(n);
+    w.key[1] = cv.take<unsigned long long>(n);
+    w.idx[0] = cv.take<unsigned>(n);
+    w.idx[1] = cv.take<unsigned>(n);
+    w.iperm = cv.take<unsigned>(n);
+    w.sbody = cv.take<double4>(n);
+    w.gstart = cv.take<unsigned>(groups + 1);
+    w.gbox = cv.take<double>(6 * groups);
+    w.dlev = cv.take<uchar4>(n);
+    w.tile_lvl = cv.take<unsigned>((size_t)(kLevels + 1) * w.tree_tiles);
+    w.nlevel = cv.take<unsigned char>(w.node_cap);
+    w.nbegin = cv.take<unsigned>(w.node_cap);
+    w.ncount = cv.take<unsigned>(w.node_cap);
+    w.nfirst = cv.take<int>(w.node_cap);
+    w.nparent = cv.take<int>(w.node_cap);
+    w.mono = cv.take<double4>(w.node_cap);
+    w.cnt_mono = cv.take<unsigned>(groups);
+    w.cnt_direct = cv.take<unsigned>(groups);
+    w.walk_stack = cv.take<unsigned>((size_t)w.walk_warps * kStackSlab);
+    w.acc = cv.take<double>(3 * n);
+    w.stage_pos = cv.take<double>(3 * n);
+    w.stage_mass = cv.take<double>(n);
+    w.peak_sink = cv.take<double>(32);
+    w.total_bytes = cv.off;
+    return w;
+}
+
+}  // namespace bh
+
+extern "C" {
+
+const char *bh_version(void) { return "bh-b200 0.1 (sm_100a)"; }
+
+const char *bh_last_error(const bh_ctx *ctx) { return ctx ? ctx->err : g_err; }
+
+static bool args_ok(int64_t max_n, int leaf_cap, int group_size)
+{
+    return max_n >= 1 && max_n <= ((int64_t)1 << 30) && leaf_cap >= 1 && leaf_cap <= 1024 &&
+           (group_size == 0 || group_size == kGroup);
+}
+
+size_t bh_workspace_bytes(int64_t max_n, int leaf_cap, int group_size)
+{
+    if (!args_ok(max_n, leaf_cap, group_size)) return 0;
+    return carve(nullptr, max_n, leaf_cap).total_bytes;
+}
+
+bh_status bh_create(bh_ctx **out, int64_t max_n, int leaf_cap, int group_size, void *workspace_dev,
+                    size_t workspace_bytes, void *cuda_stream)
+{
+    if (!out) return fail(nullptr, BH_ERR_INVALID_ARG, "out is null");
+    *out = nullptr;
+    if (!args_ok(max_n, leaf_cap, group_size))
+        return fail(nullptr, BH_ERR_INVALID_ARG, "max_n, leaf_cap or group_size out of range");
+    if (!workspace_dev || ((uintptr_t)workspace_dev & 255))
+        return fail(nullptr, BH_ERR_INVALID_ARG, "workspace is null or not 256-byte aligned");
+    Workspace w = carve((char *)workspace_dev, max_n, leaf_cap);
+    if (workspace_bytes < w.total_bytes) return fail(nullptr, BH_ERR_CAPACITY, "workspace too small");
+    bh_ctx *c = new (std::nothrow) bh_ctx();
+    if (!c) return fail(nullptr, BH_ERR_CAPACITY, "out of host memory");
+    c->max_n = max_n;
+    c->leaf_cap = leaf_cap;
+    c->stream = (cudaStream_t)cuda_stream;
+    c->ws = w;
+    cudaError_t e = cudaMallocHost((void **)&c->host_state, sizeof(DevState));
+    if (e == cudaSuccess) e = cudaMemsetAsync(w.st, 0, sizeof(DevState), c->stream);
+    for (int p = 0; p < BH_NUM_PHASES && e == cudaSuccess; ++p) {
+        e = cudaEventCreate(&c->ev[p][0]);
+        if (e == cudaSuccess) e = cudaEventCreate(&c->ev[p][1]);
+    }
+    if (e != cudaSuccess) {
+        snprintf(g_err, 256, "bh_create: %s", cudaGetErrorString(e));
+        if (c->host_state) cudaFreeHost(c->host_state);
+        delete c;
+        return BH_ERR_CUDA;
+    }
+    *out = c;
+    return BH_OK;
+}
+
+bh_status bh_destroy(bh_ctx *c)
+{
+    if (!c) return BH_ERR_INVALID_ARG;
+    cudaStreamSynchronize(c->stream);
+    for (int p = 0; p < BH_NUM_PHASES; ++p) {
+        if (c->ev[p][0]) cudaEventDestroy(c->ev[p][0]);
+        if (c->ev[p][1]) cudaEventDestroy(c->ev[p][1]);
+    }
+    if (c->host_state) cudaFreeHost(c->host_state);
+    delete c;
+    return BH_OK;
+}
+
+bh_status bh_set_stream(bh_ctx *c, void *cuda_stream)
+{
+    if (!c) return BH_ERR_INVALID_ARG;
+    cudaStreamSynchronize(c->stream);
+    c->stream = (cudaStream_t)cuda_stream;
+    return BH_OK;
+}
+
+bh_status bh_build(bh_ctx *c, const double *pos_dev, const double *mass_dev, int64_t n)
+{
+    if (!c) return BH_ERR_INVALID_ARG;
+    if (!pos_dev || !mass_dev) return fail(c, BH_ERR_INVALID_ARG, "bh_build: null pointer");
+    if (n < 1 || n > c->max_n) return fail(c, BH_ERR_INVALID_ARG, "bh_build: n out of range");
+    return do_build(c, pos_dev, mass_dev, n);
+}
+
+bh_status bh_accel(bh_ctx *c, double theta, double eps, double G, double *acc_dev)
+{
+    if (!c) return BH_ERR_INVALID_ARG;
+    if (!c->built) return fail(c, BH_ERR_STATE, "bh_accel before bh_build");
+    if (!acc_dev) return fail(c, BH_ERR_INVALID_ARG, "bh_accel: null pointer");
+    if (!(theta >= 0.0) || !(eps >= 0.0)) return fail(c, BH_ERR_INVALID_ARG, "bh_accel: theta or eps negative");
+    return do_accel(c, theta, eps, G, acc_dev);
+}
+
+bh_status bh_direct(bh_ctx *c, double eps, double G, double *acc_dev)
+{
+    if (!c) return BH_ERR_INVALID_ARG;
+    if (!c->built) return fail(c, BH_ERR_STATE, "bh_direct before bh_build");
+    if (!acc_dev) return fail(c, BH_ERR_INVALID_ARG, "bh_direct: null pointer");
+    if (!(eps >= 0.0)) return fail(c, BH_ERR_INVALID_ARG, "bh_direct: eps negative");
+    {
+        Phase p(c, 7);
+        launch_direct(c->ws, c->n, nullptr, c->n, eps, G, acc_dev, c->stream);
+    }
+    return cuda_check(c, cudaGetLastError(), "bh_direct launch");
+}
+
+bh_status bh_direct_targets(bh_ctx *c, const int32_t *tgt_dev, int64_t nt, double eps, double G, double *acc_dev)
+{
+    if (!c) return BH_ERR_INVALID_ARG;
+    if (!c->built) return fail(c, BH_ERR_STATE, "bh_direct_targets before bh_build");
+    if (!acc_dev || !tgt_dev) return fail(c, BH_ERR_INVALID_ARG, "bh_direct_targets: null pointer");
+    if (nt < 1 || !(eps >= 0.0)) return fail(c, BH_ERR_INVALID_ARG, "bh_direct_targets: nt < 1 or eps negative");
+    {
+        Phase p(c, 7);
+        launch_direct(c->ws, c->n, tgt_dev, nt, eps, G, acc_dev, c->stream);
+    }
+    return cuda_check(c, cudaGetLastError(), "bh_direct_targets launch");
+}
+
+bh_status bh_bind_state(bh_ctx *c, double *pos_dev, double *vel_dev, const double *mass_dev, int64_t n,
+                        double theta, double eps, double G)
+{
+    if (!c) return BH_ERR_INVALID_ARG;
+    if (!pos_dev || !vel_dev || !mass_dev) return fail(c, BH_ERR_INVALID_ARG, "bh_bind_state: null pointer");
+    if (n < 1 || n > c->max_n) return fail(c, BH_ERR_INVALID_ARG, "bh_bind_state: n out of range");
+    if (!(theta >= 0.0) || !(eps >= 0.0)) return fail(c, BH_ERR_INVALID_ARG, "bh_bind_state: theta or eps negative");
+    c->pos = pos_dev;
+    c->vel = vel_dev;
+    c->mass = mass_dev;
+    c->bound_n = n;
+    c->theta = theta;
+    c->eps = eps;
+    c->G = G;
+    c->bound = true;
+    c->have_acc = false;
+    return BH_OK;
+}
+
+bh_status bh_kdk_step(bh_ctx *c, double dt)
+{
+    if (!c) return BH_ERR_INVALID_ARG;
+    if (!c->bound) return fail(c, BH_ERR_STATE, "bh_kdk_step before bh_bind_state");
+    bh_status st;
+    if (!c->have_acc) {   // a(x0), once
+        if ((st = do_build(c, c->pos, c->mass, c->bound_n)) != BH_OK) return st;
+        if ((st = do_accel(c, c->theta, c->eps, c->G, c->ws.acc)) != BH_OK) return st;
+        c->have_acc = true;
+    }
+    if (c->timing) cudaEventRecord(c->ev[8][0], c->stream);
+    launch_kick_drift(c->pos, c->vel, c->ws.acc, c->bound_n, dt, c->stream);
+    if (c->timing) {
+        cudaEventRecord(c->ev[8][1], c->stream);
+        c->ev_set[8] = true;
+    }
+    if ((st = do_build(c, c->pos, c->mass, c->bound_n)) != BH_OK) return st;
+    if ((st = do_accel(c, c->theta, c->eps, c->G, c->ws.acc)) != BH_OK) return st;
+    launch_kick(c->vel, c->ws.acc, c->bound_n, dt * 0.5, c->stream);
+    return cuda_check(c, cudaGetLastError(), "bh_kdk_step launch");
+}
+
+bh_status bh_get_state_acc(bh_ctx *c, const double **acc_dev)
+{
+    if (!c || !acc_dev) return BH_ERR_INVALID_ARG;
+    if (!c->bound || !c->have_acc) return fail(c, BH_ERR_STATE, "no accelerations yet");
+    *acc_dev = c->ws.acc;
+    return BH_OK;
+}
+
+bh_status bh_eval_host(bh_ctx *c, const double *pos_host, const double *mass_host, int64_t n, double theta,
+                       double eps, double G, double *acc_host)
+{
+    if (!c) return BH_ERR_INVALID_ARG;
+    if (!pos_host || !mass_host || !acc_host) return fail(c, BH_ERR_INVALID_ARG, "bh_eval_host: null pointer");
+    if (n < 1 || n > c->max_n) return fail(c, BH_ERR_INVALID_ARG, "bh_eval_host: n out of range");
+    if (!(theta >= 0.0) || !(eps >= 0.0)) return fail(c, BH_ERR_INVALID_ARG, "bh_eval_host: theta or eps negative");
+    const Workspace &w = c->ws;
+    cudaError_t e = cudaMemcpyAsync(w.stage_pos, pos_host, 3 * n * sizeof(double), cudaMemcpyHostToDevice, c->stream);
+    if (e == cudaSuccess)
+        e = cudaMemcpyAsync(w.stage_mass, mass_host, n * sizeof(double), cudaMemcpyHostToDevice, c->stream);
+    if (e != cudaSuccess) return cuda_check(c, e, "bh_eval_host H2D");
+    bh_status st;
+    if ((st = do_build(c, w.stage_pos, w.stage_mass, n)) != BH_OK) return st;
+    if ((st = do_accel(c, theta, eps, G, w.acc)) != BH_OK) return st;
+    c->have_acc = false;   // the internal acc buffer no longer belongs to the bound state
+    e = cudaMemcpyAsync(acc_host, w.acc, 3 * n * sizeof(double), cudaMemcpyDeviceToHost, c->stream);
+    if (e != cudaSuccess) return cuda_check(c, e, "bh_eval_host D2H");
+    return fetch_state(c);
+}
+
+bh_status bh_synchronize(bh_ctx *c)
+{
+    if (!c) return BH_ERR_INVALID_ARG;
+    return fetch_state(c);
+}
+
+bh_status bh_get_cube(bh_ctx *c, double lo_host[3], double *side_host)
+{
+    if (!c || !lo_host || !side_host) return BH_ERR_INVALID_ARG;
+    if (!c->built) return fail(c, BH_ERR_STATE, "no build yet");
+    bh_status st = fetch_state(c);
+    if (st != BH_OK) return st;
+    for (int a = 0; a < 3; ++a) lo_host[a] = c->host_state->lo[a];
+    *side_host = c->host_state->side;
+    return BH_OK;
+}
+
+bh_status bh_get_keys(bh_ctx *c, uint64_t *sorted_key_dev, uint32_t *perm_dev)
+{
+    if (!c) return BH_ERR_INVALID_ARG;
+    if (!c->built) return fail(c, BH_ERR_STATE, "no build yet");
+    cudaError_t e = cudaSuccess;
+    if (sorted_key_dev)
+        e = cudaMemcpyAsync(sorted_key_dev, c->ws.key[0], c->n * sizeof(uint64_t), cudaMemcpyDeviceToDevice, c->stream);
+    if (e == cudaSuccess && perm_dev)
+        e = cudaMemcpyAsync(perm_dev, c->ws.idx[0], c->n * sizeof(uint32_t), cudaMemcpyDeviceToDevice, c->stream);
+    return cuda_check(c, e, "bh_get_keys");
+}
+
+bh_status bh_get_node_count(bh_ctx *c, int64_t *m_host, int32_t *depth_host)
+{
+    if (!c || !m_host) return BH_ERR_INVALID_ARG;
+    if (!c->built) return fail(c, BH_ERR_STATE, "no build yet");
+    bh_status st = fetch_state(c);
+    if (st != BH_OK) return st;
+    *m_host = c->host_state->n_nodes;
+    if (depth_host) *depth_host = c->host_state->depth;
+    return BH_OK;
+}
+
+bh_status bh_get_nodes(bh_ctx *c, uint8_t *level, uint32_t *begin, uint32_t *count, int32_t *first_child,
+                       uint8_t *child_mask, int32_t *parent, double *mono)
+{
+    if (!c) return BH_ERR_INVALID_ARG;
+    if (!c->built) return fail(c, BH_ERR_STATE, "no build yet");
+    bh_status st = fetch_state(c);
+    if (st != BH_OK) return st;
+    const size_t M = (size_t)c->host_state->n_nodes;
+    const Workspace &w = c->ws;
+    cudaStream_t s = c->stream;
+    cudaError_t e = cudaSuccess;
+    auto cp = [&](void *dst, const void *src, size_t bytes) {
+        if (dst && e == cudaSuccess) e = cudaMemcpyAsync(dst, src, bytes, cudaMemcpyDeviceToDevice, s);
+    };
+    cp(level, w.nlevel, M);
+    cp(begin, w.nbegin, M * 4);
+    cp(count, w.ncount, M * 4);
+    cp(first_child, w.nfirst, M * 4);
+    cp(parent, w.nparent, M * 4);
+    cp(mono, w.mono, M * 32);
+    if (child_mask && e == cudaSuccess) {
+        launch_unpack_mask(w, child_mask, (int64_t)M, s);
+        e = cudaGetLastError();
+    }
+    return cuda_check(c, e, "bh_get_nodes");
+}
+
+bh_status bh_get_groups(bh_ctx *c, int64_t *ng_host, uint32_t *gstart_dev)
+{
+    if (!c || !ng_host) return BH_ERR_INVALID_ARG;
+    if (!c->built) return fail(c, BH_ERR_STATE, "no build yet");
+    bh_status st = fetch_state(c);
+    if (st != BH_OK) return st;
+    *ng_host = c->host_state->n_groups;
+    if (!gstart_dev) return BH_OK;
+    return cuda_check(c, cudaMemcpyAsync(gstart_dev, c->ws.gstart, (size_t)(*ng_host + 1) * 4,
+                                         cudaMemcpyDeviceToDevice, c->stream), "bh_get_groups");
+}
+
+bh_status bh_get_bodies(bh_ctx *c, double *sbody_dev, double *glo_dev, double *ghi_dev)
+{
+    if (!c) return BH_ERR_INVALID_ARG;
+    if (!c->built) return fail(c, BH_ERR_STATE, "no build yet");
+    bh_status st = fetch_state(c);
+    if (st != BH_OK) return st;
+    const int64_t groups = c->host_state->n_groups;
+    cudaError_t e = cudaSuccess;
+    if (sbody_dev)
+        e = cudaMemcpyAsync(sbody_dev, c->ws.sbody, c->n * 32, cudaMemcpyDeviceToDevice, c->stream);
+    if (glo_dev && e == cudaSuccess)
+        e = cudaMemcpy2DAsync(glo_dev, 24, c->ws.gbox, 48, 24, groups, cudaMemcpyDeviceToDevice, c->stream);
+    if (ghi_dev && e == cudaSuccess)
+        e = cudaMemcpy2DAsync(ghi_dev, 24, c->ws.gbox + 3, 48, 24, groups, cudaMemcpyDeviceToDevice, c->stream);
+    return cuda_check(c, e, "bh_get_bodies");
+}
+
+bh_status bh_get_counts(bh_ctx *c, uint32_t *n_mono_dev, uint32_t *n_direct_dev)
+{
+    if (!c) return BH_ERR_INVALID_ARG;
+    if (!c->walked) return fail(c, BH_ERR_STATE, "no bh_accel since the last build");
+    bh_status st = fetch_state(c);
+    if (st != BH_OK) return st;
+    const int64_t groups = c->host_state->n_groups;
+    cudaError_t e = cudaSuccess;
+    if (n_mono_dev)
+        e = cudaMemcpyAsync(n_mono_dev, c->ws.cnt_mono, groups * 4, cudaMemcpyDeviceToDevice, c->stream);
+    if (n_direct_dev && e == cudaSuccess)
+        e = cudaMemcpyAsync(n_direct_dev, c->ws.cnt_direct, groups * 4, cudaMemcpyDeviceToDevice, c->stream);
+    return cuda_check(c, e, "bh_get_counts");
+}
+
+bh_status bh_get_stats(bh_ctx *c, uint64_t stats_host[4])
+{
+    if (!c || !stats_host) return BH_ERR_INVALID_ARG;
+    if (!c->walked) return fail(c, BH_ERR_STATE, "no bh_accel since the last build");
+    bh_status st = fetch_state(c);
+    if (st != BH_OK) return st;
+    for (int k = 0; k < 4; ++k) stats_host[k] = c->host_state->stats[k];
+    return BH_OK;
+}
+
+bh_status bh_set_timing(bh_ctx *c, int enable)
+{
+    if (!c) return BH_ERR_INVALID_ARG;
+    c->timing = enable != 0;
+    for (int p = 0; p < BH_NUM_PHASES; ++p) c->ev_set[p] = false;
+    return BH_OK;
+}
+
+bh_status bh_get_phase_ms(bh_ctx *c, float ms_host[BH_NUM_PHASES])
+{
+    if (!c || !ms_host) return BH_ERR_INVALID_ARG;
+    cudaError_t e = cudaStreamSynchronize(c->stream);
+    if (e != cudaSuccess) return cuda_check(c, e, "bh_get_phase_ms");
+    for (int p = 0; p < BH_NUM_PHASES; ++p) {
+        ms_host[p] = 0.f;
+        if (c->ev_set[p]) cudaEventElapsedTime(&ms_host[p], c->ev[p][0], c->ev[p][1]);
+    }
+    return BH_OK;
+}
+
+bh_status bh_measure_fp64_peak(bh_ctx *c, double *tflops_host)
+{
+    if (!c || !tflops_host) return BH_ERR_INVALID_ARG;
+    *tflops_host = run_fp64_peak(c->ws, c->stream);
+    return cuda_check(c, cudaGetLastError(), "bh_measure_fp64_peak");
+}
+
+}  // extern "C"

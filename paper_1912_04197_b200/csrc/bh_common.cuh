@@ -1,0 +1,118 @@
+// bh_common.cuh — shared declarations of the CUDA path (device state, workspace layout, launchers).
+// Nothing here is shared with oracle/.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "bh.h"
+
+namespace bh {
+
+constexpr int kMaxLevel = BH_MAX_LEVEL;   // 21
+constexpr int kLevels = kMaxLevel + 1;    // levels 0..21
+constexpr int kGroup = 32;                // W: bodies per walk group = one warp
+constexpr int kGroupCell = BH_GROUP_CELL;           // Gc: groups never straddle a tree cell that holds <= Gc bodies
+constexpr int kRadixBits = 8;
+constexpr int kRadix = 1 << kRadixBits;   // 256 bins
+constexpr int kSortPasses = 8;            // 63 key bits
+constexpr int kSortThreads = 256;
+constexpr int kSortItems = 16;            // keys per thread
+constexpr int kSortTile = kSortThreads * kSortItems;   // 4096 keys per tile
+constexpr int kTreeTile = 1024;           // bodies per block in the tree kernels
+constexpr int kStackSlab = 22 * 256;      // walk: global spill entries per warp (bound: 256 per level)
+
+enum StatusBits : int { kStatNonFinite = 1, kStatCapacity = 2, kStatStack = 4 };
+
+// Device-resident state of one build; written by kernels, read by later kernels (no host round trip).
+struct DevState {
+    double lo[3];          // cube corner
+    double side;           // L = 2^e
+    double scale;          // 2^(21-e)
+    int e;                 // exponent of L
+    int status;            // StatusBits, sticky until the next bh_build
+    int n_nodes;           // M
+    int depth;             // deepest level
+    unsigned n_groups;     // Ng walk groups
+    unsigned lvl_start[kLevels + 1];   // first node id of each level (lvl_start[kLevels] = M)
+    unsigned ticket_bbox;  // last-block election
+    unsigned walk_queue;   // dynamic group counter of the walk
+    unsigned long long stats[4];       // n_mono, n_direct, interactions, nodes tested
+};
+
+// Pointers into the caller's workspace.
+struct Workspace {
+    DevState *st;
+    double *bbox_part;        // [bbox blocks][6]
+    unsigned *zero_begin;     // start of the region cleared at every build
+    unsigned *hist;           // [kSortPasses][256]
+    unsigned *sort_ticket;    // [kSortPasses]
+    unsigned *lookback;       // [kSortPasses][tiles][256]
+    unsigned *node_meta;      // [cap] bits 0-7 child mask, bits 8.. arrival counter
+    size_t zero_bytes;
+    unsigned long long *key[2];   // [n] double buffer
+    unsigned *idx[2];             // [n]
+    unsigned *iperm;              // [n] original index -> sorted position
+    double4 *sbody;               // [n] sorted (x,y,z,m)
+    unsigned *gstart;             // [Ng+1] first sorted body of each walk group (capacity n+1)
+    double *gbox;                 // [Ng][6] lo xyz, hi xyz (capacity n)
+    uchar4 *dlev;                 // [n] (first level this body starts a node at, its leaf level, group-start flag, group-cell level)
+    unsigned *tile_lvl;           // [kLevels+1][tree tiles] per-tile node counts (+ group starts), then exclusive bases
+    // nodes, SoA, ids in level/Morton order
+    unsigned char *nlevel;
+    unsigned *nbegin;
+    unsigned *ncount;
+    int *nfirst;
+    int *nparent;
+    double4 *mono;
+    unsigned *cnt_mono;           // [Ng] (capacity n)
+    unsigned *cnt_direct;         // [Ng]
+    unsigned *walk_stack;         // [walk warps][kStackSlab]
+    double *acc;                  // [n][3] internal accelerations (KDK state, host staging)
+    double *stage_pos;            // [n][3] host-call staging
+    double *stage_mass;           // [n]
+    double *peak_sink;            // fp64 microbenchmark sink
+    int64_t node_cap;
+    int64_t sort_tiles;
+    int64_t tree_tiles;
+    int walk_warps;
+    size_t total_bytes;
+};
+
+struct WalkConfig {
+    static constexpr int kWarpsPerBlock = 8;
+    static constexpr int kBlocksPerSM = 2;
+    static constexpr int kSMs = 148;
+};
+
+inline int64_t node_capacity(int64_t n, int leaf_cap) { return n + 21 * (n / (leaf_cap + 1)) + 1; }
+
+// carve the workspace; base may be nullptr to compute the size only
+Workspace carve(char *base, int64_t max_n, int leaf_cap);
+
+// launchers (each enqueues on `s`)
+void launch_cube(const Workspace &w, const double *pos, int64_t n, cudaStream_t s);
+void launch_keys(const Workspace &w, const double *pos, int64_t n, cudaStream_t s);
+void launch_sort(const Workspace &w, int64_t n, cudaStream_t s);   // result in key[0]/idx[0]
+void launch_gather(const Workspace &w, const double *pos, const double *mass, int64_t n, cudaStream_t s);
+void launch_tree(const Workspace &w, int64_t n, int leaf_cap, cudaStream_t s);
+void launch_monopoles(const Workspace &w, int64_t n, cudaStream_t s);
+void launch_walk(const Workspace &w, int64_t n, double theta, double eps, double G, double *acc, cudaStream_t s);
+void launch_direct(const Workspace &w, int64_t n, const int32_t *tgt, int64_t nt, double eps, double G,
+                   double *acc, cudaStream_t s);
+void launch_kick_drift(double *pos, double *vel, const double *acc, int64_t n, double dt, cudaStream_t s);
+void launch_kick(double *vel, const double *acc, int64_t n, double h, cudaStream_t s);
+void launch_unpack_mask(const Workspace &w, unsigned char *mask_out, int64_t cap, cudaStream_t s);
+double run_fp64_peak(const Workspace &w, cudaStream_t s);
+
+// ---- small device helpers ----
+__device__ __forceinline__ unsigned lane_id() { return threadIdx.x & 31u; }
+
+// common leading 3-bit digits of two 63-bit keys (bit 63 is 0 in both): 0..21
+__device__ __forceinline__ int common_levels(unsigned long long a, unsigned long long b)
+{
+    unsigned long long x = a ^ b;
+    if (x == 0ull) return kMaxLevel;
+    return (__clzll((long long)x) - 1) / 3;
+}
+
+}  // namespace bh

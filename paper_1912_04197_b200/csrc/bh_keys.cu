@@ -1,0 +1,171 @@
+// bh_keys.cu — step a1 (canonical bounding cube) and step a2 (63-bit Morton keys over
+// that cube, plus the digit histograms of all eight radix passes).  HBM-streaming kernels.
+#include "bh_common.cuh"
+
+namespace bh {
+
+constexpr int kCubeThreads = 192;   // multiple of 3: a thread always sees the same axis
+constexpr int kCubeMaxBlocks = 148 * 4;
+
+__device__ __forceinline__ bool nonfinite(double x)
+{
+    return (__double2hiint(x) & 0x7ff00000) == 0x7ff00000;
+}
+
+// One pass over the flat [3n] coordinate array; per-block partial (min, max, bad) to part[blk][8];
+// the last block to finish reduces the partials and derives the cube (R11): corner = per-axis
+// minimum, side = smallest power of two strictly above the largest extent (1 if the extent is 0).
+__global__ void __launch_bounds__(kCubeThreads) cube_kernel(const double *__restrict__ pos, long long n3,
+                                                            DevState *st, double *part)
+{
+    __shared__ double smn[kCubeThreads], smx[kCubeThreads];
+    __shared__ int sbad[kCubeThreads];
+    __shared__ bool is_last;
+    const int tid = threadIdx.x;
+    const long long stride = (long long)gridDim.x * kCubeThreads;
+    double mn = __longlong_as_double(0x7ff0000000000000ll), mx = -mn;
+    int bad = 0;
+    for (long long k = (long long)blockIdx.x * kCubeThreads + tid; k < n3; k += stride) {
+        double x = __ldg(pos + k);
+        bad |= nonfinite(x);
+        mn = fmin(mn, x);
+        mx = fmax(mx, x);
+    }
+    smn[tid] = mn;
+    smx[tid] = mx;
+    sbad[tid] = bad;
+    __syncthreads();
+    if (tid < 3) {
+        for (int k = tid + 3; k < kCubeThreads; k += 3) {
+            mn = fmin(mn, smn[k]);
+            mx = fmax(mx, smx[k]);
+        }
+        part[blockIdx.x * 8 + tid] = mn;
+        part[blockIdx.x * 8 + 3 + tid] = mx;
+    }
+    if (tid == 0) {
+        int b = 0;
+        for (int k = 0; k < kCubeThreads; ++k) b |= sbad[k];
+        part[blockIdx.x * 8 + 6] = b ? 1.0 : 0.0;
+    }
+    __threadfence();
+    __syncthreads();
+    if (tid == 0) is_last = (atomicAdd(&st->ticket_bbox, 1u) == gridDim.x - 1);
+    __syncthreads();
+    if (!is_last) return;
+    __threadfence();
+    // final reduction over blocks: thread t takes axis t%3 of blocks t/3, t/3+64, ...
+    const int axis = tid % 3;
+    mn = __longlong_as_double(0x7ff0000000000000ll);
+    mx = -mn;
+    bad = 0;
+    for (int b = tid / 3; b < (int)gridDim.x; b += kCubeThreads / 3) {
+        mn = fmin(mn, __ldcg(part + b * 8 + axis));
+        mx = fmax(mx, __ldcg(part + b * 8 + 3 + axis));
+        bad |= (__ldcg(part + b * 8 + 6) != 0.0);
+    }
+    smn[tid] = mn;
+    smx[tid] = mx;
+    sbad[tid] = bad;
+    __syncthreads();
+    if (tid == 0) {
+        double lo[3], hi[3];
+        for (int a = 0; a < 3; ++a) {
+            lo[a] = smn[a];
+            hi[a] = smx[a];
+        }
+        for (int k = 3; k < kCubeThreads; ++k) {
+            lo[k % 3] = fmin(lo[k % 3], smn[k]);
+            hi[k % 3] = fmax(hi[k % 3], smx[k]);
+        }
+        for (int k = 0; k < kCubeThreads; ++k) bad |= sbad[k];
+        double E = 0.0;
+        for (int a = 0; a < 3; ++a) E = fmax(E, __dsub_rn(hi[a], lo[a]));   // one rounding per extent
+        if (nonfinite(E)) bad = 1;
+        int e = 0;
+        if (bad) {   // keep every later kernel memory-safe; the error is reported by the host
+            lo[0] = lo[1] = lo[2] = 0.0;
+        } else if (E != 0.0) {
+            (void)frexp(E, &e);   // E = f 2^e, 1/2 <= f < 1  =>  2^(e-1) <= E < 2^e
+        }
+        st->lo[0] = lo[0];
+        st->lo[1] = lo[1];
+        st->lo[2] = lo[2];
+        st->e = e;
+        st->side = ldexp(1.0, e);
+        st->scale = ldexp(1.0, 21 - e);
+        st->status = bad ? kStatNonFinite : 0;
+        st->n_nodes = 0;
+        st->n_groups = 0;
+        st->depth = 0;
+        st->ticket_bbox = 0;
+        st->walk_queue = 0;
+        st->stats[0] = st->stats[1] = st->stats[2] = st->stats[3] = 0ull;
+    }
+}
+
+// spread the low 21 bits of v so that bit k lands on bit 3k
+__device__ __forceinline__ unsigned long long spread3(unsigned v)
+{
+    unsigned long long x = v & 0x1fffffu;
+    x = (x | (x << 32)) & 0x001f00000000ffffull;
+    x = (x | (x << 16)) & 0x001f0000ff0000ffull;
+    x = (x | (x << 8)) & 0x100f00f00f00f00full;
+    x = (x | (x << 4)) & 0x10c30c30c30c30c3ull;
+    x = (x | (x << 2)) & 0x1249249249249249ull;
+    return x;
+}
+
+__device__ __forceinline__ unsigned quantise(double x, double lo, double scale)
+{
+    // one rounded subtraction, exact power-of-two scaling, truncation (R11/R12); the clamp is a
+    // no-op for finite input (x - lo <= extent < L) and keeps non-finite input memory-safe
+    double d = __dmul_rn(__dsub_rn(x, lo), scale);
+    d = fmin(fmax(d, 0.0), 2097151.0);
+    return (unsigned)__double2uint_rz(d);
+}
+
+// keys + the 8 x 256 digit histograms (shared-memory atomics, flushed once per block)
+__global__ void __launch_bounds__(256) keys_kernel(const double *__restrict__ pos, long long n,
+                                                   const DevState *__restrict__ st,
+                                                   unsigned long long *__restrict__ key,
+                                                   unsigned *__restrict__ hist)
+{
+    __shared__ unsigned sh[kSortPasses * kRadix];
+    for (int k = threadIdx.x; k < kSortPasses * kRadix; k += blockDim.x) sh[k] = 0u;
+    __syncthreads();
+    const double lx = st->lo[0], ly = st->lo[1], lz = st->lo[2], sc = st->scale;
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n;
+         i += (long long)gridDim.x * blockDim.x) {
+        unsigned qx = quantise(__ldg(pos + 3 * i + 0), lx, sc);
+        unsigned qy = quantise(__ldg(pos + 3 * i + 1), ly, sc);
+        unsigned qz = quantise(__ldg(pos + 3 * i + 2), lz, sc);
+        unsigned long long k = spread3(qx) | (spread3(qy) << 1) | (spread3(qz) << 2);
+        key[i] = k;
+#pragma unroll
+        for (int p = 0; p < kSortPasses; ++p)
+            atomicAdd(&sh[p * kRadix + (unsigned)((k >> (p * kRadixBits)) & (kRadix - 1))], 1u);
+    }
+    __syncthreads();
+    for (int k = threadIdx.x; k < kSortPasses * kRadix; k += blockDim.x)
+        if (sh[k]) atomicAdd(&hist[k], sh[k]);
+}
+
+void launch_cube(const Workspace &w, const double *pos, int64_t n, cudaStream_t s)
+{
+    long long n3 = 3 * (long long)n;
+    int blocks = (int)((n3 + kCubeThreads * 8 - 1) / (kCubeThreads * 8));
+    if (blocks > kCubeMaxBlocks) blocks = kCubeMaxBlocks;
+    if (blocks < 1) blocks = 1;
+    cube_kernel<<<blocks, kCubeThreads, 0, s>>>(pos, n3, w.st, w.bbox_part);
+}
+
+void launch_keys(const Workspace &w, const double *pos, int64_t n, cudaStream_t s)
+{
+    int blocks = (int)((n + 256 * 4 - 1) / (256 * 4));
+    if (blocks > 148 * 8) blocks = 148 * 8;
+    if (blocks < 1) blocks = 1;
+    keys_kernel<<<blocks, 256, 0, s>>>(pos, n, w.st, w.key[0], w.hist);
+}
+
+}  // namespace bh

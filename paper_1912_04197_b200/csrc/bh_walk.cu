@@ -1,0 +1,396 @@
+// bh_walk.cu — step a7 (group-cooperative tree walk, Eqs. (3)-(6) PAPER.md:84-106), step a8 (direct
+// N^2 sum, Eq. (1)), step a9 (leapfrog kernels) and the fp64 peak microbenchmark.
+//
+// Walk: one warp owns a group of up to 32 Morton-consecutive bodies of one group cell (R6).  Traversal and evaluation
+// alternate inside the warp:
+//   traverse  lanes = candidate nodes.  The warp pops up to 32 node ids from a LIFO stack (top part
+//             in shared memory, spill slab in global memory), each lane applies the opening test
+//             of the GROUP (R3-R7: node edge s, distance from the node's centre of mass to the
+//             group's bounding box, accept iff s*s < theta^2 d^2, never accept a node that holds a
+//             body of the group), and the results are appended by ballot/prefix: accepted nodes ->
+//             their (cx,cy,cz,m) into the shared source list; opened internal nodes -> their
+//             children onto the stack; opened leaves -> their bodies (x,y,z,m) into the same list.
+//   evaluate  lanes = bodies.  Whenever the list holds a full chunk, every lane reads the chunk's
+//             sources by shared-memory broadcast and accumulates m d / (|d|^2+eps^2)^(3/2) in fp64.
+// The test arithmetic is the canonical one (each operation rounded once, fma where stated) so that
+// every accept/open decision equals the oracle's; the accumulation order is free.
+#include "bh_common.cuh"
+
+namespace bh {
+
+constexpr int kWalkWarps = WalkConfig::kWarpsPerBlock;
+constexpr int kChunk = 64;                  // sources evaluated per flush
+constexpr int kListCap = 2 * kChunk;        // ring capacity (sources); append adds <= 32 at a time
+constexpr int kStackSmem = 768;             // node ids kept in shared memory per warp
+constexpr int kSpill = 256;                 // spill / refill unit
+
+// 1/sqrt(x) for normal positive x: MUFU.RSQ64H seed (about 20 good bits) and one third-order step.
+__device__ __forceinline__ double rsqrt_fast(double x)
+{
+    double y;
+    asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+    double t = x * y;
+    double e = fma(-t, y, 1.0);                 // 1 - x y^2
+    double p = fma(0.375, e, 0.5);
+    double q = e * p;                           // e/2 + 3 e^2/8
+    return fma(y, q, y);
+}
+
+// accumulate the pull of one source (sx,sy,sz,sm) on the body at (px,py,pz)
+__device__ __forceinline__ void interact(double px, double py, double pz, double eps2, const double4 s,
+                                         double &ax, double &ay, double &az)
+{
+    const double dx = s.x - px, dy = s.y - py, dz = s.z - pz;
+    const double r2 = fma(dx, dx, fma(dy, dy, fma(dz, dz, eps2)));
+    double y = rsqrt_fast(r2);
+    y = (r2 > 0.0) ? y : 0.0;                   // R13: a pair at zero softened distance adds nothing
+    const double y2 = y * y;
+    const double f = (s.w * y) * y2;
+    ax = fma(f, dx, ax);
+    ay = fma(f, dy, ay);
+    az = fma(f, dz, az);
+}
+
+struct WalkSmem {
+    double4 src[kWalkWarps][kListCap];
+    unsigned stack[kWalkWarps][kStackSmem];
+};
+
+__device__ __forceinline__ void eval_range(const double4 *src, int first, int count, double px, double py,
+                                           double pz, double eps2, double &ax, double &ay, double &az)
+{
+    int i = 0;
+#pragma unroll 1
+    for (; i + 4 <= count; i += 4) {
+        const double4 s0 = src[(first + i) & (kListCap - 1)];
+        const double4 s1 = src[(first + i + 1) & (kListCap - 1)];
+        const double4 s2 = src[(first + i + 2) & (kListCap - 1)];
+        const double4 s3 = src[(first + i + 3) & (kListCap - 1)];
+        interact(px, py, pz, eps2, s0, ax, ay, az);
+        interact(px, py, pz, eps2, s1, ax, ay, az);
+        interact(px, py, pz, eps2, s2, ax, ay, az);
+        interact(px, py, pz, eps2, s3, ax, ay, az);
+    }
+    for (; i < count; ++i) interact(px, py, pz, eps2, src[(first + i) & (kListCap - 1)], ax, ay, az);
+}
+
+__global__ void __launch_bounds__(kWalkWarps * 32, WalkConfig::kBlocksPerSM)
+walk_kernel(DevState *st, const unsigned *__restrict__ gstart, const double4 *__restrict__ sbody,
+            const double *__restrict__ gbox,
+            const unsigned *__restrict__ perm, const unsigned char *__restrict__ nlevel,
+            const unsigned *__restrict__ nbegin, const unsigned *__restrict__ ncount,
+            const int *__restrict__ nfirst, const unsigned *__restrict__ node_meta,
+            const double4 *__restrict__ mono, double theta2, double eps2, double G, double *__restrict__ acc,
+            unsigned *__restrict__ cnt_mono, unsigned *__restrict__ cnt_direct, unsigned *walk_stack)
+{
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    WalkSmem &sm = *reinterpret_cast<WalkSmem *>(smem_raw);
+    const unsigned lane = lane_id(), warp = threadIdx.x >> 5;
+    const unsigned lt = (1u << lane) - 1u;
+    double4 *src = sm.src[warp];
+    unsigned *stack = sm.stack[warp];
+    unsigned *slab = walk_stack + (size_t)(blockIdx.x * kWalkWarps + warp) * kStackSlab;
+    const unsigned ngroups = st->n_groups;
+    const int e2 = 2 * st->e;
+    unsigned long long tot_mono = 0, tot_direct = 0, tot_inter = 0, tot_tested = 0;
+
+    while (true) {
+        unsigned g = 0;
+        if (lane == 0) g = atomicAdd(&st->walk_queue, 1u);
+        g = __shfl_sync(0xffffffffu, g, 0);
+        if (g >= ngroups) break;
+        const long long gb = gstart[g];
+        const long long ge = gstart[g + 1];
+        const long long j = gb + lane;
+        const bool valid = j < ge;
+        const double4 me = sbody[valid ? j : gb];
+        const double px = me.x, py = me.y, pz = me.z;
+        const double glx = gbox[6 * g + 0], gly = gbox[6 * g + 1], glz = gbox[6 * g + 2];
+        const double ghx = gbox[6 * g + 3], ghy = gbox[6 * g + 4], ghz = gbox[6 * g + 5];
+        double ax = 0.0, ay = 0.0, az = 0.0;
+        int head = 0, tail = 0;        // ring [head, tail) of pending sources
+        int sp = 1, gsp = 0;           // shared stack size, spilled entries in the slab
+        unsigned n_mono = 0, n_direct = 0, n_tested = 0;
+        if (lane == 0) stack[0] = 0u;  // the root
+        __syncwarp();
+
+        while (sp > 0 || gsp > 0) {
+            if (sp == 0) {             // refill from the slab
+                gsp -= kSpill;
+                for (int k = lane; k < kSpill; k += 32) stack[k] = slab[gsp + k];
+                sp = kSpill;
+                __syncwarp();
+            }
+            const int take = sp < 32 ? sp : 32;
+            sp -= take;
+            const bool have = (int)lane < take;
+            unsigned t = 0;
+            if (have) t = stack[sp + lane];
+            __syncwarp();
+            n_tested += take;
+            // ---- opening test (canonical arithmetic) ----
+            bool accept = false, open_internal = false, open_leaf = false;
+            unsigned b = 0, c = 0, nch = 0;
+            int fc = -1;
+            double4 mn = make_double4(0.0, 0.0, 0.0, 0.0);
+            if (have) {
+                b = nbegin[t];
+                c = ncount[t];
+                fc = nfirst[t];
+                mn = mono[t];
+                const bool overlap = ((long long)b < ge) && (gb < (long long)b + c);
+                if (!overlap) {
+                    const double dx = fmax(fmax(__dsub_rn(glx, mn.x), __dsub_rn(mn.x, ghx)), 0.0);
+                    const double dy = fmax(fmax(__dsub_rn(gly, mn.y), __dsub_rn(mn.y, ghy)), 0.0);
+                    const double dz = fmax(fmax(__dsub_rn(glz, mn.z), __dsub_rn(mn.z, ghz)), 0.0);
+                    const double d2 = __fma_rn(dz, dz, __fma_rn(dy, dy, __dmul_rn(dx, dx)));
+                    const int lv = nlevel[t];
+                    const double s2 = __hiloint2double((e2 - 2 * lv + 1023) << 20, 0);   // (L 2^-lv)^2
+                    accept = s2 < __dmul_rn(theta2, d2);
+                }
+                if (!accept) {
+                    if (fc >= 0) {
+                        open_internal = true;
+                        nch = __popc(node_meta[t] & 0xffu);
+                    } else {
+                        open_leaf = true;
+                    }
+                }
+            }
+            // ---- accepted nodes -> source list ----
+            {
+                const unsigned m = __ballot_sync(0xffffffffu, accept);
+                if (accept) src[(tail + __popc(m & lt)) & (kListCap - 1)] = mn;
+                const int k = __popc(m);
+                tail += k;
+                n_mono += k;
+            }
+            // ---- opened internal nodes -> children onto the stack ----
+            {
+                unsigned inc = nch;
+#pragma unroll
+                for (int o = 1; o < 32; o <<= 1) {
+                    unsigned u = __shfl_up_sync(0xffffffffu, inc, o);
+                    if (lane >= (unsigned)o) inc += u;
+                }
+                const int total = __shfl_sync(0xffffffffu, inc, 31);
+                if (sp + total > kStackSmem) {        // spill the oldest kSpill entries
+                    for (int k = lane; k < kSpill; k += 32) slab[gsp + k] = stack[k];
+                    gsp += kSpill;
+                    __syncwarp();
+                    for (int k0 = 0; k0 < sp - kSpill; k0 += 32) {
+                        unsigned v = 0;
+                        if (k0 + (int)lane < sp - kSpill) v = stack[kSpill + k0 + lane];
+                        __syncwarp();
+                        if (k0 + (int)lane < sp - kSpill) stack[k0 + lane] = v;
+                        __syncwarp();
+                    }
+                    sp -= kSpill;
+                }
+                if (open_internal) {
+                    const int off = sp + (int)(inc - nch);
+                    for (unsigned u = 0; u < nch; ++u) stack[off + u] = (unsigned)fc + u;
+                }
+                sp += total;
+                __syncwarp();
+            }
+            // ---- opened leaves -> their bodies into the source list ----
+            {
+                unsigned lc = open_leaf ? c : 0u;
+                unsigned inc = lc;
+#pragma unroll
+                for (int o = 1; o < 32; o <<= 1) {
+                    unsigned u = __shfl_up_sync(0xffffffffu, inc, o);
+                    if (lane >= (unsigned)o) inc += u;
+                }
+                const unsigned total = __shfl_sync(0xffffffffu, inc, 31);
+                n_direct += total;
+                for (unsigned base = 0; base < total; base += 32) {
+                    // make room first: a full chunk is evaluated as soon as it exists
+                    while (tail - head >= kChunk) {
+                        __syncwarp();
+                        eval_range(src, head, kChunk, px, py, pz, eps2, ax, ay, az);
+                        head += kChunk;
+                        __syncwarp();
+                    }
+                    const unsigned idx = base + lane;
+                    // owner lane = first lane whose inclusive count exceeds idx (binary search by shuffles)
+                    unsigned lo = 0;
+#pragma unroll
+                    for (int step = 16; step > 0; step >>= 1) {
+                        unsigned probe = __shfl_sync(0xffffffffu, inc, lo + step - 1);
+                        if (probe <= idx) lo += step;
+                    }
+                    lo = lo > 31u ? 31u : lo;
+                    const unsigned oinc = __shfl_sync(0xffffffffu, inc, lo);
+                    const unsigned ocnt = __shfl_sync(0xffffffffu, lc, lo);
+                    const unsigned obeg = __shfl_sync(0xffffffffu, b, lo);
+                    if (idx < total) {
+                        const unsigned body = obeg + (idx - (oinc - ocnt));
+                        src[(tail + lane) & (kListCap - 1)] = sbody[body];
+                    }
+                    const unsigned got = total - base < 32u ? total - base : 32u;
+                    tail += (int)got;
+                }
+            }
+            while (tail - head >= kChunk) {
+                __syncwarp();
+                eval_range(src, head, kChunk, px, py, pz, eps2, ax, ay, az);
+                head += kChunk;
+                __syncwarp();
+            }
+        }
+        __syncwarp();
+        eval_range(src, head, tail - head, px, py, pz, eps2, ax, ay, az);
+        __syncwarp();
+        if (valid) {
+            const unsigned i = perm[j];
+            acc[3ll * i + 0] = G * ax;
+            acc[3ll * i + 1] = G * ay;
+            acc[3ll * i + 2] = G * az;
+        }
+        if (lane == 0) {
+            cnt_mono[g] = n_mono;
+            cnt_direct[g] = n_direct;
+        }
+        tot_mono += n_mono;
+        tot_direct += n_direct;
+        tot_inter += (unsigned long long)(n_mono + n_direct) * (unsigned long long)(ge - gb);
+        tot_tested += n_tested;
+    }
+    if (lane == 0) {
+        atomicAdd(&st->stats[0], tot_mono);
+        atomicAdd(&st->stats[1], tot_direct);
+        atomicAdd(&st->stats[2], tot_inter);
+        atomicAdd(&st->stats[3], tot_tested);
+    }
+}
+
+// ------------------------------------------------------------------------------------------ a8
+// Direct sum: one target per thread, sources streamed through shared-memory tiles.
+constexpr int kDirectThreads = 256;
+
+__global__ void __launch_bounds__(kDirectThreads)
+direct_kernel(long long n, const double4 *__restrict__ sbody, const unsigned *__restrict__ perm,
+              const unsigned *__restrict__ iperm, const int32_t *__restrict__ tgt, long long nt, double eps2,
+              double G, double *__restrict__ acc)
+{
+    __shared__ double4 tile[kDirectThreads];
+    const long long r = (long long)blockIdx.x * kDirectThreads + threadIdx.x;
+    const bool valid = r < nt;
+    // all bodies: row r is sorted body r, written to its original index; sampled: row r is target tgt[r]
+    long long jme = 0;
+    if (valid) jme = tgt ? (long long)iperm[tgt[r]] : r;
+    const double4 me = sbody[jme];
+    double ax = 0.0, ay = 0.0, az = 0.0;
+    for (long long t0 = 0; t0 < n; t0 += kDirectThreads) {
+        const long long k = t0 + threadIdx.x;
+        tile[threadIdx.x] = k < n ? sbody[k] : make_double4(0.0, 0.0, 0.0, 0.0);   // zero mass: no pull
+        __syncthreads();
+#pragma unroll 4
+        for (int q = 0; q < kDirectThreads; ++q) interact(me.x, me.y, me.z, eps2, tile[q], ax, ay, az);
+        __syncthreads();
+    }
+    if (valid) {
+        const long long o = tgt ? r : (long long)perm[r];
+        acc[3 * o + 0] = G * ax;
+        acc[3 * o + 1] = G * ay;
+        acc[3 * o + 2] = G * az;
+    }
+}
+
+// ------------------------------------------------------------------------------------------ a9
+__global__ void kick_drift_kernel(double *__restrict__ pos, double *__restrict__ vel, const double *__restrict__ acc,
+                                  long long n3, double h, double dt)
+{
+    for (long long k = (long long)blockIdx.x * blockDim.x + threadIdx.x; k < n3;
+         k += (long long)gridDim.x * blockDim.x) {
+        const double v = __fma_rn(acc[k], h, vel[k]);
+        vel[k] = v;
+        pos[k] = __fma_rn(v, dt, pos[k]);
+    }
+}
+
+__global__ void kick_kernel(double *__restrict__ vel, const double *__restrict__ acc, long long n3, double h)
+{
+    for (long long k = (long long)blockIdx.x * blockDim.x + threadIdx.x; k < n3;
+         k += (long long)gridDim.x * blockDim.x)
+        vel[k] = __fma_rn(acc[k], h, vel[k]);
+}
+
+// ------------------------------------------------------------------------------------------ fp64 peak
+__global__ void __launch_bounds__(256) fp64_peak_kernel(double *sink, int iters, double seed)
+{
+    double a0 = seed + threadIdx.x, a1 = a0 + 1, a2 = a0 + 2, a3 = a0 + 3, a4 = a0 + 4, a5 = a0 + 5, a6 = a0 + 6,
+           a7 = a0 + 7;
+    const double m = 0.999999, c = 1e-9;
+    for (int i = 0; i < iters; ++i) {
+        a0 = fma(a0, m, c); a1 = fma(a1, m, c); a2 = fma(a2, m, c); a3 = fma(a3, m, c);
+        a4 = fma(a4, m, c); a5 = fma(a5, m, c); a6 = fma(a6, m, c); a7 = fma(a7, m, c);
+    }
+    double s = a0 + a1 + a2 + a3 + a4 + a5 + a6 + a7;
+    if (s == 123456.789) sink[0] = s;
+}
+
+// ------------------------------------------------------------------------------------------ launchers
+void launch_walk(const Workspace &w, int64_t n, double theta, double eps, double G, double *acc, cudaStream_t s)
+{
+    static bool configured = false;
+    if (!configured) {
+        cudaFuncSetAttribute(walk_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(WalkSmem));
+        configured = true;
+    }
+    const int blocks = w.walk_warps / kWalkWarps;
+    walk_kernel<<<blocks, kWalkWarps * 32, sizeof(WalkSmem), s>>>(
+        w.st, w.gstart, w.sbody, w.gbox, w.idx[0], w.nlevel, w.nbegin, w.ncount, w.nfirst, w.node_meta, w.mono,
+        theta * theta, eps * eps, G, acc, w.cnt_mono, w.cnt_direct, w.walk_stack);
+}
+
+void launch_direct(const Workspace &w, int64_t n, const int32_t *tgt, int64_t nt, double eps, double G,
+                   double *acc, cudaStream_t s)
+{
+    const int64_t rows = tgt ? nt : n;
+    const int blocks = (int)((rows + kDirectThreads - 1) / kDirectThreads);
+    direct_kernel<<<blocks, kDirectThreads, 0, s>>>(n, w.sbody, w.idx[0], w.iperm, tgt, rows, eps * eps, G, acc);
+}
+
+void launch_kick_drift(double *pos, double *vel, const double *acc, int64_t n, double dt, cudaStream_t s)
+{
+    const long long n3 = 3ll * n;
+    int blocks = (int)((n3 + 1023) / 1024);
+    if (blocks > 148 * 8) blocks = 148 * 8;
+    kick_drift_kernel<<<blocks, 256, 0, s>>>(pos, vel, acc, n3, dt * 0.5, dt);
+}
+
+void launch_kick(double *vel, const double *acc, int64_t n, double h, cudaStream_t s)
+{
+    const long long n3 = 3ll * n;
+    int blocks = (int)((n3 + 1023) / 1024);
+    if (blocks > 148 * 8) blocks = 148 * 8;
+    kick_kernel<<<blocks, 256, 0, s>>>(vel, acc, n3, h);
+}
+
+double run_fp64_peak(const Workspace &w, cudaStream_t s)
+{
+    const int iters = 1 << 16, blocks = 148 * 8, threads = 256;
+    cudaEvent_t a, b;
+    cudaEventCreate(&a);
+    cudaEventCreate(&b);
+    fp64_peak_kernel<<<blocks, threads, 0, s>>>(w.peak_sink, 1 << 10, 1.0);   // warm-up
+    float best = 1e30f;
+    for (int rep = 0; rep < 3; ++rep) {
+        cudaEventRecord(a, s);
+        fp64_peak_kernel<<<blocks, threads, 0, s>>>(w.peak_sink, iters, 1.0);
+        cudaEventRecord(b, s);
+        cudaEventSynchronize(b);
+        float ms = 0.f;
+        cudaEventElapsedTime(&ms, a, b);
+        if (ms < best) best = ms;
+    }
+    cudaEventDestroy(a);
+    cudaEventDestroy(b);
+    const double flops = 2.0 * 8.0 * (double)iters * (double)blocks * (double)threads;
+    return flops / (best * 1e-3) / 1e12;
+}
+
+}  // namespace bh

@@ -31,13 +31,13 @@ def main():
     acc, nm, nd, _ = orc.accel(t, w.theta, w.eps, w.G)
     ad = orc.direct(w.pos, w.mass, w.eps, w.G)
     out = {
-        "config": "c1: N=1024 uniform unit ball, m=1/N, G=1, eps=1e-3, theta=0.5, C=8, W=32",
+        "config": "c1: N=1024 uniform unit ball, m=1/N, G=1, eps=1e-3, theta=0.5, C=8, W=32, Gc=512",
         "pos_sha256": sha(w.pos), "lo_hex": [float(x).hex() for x in t.lo], "L": t.L,
         "M": t.M, "depth": t.depth, "nodes_per_level": np.bincount(t.level).tolist(),
         "key_sha256": sha(t.key), "perm_sha256": sha(t.perm),
         "topology_sha256": sha(np.concatenate([t.level.astype(np.int64), t.begin, t.count, t.first_child,
                                                t.child_mask, t.parent]).astype(np.int64)),
-        "mono_sha256": sha(t.mono),
+        "mono_sha256": sha(t.mono), "n_groups": t.ngroups, "gstart_sha256": sha(t.gstart),
         "n_mono_sum": int(nm.sum()), "n_direct_sum": int(nd.sum()),
         "acc_first3_hex": [[float(x).hex() for x in r] for r in acc[:3]],
         "direct_first3_hex": [[float(x).hex() for x in r] for r in ad[:3]],

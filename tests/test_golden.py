@@ -19,6 +19,7 @@ def test_c1_fixture():
     assert np.bincount(t.level).tolist() == g["nodes_per_level"]
     assert sha(t.key) == g["key_sha256"] and sha(t.perm) == g["perm_sha256"]
     assert sha(t.mono) == g["mono_sha256"]
+    assert t.ngroups == g["n_groups"] and sha(t.gstart) == g["gstart_sha256"]
     acc, nm, nd, _ = orc.accel(t, w.theta, w.eps, w.G)
     assert (int(nm.sum()), int(nd.sum())) == (g["n_mono_sum"], g["n_direct_sum"])
     ref = np.array([[float.fromhex(x) for x in r] for r in g["acc_first3_hex"]])

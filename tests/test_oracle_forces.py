@@ -69,14 +69,55 @@ def test_monopole_fixed_order_arithmetic_exact():
         assert list(t.mono[i, :3]) == [ws[a] / m for a in range(3)]
 
 
-def test_group_boxes():
-    w = wl.make("c1", 1000)
-    t = orc.build(w.pos, w.mass, 8, W=32)
-    assert t.ngroups == 32
+def _group_cells_by_search(skey, leaf_cap, Gc):
+    """Independent derivation of the group cells (O7): for every sorted body, by binary search on
+    the keys, the shallowest cell that holds <= Gc bodies, but never deeper than the body's leaf."""
+    n = len(skey)
+    cells = set()
+    for j in range(n):
+        for lvl in range(22):
+            sh = 63 - 3 * lvl
+            pre = int(skey[j]) >> sh if lvl else 0
+            lo = int(np.searchsorted(skey, np.uint64(pre << sh), side="left")) if lvl else 0
+            hi = int(np.searchsorted(skey, np.uint64(((pre + 1) << sh) - 1), side="right")) if lvl else n
+            cnt = hi - lo
+            if cnt <= Gc or cnt <= leaf_cap or lvl == 21:
+                cells.add((lo, hi))
+                break
+    return sorted(cells)
+
+
+@pytest.mark.parametrize("name,n,C,W,Gc", [("c1", 1000, 8, 32, 512), ("c4", 3000, 16, 32, 64),
+                                           ("c4", 3000, 4, 8, 20), ("c2", 700, 16, 32, 8), ("c1", 300, 8, 32, 512)])
+def test_groups_partition_group_cells(name, n, C, W, Gc):
+    w = wl.make(name, n)
+    t = orc.build(w.pos, w.mass, C, W=W, Gc=Gc)
+    cells = _group_cells_by_search(t.skey, C, Gc)
+    assert cells[0][0] == 0 and cells[-1][1] == n
+    assert all(a[1] == b[0] for a, b in zip(cells, cells[1:]))          # the cells tile [0, n)
+    expect = [j for lo, hi in cells for j in range(lo, hi, W)] + [n]    # runs of W inside each cell
+    assert t.gstart.tolist() == expect
+    sizes = np.diff(t.gstart.astype(np.int64))
+    assert sizes.min() >= 1 and sizes.max() <= W
     for g in range(t.ngroups):
-        sl = t.sbody[g * 32:min(1000, g * 32 + 32), :3]
+        sl = t.sbody[t.gstart[g]:t.gstart[g + 1], :3]
         assert np.array_equal(t.glo[g], sl.min(axis=0)) and np.array_equal(t.ghi[g], sl.max(axis=0))
     assert np.array_equal(t.sbody[:, :3], w.pos[t.perm]) and np.array_equal(t.sbody[:, 3], w.mass[t.perm])
+
+
+def test_groups_degenerate():
+    # n <= Gc: the root is the only group cell; coincident bodies beyond Gc: the level-21 leaf is one
+    w = wl.make("c1", 100)
+    t = orc.build(w.pos, w.mass, 8, W=32, Gc=512)
+    assert t.gstart.tolist() == [0, 32, 64, 96, 100]
+    pos = np.concatenate([np.full((50, 3), 0.25), np.random.default_rng(1).random((30, 3))])
+    t = orc.build(pos, np.ones(80), 4, W=8, Gc=16)
+    deep = int(np.flatnonzero(t.level == 21)[0])
+    b = int(t.begin[deep])
+    assert t.count[deep] == 50
+    assert [x for x in t.gstart.tolist() if b <= x < b + 50] == list(range(b, b + 50, 8))
+    t1 = orc.build(w.pos, w.mass, 8, W=1)
+    assert t1.gstart.tolist() == list(range(101))                       # W = 1: one body per group
 
 
 # ------------------------------------------------------------------ O8 walk structure
@@ -92,7 +133,7 @@ def test_walk_lists_cover_every_source_exactly_once(theta):
         np.add.at(seen, ld, 1)
         assert (seen == 1).all()
         # R7: no accepted node holds a body of the group
-        gb, ge = g * 32, min(t.n, g * 32 + 32)
+        gb, ge = int(t.gstart[g]), int(t.gstart[g + 1])
         assert all(t.begin[x] >= ge or t.begin[x] + t.count[x] <= gb for x in lm)
         if theta == 0.0:
             assert len(lm) == 0 and len(ld) == t.n
@@ -337,8 +378,9 @@ def test_group_walk_is_at_least_as_accurate_as_per_body_walk():
     a32, nm32, nd32, _ = orc.accel(t32, 0.5, w.eps, w.G)
     a1, nm1, nd1, _ = orc.accel(t1, 0.5, w.eps, w.G)
     assert np.median(relerr(a32, ref)) <= np.median(relerr(a1, ref))
-    per_body_1 = (nm1.astype(np.int64) + nd1)[np.argsort(np.argsort(t1.perm))]   # not needed sorted
-    assert (nm32.astype(np.int64) + nd32).mean() >= per_body_1.mean()
+    # interactions per body: every body of a group pays the group's list
+    per_body_32 = np.repeat(nm32.astype(np.int64) + nd32, np.diff(t32.gstart.astype(np.int64)))
+    assert per_body_32.mean() >= (nm1.astype(np.int64) + nd1).mean()
 
 
 # ------------------------------------------------------------------ O11 leapfrog
