@@ -125,6 +125,9 @@ bh_status bh_get_counts(bh_ctx *ctx, uint32_t *n_mono_per_group_dev, uint32_t *n
  * stats[3] = nodes tested by the opening criterion. */
 bh_status bh_get_stats(bh_ctx *ctx, uint64_t stats_host[4]);
 
+/* Number of CUDA kernels this context has launched since bh_create (memsets and copies excluded). */
+bh_status bh_get_launches(bh_ctx *ctx, uint64_t *count_host);
+
 /* Phase timing with CUDA events on the context's stream.  After bh_set_timing(ctx, 1) every
  * bh_build/bh_accel/bh_direct records events; bh_get_phase_ms (synchronising) returns the last
  * durations in ms: [0] cube, [1] keys+histogram, [2] sort, [3] gather+boxes, [4] tree,

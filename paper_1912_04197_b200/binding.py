@@ -61,6 +61,7 @@ def lib() -> C.CDLL:
             "bh_get_bodies": [vp, vp, vp, vp],
             "bh_get_counts": [vp, vp, vp],
             "bh_get_stats": [vp, C.POINTER(C.c_uint64)],
+            "bh_get_launches": [vp, C.POINTER(C.c_uint64)],
             "bh_set_timing": [vp, i32],
             "bh_get_phase_ms": [vp, C.POINTER(C.c_float)],
             "bh_measure_fp64_peak": [vp, C.POINTER(dbl)],
@@ -76,7 +77,8 @@ def lib() -> C.CDLL:
 EXPORTS = ("bh_workspace_bytes", "bh_create", "bh_destroy", "bh_set_stream", "bh_build", "bh_accel",
            "bh_direct", "bh_direct_targets", "bh_bind_state", "bh_kdk_step", "bh_get_state_acc",
            "bh_eval_host", "bh_synchronize", "bh_get_cube", "bh_get_keys", "bh_get_node_count",
-           "bh_get_nodes", "bh_get_groups", "bh_get_bodies", "bh_get_counts", "bh_get_stats", "bh_set_timing",
+           "bh_get_nodes", "bh_get_groups", "bh_get_bodies", "bh_get_counts", "bh_get_stats", "bh_get_launches",
+           "bh_set_timing",
            "bh_get_phase_ms", "bh_measure_fp64_peak", "bh_last_error", "bh_version")
 
 
@@ -208,6 +210,12 @@ def bh_get_stats(ctx):
     s = (C.c_uint64 * 4)()
     _check(ctx, lib().bh_get_stats(ctx, s))
     return {"n_mono": s[0], "n_direct": s[1], "interactions": s[2], "nodes_tested": s[3]}
+
+
+def bh_get_launches(ctx) -> int:
+    v = C.c_uint64()
+    _check(ctx, lib().bh_get_launches(ctx, C.byref(v)))
+    return v.value
 
 
 def bh_set_timing(ctx, enable: bool):

@@ -27,6 +27,7 @@ struct bh_ctx {
     cudaEvent_t ev[BH_NUM_PHASES][2]{};
     bool ev_set[BH_NUM_PHASES]{};
     DevState *host_state = nullptr;   // pinned mirror for synchronising getters
+    uint64_t launches = 0;            // kernels launched so far (bench.py's gpu_launches)
     char err[256] = "";
 };
 
@@ -124,6 +125,7 @@ bh_status do_build(bh_ctx *c, const double *pos, const double *mass, int64_t n)
     if (st != BH_OK) return st;
     c->n = n;
     c->built = true;
+    c->launches += 2 + kSortPasses + 1 + 4 + 1;   // cube, keys, sort passes, gather, tree (3) + boxes, monopoles
     return BH_OK;
 }
 
@@ -138,7 +140,10 @@ bh_status do_accel(bh_ctx *c, double theta, double eps, double G, double *acc)
         launch_walk(w, c->n, theta, eps, G, acc, c->stream);
     }
     bh_status st = cuda_check(c, cudaGetLastError(), "bh_accel launch");
-    if (st == BH_OK) c->walked = true;
+    if (st == BH_OK) {
+        c->walked = true;
+        c->launches += 1;
+    }
     return st;
 }
 
@@ -294,6 +299,7 @@ bh_status bh_direct(bh_ctx *c, double eps, double G, double *acc_dev)
     {
         Phase p(c, 7);
         launch_direct(c->ws, c->n, nullptr, c->n, eps, G, acc_dev, c->stream);
+        c->launches += 1;
     }
     return cuda_check(c, cudaGetLastError(), "bh_direct launch");
 }
@@ -307,6 +313,7 @@ bh_status bh_direct_targets(bh_ctx *c, const int32_t *tgt_dev, int64_t nt, doubl
     {
         Phase p(c, 7);
         launch_direct(c->ws, c->n, tgt_dev, nt, eps, G, acc_dev, c->stream);
+        c->launches += 1;
     }
     return cuda_check(c, cudaGetLastError(), "bh_direct_targets launch");
 }
@@ -349,6 +356,7 @@ bh_status bh_kdk_step(bh_ctx *c, double dt)
     if ((st = do_build(c, c->pos, c->mass, c->bound_n)) != BH_OK) return st;
     if ((st = do_accel(c, c->theta, c->eps, c->G, c->ws.acc)) != BH_OK) return st;
     launch_kick(c->vel, c->ws.acc, c->bound_n, dt * 0.5, c->stream);
+    c->launches += 2;   // kick+drift, kick
     return cuda_check(c, cudaGetLastError(), "bh_kdk_step launch");
 }
 
@@ -499,6 +507,13 @@ bh_status bh_get_stats(bh_ctx *c, uint64_t stats_host[4])
     bh_status st = fetch_state(c);
     if (st != BH_OK) return st;
     for (int k = 0; k < 4; ++k) stats_host[k] = c->host_state->stats[k];
+    return BH_OK;
+}
+
+bh_status bh_get_launches(bh_ctx *c, uint64_t *count_host)
+{
+    if (!c || !count_host) return BH_ERR_INVALID_ARG;
+    *count_host = c->launches;
     return BH_OK;
 }
 
