@@ -188,6 +188,7 @@ Workspace carve(char *base, int64_t max_n, int leaf_cap)
     w.nfirst = cv.take<int>(w.node_cap);
     w.nparent = cv.take<int>(w.node_cap);
     w.mono = cv.take<double4>(w.node_cap);
+    w.winfo = cv.take<uint4>(w.node_cap);
     w.cnt_mono = cv.take<unsigned>(groups);
     w.cnt_direct = cv.take<unsigned>(groups);
     w.walk_stack = cv.take<unsigned>((size_t)w.walk_warps * kStackSlab);

@@ -64,6 +64,7 @@ struct Workspace {
     int *nfirst;
     int *nparent;
     double4 *mono;
+    uint4 *winfo;                 // [M] walk record: begin, count, first_child, level | children << 8
     unsigned *cnt_mono;           // [Ng] (capacity n)
     unsigned *cnt_direct;         // [Ng]
     unsigned *walk_stack;         // [walk warps][kStackSlab]

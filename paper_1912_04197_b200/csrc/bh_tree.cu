@@ -333,12 +333,19 @@ __global__ void __launch_bounds__(256) monopole_kernel(const DevState *__restric
                                                        const unsigned *__restrict__ ncount,
                                                        const int *__restrict__ nfirst,
                                                        const int *__restrict__ nparent, unsigned *node_meta,
-                                                       double4 *mono, long long node_cap)
+                                                       double4 *mono, long long node_cap,
+                                                       const unsigned char *__restrict__ nlevel,
+                                                       uint4 *__restrict__ winfo)
 {
     const int M = st->n_nodes;
     if ((long long)M > node_cap) return;
     for (int t = blockIdx.x * blockDim.x + threadIdx.x; t < M; t += gridDim.x * blockDim.x) {
-        if (nfirst[t] >= 0) continue;   // internal nodes are computed by their last child
+        // the walk's packed record of this node (the child mask is complete: bits 0-7 are only
+        // written by tree_emit_kernel)
+        const int first = nfirst[t];
+        const unsigned kids = (unsigned)__popc(__ldcg(node_meta + t) & 0xffu);
+        winfo[t] = make_uint4(nbegin[t], ncount[t], (unsigned)first, (unsigned)nlevel[t] | (kids << 8));
+        if (first >= 0) continue;   // internal nodes are computed by their last child
         const unsigned b = nbegin[t], c = ncount[t];
         double4 r;
         if (c == 1) {
@@ -414,7 +421,7 @@ void launch_monopoles(const Workspace &w, int64_t n, cudaStream_t s)
     int blocks = (int)(want < 148 * 16 ? want : 148 * 16);
     (void)n;
     monopole_kernel<<<blocks, 256, 0, s>>>(w.st, w.sbody, w.nbegin, w.ncount, w.nfirst, w.nparent, w.node_meta,
-                                           w.mono, w.node_cap);
+                                           w.mono, w.node_cap, w.nlevel, w.winfo);
 }
 
 void launch_unpack_mask(const Workspace &w, unsigned char *mask_out, int64_t cap, cudaStream_t s)

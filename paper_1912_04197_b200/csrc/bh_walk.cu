@@ -10,8 +10,8 @@
 //             body of the group), and the results are appended by ballot/prefix: accepted nodes ->
 //             their (cx,cy,cz,m) into the shared source list; opened internal nodes -> their
 //             children onto the stack; opened leaves -> their bodies (x,y,z,m) into the same list.
-//   evaluate  lanes = bodies.  Whenever the list holds a full chunk, every lane reads the chunk's
-//             sources by shared-memory broadcast and accumulates m d / (|d|^2+eps^2)^(3/2) in fp64.
+//   evaluate  lanes = bodies.  After every traversal step every lane reads the sources that are ready
+//             (in quads) by shared-memory broadcast and accumulates m d / (|d|^2+eps^2)^(3/2) in fp64.
 // The test arithmetic is the canonical one (each operation rounded once, fma where stated) so that
 // every accept/open decision equals the oracle's; the accumulation order is free.
 #include "bh_common.cuh"
@@ -19,8 +19,7 @@
 namespace bh {
 
 constexpr int kWalkWarps = WalkConfig::kWarpsPerBlock;
-constexpr int kChunk = 64;                  // sources evaluated per flush
-constexpr int kListCap = 2 * kChunk;        // ring capacity (sources); append adds <= 32 at a time
+constexpr int kListCap = 256;               // ring capacity (sources); body copies are issued while 32 slots are free
 constexpr int kStackSmem = 768;             // node ids kept in shared memory per warp
 constexpr int kSpill = 256;                 // spill / refill unit
 
@@ -36,14 +35,16 @@ __device__ __forceinline__ double rsqrt_fast(double x)
     return fma(y, q, y);
 }
 
-// accumulate the pull of one source (sx,sy,sz,sm) on the body at (px,py,pz)
+// accumulate the pull of one source (sx,sy,sz,sm) on the body at (px,py,pz).  GUARD: a pair at zero
+// softened distance adds nothing (R13); it can only happen when eps == 0, so eps > 0 skips the test.
+template <bool GUARD>
 __device__ __forceinline__ void interact(double px, double py, double pz, double eps2, const double4 s,
                                          double &ax, double &ay, double &az)
 {
     const double dx = s.x - px, dy = s.y - py, dz = s.z - pz;
     const double r2 = fma(dx, dx, fma(dy, dy, fma(dz, dz, eps2)));
     double y = rsqrt_fast(r2);
-    y = (r2 > 0.0) ? y : 0.0;                   // R13: a pair at zero softened distance adds nothing
+    if (GUARD) y = (r2 > 0.0) ? y : 0.0;
     const double y2 = y * y;
     const double f = (s.w * y) * y2;
     ax = fma(f, dx, ax);
@@ -52,10 +53,23 @@ __device__ __forceinline__ void interact(double px, double py, double pz, double
 }
 
 struct WalkSmem {
-    double4 src[kWalkWarps][kListCap];
+    double4 src[kWalkWarps][kListCap];        // ring of pending sources
+    double4 stage_mono[kWalkWarps][32];       // async landing zone of the next node batch
+    uint4 stage_info[kWalkWarps][32];
     unsigned stack[kWalkWarps][kStackSmem];
 };
 
+__device__ __forceinline__ void cp_async16(void *smem, const void *gmem)
+{
+    const unsigned s = (unsigned)__cvta_generic_to_shared(smem);
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 16;" ::"r"(s), "l"(gmem) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;" ::: "memory"); }
+
+// count sources starting at ring position first (no wrap inside: callers pass chunk-aligned ranges
+// or the tail remainder, handled with the mask)
+template <bool GUARD>
 __device__ __forceinline__ void eval_range(const double4 *src, int first, int count, double px, double py,
                                            double pz, double eps2, double &ax, double &ay, double &az)
 {
@@ -66,22 +80,43 @@ __device__ __forceinline__ void eval_range(const double4 *src, int first, int co
         const double4 s1 = src[(first + i + 1) & (kListCap - 1)];
         const double4 s2 = src[(first + i + 2) & (kListCap - 1)];
         const double4 s3 = src[(first + i + 3) & (kListCap - 1)];
-        interact(px, py, pz, eps2, s0, ax, ay, az);
-        interact(px, py, pz, eps2, s1, ax, ay, az);
-        interact(px, py, pz, eps2, s2, ax, ay, az);
-        interact(px, py, pz, eps2, s3, ax, ay, az);
+        interact<GUARD>(px, py, pz, eps2, s0, ax, ay, az);
+        interact<GUARD>(px, py, pz, eps2, s1, ax, ay, az);
+        interact<GUARD>(px, py, pz, eps2, s2, ax, ay, az);
+        interact<GUARD>(px, py, pz, eps2, s3, ax, ay, az);
     }
-    for (; i < count; ++i) interact(px, py, pz, eps2, src[(first + i) & (kListCap - 1)], ax, ay, az);
+    for (; i < count; ++i) interact<GUARD>(px, py, pz, eps2, src[(first + i) & (kListCap - 1)], ax, ay, az);
 }
 
+// evaluate the largest multiple of four sources that is ready; head stays a multiple of four, so a
+// quad never wraps around the ring
+template <bool GUARD>
+__device__ __forceinline__ int eval_quads(const double4 *src, int head, int tail, double px, double py, double pz,
+                                          double eps2, double &ax, double &ay, double &az)
+{
+    const int n4 = (tail - head) & ~3;
+#pragma unroll 1
+    for (int i = 0; i < n4; i += 4) {
+        const double4 *p = src + ((head + i) & (kListCap - 1));
+        const double4 s0 = p[0], s1 = p[1], s2 = p[2], s3 = p[3];
+        interact<GUARD>(px, py, pz, eps2, s0, ax, ay, az);
+        interact<GUARD>(px, py, pz, eps2, s1, ax, ay, az);
+        interact<GUARD>(px, py, pz, eps2, s2, ax, ay, az);
+        interact<GUARD>(px, py, pz, eps2, s3, ax, ay, az);
+    }
+    return head + n4;
+}
+
+// The traversal is software-pipelined with asynchronous copies (cp.async / LDGSTS): while the warp
+// evaluates the chunks that are ready, the node records of the NEXT batch and the bodies of the
+// leaves opened by THIS batch are already in flight from L2 straight into shared memory.
+template <bool GUARD>
 __global__ void __launch_bounds__(kWalkWarps * 32, WalkConfig::kBlocksPerSM)
 walk_kernel(DevState *st, const unsigned *__restrict__ gstart, const double4 *__restrict__ sbody,
-            const double *__restrict__ gbox,
-            const unsigned *__restrict__ perm, const unsigned char *__restrict__ nlevel,
-            const unsigned *__restrict__ nbegin, const unsigned *__restrict__ ncount,
-            const int *__restrict__ nfirst, const unsigned *__restrict__ node_meta,
-            const double4 *__restrict__ mono, double theta2, double eps2, double G, double *__restrict__ acc,
-            unsigned *__restrict__ cnt_mono, unsigned *__restrict__ cnt_direct, unsigned *walk_stack)
+            const double *__restrict__ gbox, const unsigned *__restrict__ perm,
+            const uint4 *__restrict__ winfo, const double4 *__restrict__ mono, double theta2, double eps2,
+            double G, double *__restrict__ acc, unsigned *__restrict__ cnt_mono,
+            unsigned *__restrict__ cnt_direct, unsigned *walk_stack)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     WalkSmem &sm = *reinterpret_cast<WalkSmem *>(smem_raw);
@@ -89,6 +124,8 @@ walk_kernel(DevState *st, const unsigned *__restrict__ gstart, const double4 *__
     const unsigned lt = (1u << lane) - 1u;
     double4 *src = sm.src[warp];
     unsigned *stack = sm.stack[warp];
+    double4 *st_mono = sm.stage_mono[warp];
+    uint4 *st_info = sm.stage_info[warp];
     unsigned *slab = walk_stack + (size_t)(blockIdx.x * kWalkWarps + warp) * kStackSlab;
     const unsigned ngroups = st->n_groups;
     const int e2 = 2 * st->e;
@@ -108,25 +145,24 @@ walk_kernel(DevState *st, const unsigned *__restrict__ gstart, const double4 *__
         const double glx = gbox[6 * g + 0], gly = gbox[6 * g + 1], glz = gbox[6 * g + 2];
         const double ghx = gbox[6 * g + 3], ghy = gbox[6 * g + 4], ghz = gbox[6 * g + 5];
         double ax = 0.0, ay = 0.0, az = 0.0;
-        int head = 0, tail = 0;        // ring [head, tail) of pending sources
-        int sp = 1, gsp = 0;           // shared stack size, spilled entries in the slab
+        int head = 0, tail = 0, pending = 0;   // ring [head, tail) ready, then `pending` bodies in flight
+        int sp = 0, gsp = 0;                   // shared stack size, spilled entries in the slab
         unsigned n_mono = 0, n_direct = 0, n_tested = 0;
-        if (lane == 0) stack[0] = 0u;  // the root
-        __syncwarp();
+        // prime the pipeline with the root
+        int take = 1;
+        if (lane == 0) {
+            cp_async16(&st_info[0], winfo);
+            cp_async16(&st_mono[0], mono);
+            cp_async16(reinterpret_cast<char *>(&st_mono[0]) + 16, reinterpret_cast<const char *>(mono) + 16);
+        }
+        cp_async_commit();
 
-        while (sp > 0 || gsp > 0) {
-            if (sp == 0) {             // refill from the slab
-                gsp -= kSpill;
-                for (int k = lane; k < kSpill; k += 32) stack[k] = slab[gsp + k];
-                sp = kSpill;
-                __syncwarp();
-            }
-            const int take = sp < 32 ? sp : 32;
-            sp -= take;
-            const bool have = (int)lane < take;
-            unsigned t = 0;
-            if (have) t = stack[sp + lane];
+        while (take > 0) {
+            cp_async_wait_all();
             __syncwarp();
+            tail += pending;
+            pending = 0;
+            const bool have = (int)lane < take;
             n_tested += take;
             // ---- opening test (canonical arithmetic) ----
             bool accept = false, open_internal = false, open_leaf = false;
@@ -134,29 +170,31 @@ walk_kernel(DevState *st, const unsigned *__restrict__ gstart, const double4 *__
             int fc = -1;
             double4 mn = make_double4(0.0, 0.0, 0.0, 0.0);
             if (have) {
-                b = nbegin[t];
-                c = ncount[t];
-                fc = nfirst[t];
-                mn = mono[t];
+                const uint4 info = st_info[lane];
+                mn = st_mono[lane];
+                b = info.x;
+                c = info.y;
+                fc = (int)info.z;
                 const bool overlap = ((long long)b < ge) && (gb < (long long)b + c);
                 if (!overlap) {
                     const double dx = fmax(fmax(__dsub_rn(glx, mn.x), __dsub_rn(mn.x, ghx)), 0.0);
                     const double dy = fmax(fmax(__dsub_rn(gly, mn.y), __dsub_rn(mn.y, ghy)), 0.0);
                     const double dz = fmax(fmax(__dsub_rn(glz, mn.z), __dsub_rn(mn.z, ghz)), 0.0);
                     const double d2 = __fma_rn(dz, dz, __fma_rn(dy, dy, __dmul_rn(dx, dx)));
-                    const int lv = nlevel[t];
+                    const int lv = (int)(info.w & 0xffu);
                     const double s2 = __hiloint2double((e2 - 2 * lv + 1023) << 20, 0);   // (L 2^-lv)^2
                     accept = s2 < __dmul_rn(theta2, d2);
                 }
                 if (!accept) {
                     if (fc >= 0) {
                         open_internal = true;
-                        nch = __popc(node_meta[t] & 0xffu);
+                        nch = (info.w >> 8) & 0xffu;
                     } else {
                         open_leaf = true;
                     }
                 }
             }
+            __syncwarp();   // staging area is free again
             // ---- accepted nodes -> source list ----
             {
                 const unsigned m = __ballot_sync(0xffffffffu, accept);
@@ -192,11 +230,10 @@ walk_kernel(DevState *st, const unsigned *__restrict__ gstart, const double4 *__
                     for (unsigned u = 0; u < nch; ++u) stack[off + u] = (unsigned)fc + u;
                 }
                 sp += total;
-                __syncwarp();
             }
-            // ---- opened leaves -> their bodies into the source list ----
+            // ---- opened leaves -> their bodies, asynchronously into the ring ----
             {
-                unsigned lc = open_leaf ? c : 0u;
+                const unsigned lc = open_leaf ? c : 0u;
                 unsigned inc = lc;
 #pragma unroll
                 for (int o = 1; o < 32; o <<= 1) {
@@ -206,11 +243,14 @@ walk_kernel(DevState *st, const unsigned *__restrict__ gstart, const double4 *__
                 const unsigned total = __shfl_sync(0xffffffffu, inc, 31);
                 n_direct += total;
                 for (unsigned base = 0; base < total; base += 32) {
-                    // make room first: a full chunk is evaluated as soon as it exists
-                    while (tail - head >= kChunk) {
+                    // keep 32 slots for this round and 32 for the next batch's accepted nodes
+                    if (kListCap - (tail + pending - head) < 64) {   // ring full: drain, evaluate, go on
+                        cp_async_commit();
+                        cp_async_wait_all();
                         __syncwarp();
-                        eval_range(src, head, kChunk, px, py, pz, eps2, ax, ay, az);
-                        head += kChunk;
+                        tail += pending;
+                        pending = 0;
+                        head = eval_quads<GUARD>(src, head, tail, px, py, pz, eps2, ax, ay, az);
                         __syncwarp();
                     }
                     const unsigned idx = base + lane;
@@ -227,21 +267,40 @@ walk_kernel(DevState *st, const unsigned *__restrict__ gstart, const double4 *__
                     const unsigned obeg = __shfl_sync(0xffffffffu, b, lo);
                     if (idx < total) {
                         const unsigned body = obeg + (idx - (oinc - ocnt));
-                        src[(tail + lane) & (kListCap - 1)] = sbody[body];
+                        char *dst = reinterpret_cast<char *>(&src[(tail + pending + lane) & (kListCap - 1)]);
+                        const char *from = reinterpret_cast<const char *>(sbody + body);
+                        cp_async16(dst, from);
+                        cp_async16(dst + 16, from + 16);
                     }
-                    const unsigned got = total - base < 32u ? total - base : 32u;
-                    tail += (int)got;
+                    pending += (int)(total - base < 32u ? total - base : 32u);
                 }
             }
-            while (tail - head >= kChunk) {
-                __syncwarp();
-                eval_range(src, head, kChunk, px, py, pz, eps2, ax, ay, az);
-                head += kChunk;
+            __syncwarp();   // children are on the stack
+            // ---- pop the next batch and start its loads ----
+            if (sp == 0 && gsp > 0) {             // refill from the slab
+                gsp -= kSpill;
+                for (int k = lane; k < kSpill; k += 32) stack[k] = slab[gsp + k];
+                sp = kSpill;
                 __syncwarp();
             }
+            take = sp < 32 ? sp : 32;
+            sp -= take;
+            if ((int)lane < take) {
+                const unsigned t = stack[sp + lane];
+                cp_async16(&st_info[lane], winfo + t);
+                const char *from = reinterpret_cast<const char *>(mono + t);
+                cp_async16(&st_mono[lane], from);
+                cp_async16(reinterpret_cast<char *>(&st_mono[lane]) + 16, from + 16);
+            }
+            cp_async_commit();
+            __syncwarp();
+            // ---- evaluate what is ready while the copies fly ----
+            head = eval_quads<GUARD>(src, head, tail, px, py, pz, eps2, ax, ay, az);
         }
+        cp_async_wait_all();
         __syncwarp();
-        eval_range(src, head, tail - head, px, py, pz, eps2, ax, ay, az);
+        tail += pending;
+        eval_range<GUARD>(src, head, tail - head, px, py, pz, eps2, ax, ay, az);
         __syncwarp();
         if (valid) {
             const unsigned i = perm[j];
@@ -288,7 +347,7 @@ direct_kernel(long long n, const double4 *__restrict__ sbody, const unsigned *__
         tile[threadIdx.x] = k < n ? sbody[k] : make_double4(0.0, 0.0, 0.0, 0.0);   // zero mass: no pull
         __syncthreads();
 #pragma unroll 4
-        for (int q = 0; q < kDirectThreads; ++q) interact(me.x, me.y, me.z, eps2, tile[q], ax, ay, az);
+        for (int q = 0; q < kDirectThreads; ++q) interact<true>(me.x, me.y, me.z, eps2, tile[q], ax, ay, az);
         __syncthreads();
     }
     if (valid) {
@@ -337,13 +396,21 @@ void launch_walk(const Workspace &w, int64_t n, double theta, double eps, double
 {
     static bool configured = false;
     if (!configured) {
-        cudaFuncSetAttribute(walk_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(WalkSmem));
+        cudaFuncSetAttribute(walk_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(WalkSmem));
+        cudaFuncSetAttribute(walk_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(WalkSmem));
         configured = true;
     }
+    (void)n;
     const int blocks = w.walk_warps / kWalkWarps;
-    walk_kernel<<<blocks, kWalkWarps * 32, sizeof(WalkSmem), s>>>(
-        w.st, w.gstart, w.sbody, w.gbox, w.idx[0], w.nlevel, w.nbegin, w.ncount, w.nfirst, w.node_meta, w.mono,
-        theta * theta, eps * eps, G, acc, w.cnt_mono, w.cnt_direct, w.walk_stack);
+    const double eps2 = eps * eps;
+    if (eps2 > 0.0)
+        walk_kernel<false><<<blocks, kWalkWarps * 32, sizeof(WalkSmem), s>>>(
+            w.st, w.gstart, w.sbody, w.gbox, w.idx[0], w.winfo, w.mono, theta * theta, eps2, G, acc, w.cnt_mono,
+            w.cnt_direct, w.walk_stack);
+    else
+        walk_kernel<true><<<blocks, kWalkWarps * 32, sizeof(WalkSmem), s>>>(
+            w.st, w.gstart, w.sbody, w.gbox, w.idx[0], w.winfo, w.mono, theta * theta, eps2, G, acc, w.cnt_mono,
+            w.cnt_direct, w.walk_stack);
 }
 
 void launch_direct(const Workspace &w, int64_t n, const int32_t *tgt, int64_t nt, double eps, double G,
