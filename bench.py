@@ -151,6 +151,20 @@ def run_reference(args):
     print(json.dumps(line), flush=True)
 
 
+# ------------------------------------------------------------------------------------------ multi-rank
+def aggregate(total_ms: float, bodies_per_rank: int, steps: int, world: int, device=None):
+    """Replicas only: every rank runs the same workload; the job's time is the MAX over
+    ranks of the summed per-step device time, its throughput the bodies of ALL ranks over that time.
+    Works on any backend (nccl on GPUs, gloo in the CPU tests)."""
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([total_ms], dtype=torch.float64, device=device)
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    tmax = float(t.item())
+    return tmax, world * bodies_per_rank * steps / (tmax * 1e-3)
+
+
 # ------------------------------------------------------------------------------------------ own arm
 def run_own(args):
     import numpy as np
@@ -212,11 +226,7 @@ def run_own(args):
     clocks = sampler.stop()
     launches = bh.bh_get_launches(ctx.ctx) - l0
     step_ms = [a.elapsed_time(b) for a, b in ev]
-    total_ms = torch.tensor([sum(step_ms)], dtype=torch.float64, device=dev)
-    if world > 1:
-        dist.all_reduce(total_ms, op=dist.ReduceOp.MAX)
-    total_ms = float(total_ms.item())
-    value = world * w.n * args.steps / (total_ms * 1e-3)
+    total_ms, value = aggregate(sum(step_ms), w.n, args.steps, world, dev)
     nph = len(walk_ms)
     phases = {k: v / nph for k, v in phase_sum.items() if k != "direct"}
     M, depth = bh.bh_get_node_count(ctx.ctx)

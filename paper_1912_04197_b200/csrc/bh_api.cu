@@ -194,6 +194,7 @@ Workspace carve(char *base, int64_t max_n, int leaf_cap)
     w.walk_stack = cv.take<unsigned>((size_t)w.walk_warps * kStackSlab);
     w.acc = cv.take<double>(3 * n);
     w.stage_pos = cv.take<double>(3 * n);
+    w.stage_doubles = 3 * n;
     w.stage_mass = cv.take<double>(n);
     w.peak_sink = cv.take<double>(32);
     w.total_bytes = cv.off;
@@ -299,8 +300,7 @@ bh_status bh_direct(bh_ctx *c, double eps, double G, double *acc_dev)
     if (!(eps >= 0.0)) return fail(c, BH_ERR_INVALID_ARG, "bh_direct: eps negative");
     {
         Phase p(c, 7);
-        launch_direct(c->ws, c->n, nullptr, c->n, eps, G, acc_dev, c->stream);
-        c->launches += 1;
+        c->launches += launch_direct(c->ws, c->n, nullptr, c->n, eps, G, acc_dev, c->stream);
     }
     return cuda_check(c, cudaGetLastError(), "bh_direct launch");
 }
@@ -313,8 +313,7 @@ bh_status bh_direct_targets(bh_ctx *c, const int32_t *tgt_dev, int64_t nt, doubl
     if (nt < 1 || !(eps >= 0.0)) return fail(c, BH_ERR_INVALID_ARG, "bh_direct_targets: nt < 1 or eps negative");
     {
         Phase p(c, 7);
-        launch_direct(c->ws, c->n, tgt_dev, nt, eps, G, acc_dev, c->stream);
-        c->launches += 1;
+        c->launches += launch_direct(c->ws, c->n, tgt_dev, nt, eps, G, acc_dev, c->stream);
     }
     return cuda_check(c, cudaGetLastError(), "bh_direct_targets launch");
 }

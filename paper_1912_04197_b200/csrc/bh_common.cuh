@@ -69,7 +69,8 @@ struct Workspace {
     unsigned *cnt_direct;         // [Ng]
     unsigned *walk_stack;         // [walk warps][kStackSlab]
     double *acc;                  // [n][3] internal accelerations (KDK state, host staging)
-    double *stage_pos;            // [n][3] host-call staging
+    double *stage_pos;            // [n][3] host-call staging; also the direct kernel's partial sums
+    int64_t stage_doubles;        // capacity of stage_pos in doubles
     double *stage_mass;           // [n]
     double *peak_sink;            // fp64 microbenchmark sink
     int64_t node_cap;
@@ -98,8 +99,8 @@ void launch_gather(const Workspace &w, const double *pos, const double *mass, in
 void launch_tree(const Workspace &w, int64_t n, int leaf_cap, cudaStream_t s);
 void launch_monopoles(const Workspace &w, int64_t n, cudaStream_t s);
 void launch_walk(const Workspace &w, int64_t n, double theta, double eps, double G, double *acc, cudaStream_t s);
-void launch_direct(const Workspace &w, int64_t n, const int32_t *tgt, int64_t nt, double eps, double G,
-                   double *acc, cudaStream_t s);
+int launch_direct(const Workspace &w, int64_t n, const int32_t *tgt, int64_t nt, double eps, double G,
+                  double *acc, cudaStream_t s);   // returns the number of kernels launched
 void launch_kick_drift(double *pos, double *vel, const double *acc, int64_t n, double dt, cudaStream_t s);
 void launch_kick(double *vel, const double *acc, int64_t n, double h, cudaStream_t s);
 void launch_unpack_mask(const Workspace &w, unsigned char *mask_out, int64_t cap, cudaStream_t s);
