@@ -159,7 +159,7 @@ Workspace carve(char *base, int64_t max_n, int leaf_cap)
     w.node_cap = node_capacity(n, leaf_cap);
     w.sort_tiles = (n + kSortTile - 1) / kSortTile;
     w.tree_tiles = (n + kTreeTile - 1) / kTreeTile;
-    w.walk_warps = WalkConfig::kSMs * WalkConfig::kBlocksPerSM * WalkConfig::kWarpsPerBlock;
+    w.walk_warps = WalkConfig::kSMs * WalkConfig::kPairsPerBlock;
     const int64_t groups = n;   // capacity: a group holds at least one body
     w.st = cv.take<DevState>(1);
     w.bbox_part = cv.take<double>(148 * 4 * 8);
@@ -191,7 +191,7 @@ Workspace carve(char *base, int64_t max_n, int leaf_cap)
     w.winfo = cv.take<uint4>(w.node_cap);
     w.cnt_mono = cv.take<unsigned>(groups);
     w.cnt_direct = cv.take<unsigned>(groups);
-    w.walk_stack = cv.take<unsigned>((size_t)w.walk_warps * kStackSlab);
+    w.walk_stack = cv.take<unsigned>((size_t)w.walk_warps * kStackSlab * 2);
     w.acc = cv.take<double>(3 * n);
     w.stage_pos = cv.take<double>(3 * n);
     w.stage_doubles = 3 * n;

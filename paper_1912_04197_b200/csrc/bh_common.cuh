@@ -19,7 +19,7 @@ constexpr int kSortThreads = 256;
 constexpr int kSortItems = 16;            // keys per thread
 constexpr int kSortTile = kSortThreads * kSortItems;   // 4096 keys per tile
 constexpr int kTreeTile = 1024;           // bodies per block in the tree kernels
-constexpr int kStackSlab = 22 * 256;      // walk: global spill entries per warp (bound: 256 per level)
+constexpr int kStackSlab = 22 * 256;      // walk: spill entries (8 bytes each) per producer warp: <= 32 x 7 ranges per level; overflow sets kStatStack
 
 enum StatusBits : int { kStatNonFinite = 1, kStatCapacity = 2, kStatStack = 4 };
 
@@ -67,7 +67,7 @@ struct Workspace {
     uint4 *winfo;                 // [M] walk record: begin, count, first_child, level | children << 8
     unsigned *cnt_mono;           // [Ng] (capacity n)
     unsigned *cnt_direct;         // [Ng]
-    unsigned *walk_stack;         // [walk warps][kStackSlab]
+    unsigned *walk_stack;         // [walk producer warps][kStackSlab][2]
     double *acc;                  // [n][3] internal accelerations (KDK state, host staging)
     double *stage_pos;            // [n][3] host-call staging; also the direct kernel's partial sums
     int64_t stage_doubles;        // capacity of stage_pos in doubles
@@ -76,13 +76,12 @@ struct Workspace {
     int64_t node_cap;
     int64_t sort_tiles;
     int64_t tree_tiles;
-    int walk_warps;
+    int walk_warps;               // producer warps of the walk = SMs x pairs per block
     size_t total_bytes;
 };
 
 struct WalkConfig {
-    static constexpr int kWarpsPerBlock = 8;
-    static constexpr int kBlocksPerSM = 2;
+    static constexpr int kPairsPerBlock = 8;   // producer/consumer warp pairs in the one block of an SM
     static constexpr int kSMs = 148;
 };
 

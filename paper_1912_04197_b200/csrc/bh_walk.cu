@@ -1,104 +1,516 @@
 // bh_walk.cu — step a7 (group-cooperative tree walk, Eqs. (3)-(6) PAPER.md:84-106), step a8 (direct
 // N^2 sum, Eq. (1)), step a9 (leapfrog kernels) and the fp64 peak microbenchmark.
 //
-// Walk: one warp owns a group of up to 32 Morton-consecutive bodies of one group cell (R6).  Traversal and evaluation
-// alternate inside the warp:
-//   traverse  lanes = candidate nodes.  The warp pops up to 32 node ids from a LIFO stack (top part
-//             in shared memory, spill slab in global memory), each lane applies the opening test
-//             of the GROUP (R3-R7: node edge s, distance from the node's centre of mass to the
-//             group's bounding box, accept iff s*s < theta^2 d^2, never accept a node that holds a
-//             body of the group), and the results are appended by ballot/prefix: accepted nodes ->
-//             their (cx,cy,cz,m) into the shared source list; opened internal nodes -> their
-//             children onto the stack; opened leaves -> their bodies (x,y,z,m) into the same list.
-//   evaluate  lanes = bodies.  After every traversal step every lane reads the sources that are ready
-//             (in quads) by shared-memory broadcast and accumulates m d / (|d|^2+eps^2)^(3/2) in fp64.
+// Walk: a group is up to 32 Morton-consecutive bodies of one group cell (R6).  The kernel is warp
+// specialised: one persistent 512-thread block per SM holds eight PAIRS of warps, a producer and a
+// consumer, joined by a ring of sources (x,y,z,m) in shared memory.
+//   producer  lanes = candidate nodes.  It takes a group from the atomic queue and traverses the tree
+//             for it: pops up to 32 sibling ranges (first child, count) from a LIFO stack (shared-memory
+//             ring, spill slab in global memory); every lane walks its range one node per trip and
+//             applies the opening test of the GROUP (R3-R7: node edge s, distance from the node's
+//             centre of mass to the group's bounding box, accept iff s*s < theta^2 d^2, never accept a
+//             node that holds a body of the group); the results are appended by ballot/prefix:
+//             accepted nodes -> their (cx,cy,cz,m) into the ring; opened internal nodes -> their child
+//             range onto the stack; opened leaves -> their bodies (x,y,z,m) into the ring (cp.async,
+//             straight from L2).  The record of a lane's next sibling is loaded while the current one
+//             is tested.  The producer is written for instruction count: on sm_100 every instruction
+//             another warp issues costs the fp64 warps of the same sub-partition an issue slot.
+//   consumer  lanes = bodies.  It evaluates the sources the producer has published, in fp64: every
+//             lane carries FOUR bodies of the group (lane l: bodies l%8 + 8k) and the four quarter-warps
+//             take alternate sources, so one shared-memory read of a source feeds four interactions and
+//             the fp64 pipe, not the load-store path, sets the pace.
+// The two roles meet only through release/acquire counters in shared memory, so the fp64 pipe of an SM
+// sub-partition is fed by its two consumers while its two producers wait on L2.
 // The test arithmetic is the canonical one (each operation rounded once, fma where stated) so that
-// every accept/open decision equals the oracle's; the accumulation order is free.
+// every accept/open decision equals the oracle's; traversal and accumulation order are free (R23).
 #include "bh_common.cuh"
 
 namespace bh {
 
-constexpr int kWalkWarps = WalkConfig::kWarpsPerBlock;
-constexpr int kListCap = 256;               // ring capacity (sources); body copies are issued while 32 slots are free
-constexpr int kStackSmem = 768;             // node ids kept in shared memory per warp
-constexpr int kSpill = 256;                 // spill / refill unit
+constexpr int kPairs = WalkConfig::kPairsPerBlock;       // producer/consumer pairs per block
+constexpr int kWalkThreads = kPairs * 64;
+constexpr int kRing = 512;                  // sources per pair (power of two, multiple of 8)
+constexpr int kStack = 512;                 // sibling ranges per producer in shared memory (ring)
+constexpr int kSpill = 128;                 // spill / refill unit
+constexpr int kDesc = 4;                    // group descriptors in flight per pair
+constexpr unsigned kNoGroup = 0xffffffffu;
 
-// 1/sqrt(x) for normal positive x: MUFU.RSQ64H seed (about 20 good bits) and one third-order step.
-__device__ __forceinline__ double rsqrt_fast(double x)
-{
-    double y;
-    asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
-    double t = x * y;
-    double e = fma(-t, y, 1.0);                 // 1 - x y^2
-    double p = fma(0.375, e, 0.5);
-    double q = e * p;                           // e/2 + 3 e^2/8
-    return fma(y, q, y);
-}
-
-// accumulate the pull of one source (sx,sy,sz,sm) on the body at (px,py,pz).  GUARD: a pair at zero
-// softened distance adds nothing (R13); it can only happen when eps == 0, so eps > 0 skips the test.
+// m / r^3 from r2 = |d|^2 + eps^2: MUFU.RSQ64H seed y (about 20 good bits), e = 1 - r2 y^2 and the
+// series (1-e)^(-3/2) = 1 + e (3/2 + 15/8 e) + O(e^3).  Every fp64 instruction except the three
+// accumulations reads at most two distinct register operands (a third costs the pipe a cycle on sm_100).
 template <bool GUARD>
 __device__ __forceinline__ void interact(double px, double py, double pz, double eps2, const double4 s,
                                          double &ax, double &ay, double &az)
 {
     const double dx = s.x - px, dy = s.y - py, dz = s.z - pz;
     const double r2 = fma(dx, dx, fma(dy, dy, fma(dz, dz, eps2)));
-    double y = rsqrt_fast(r2);
-    if (GUARD) y = (r2 > 0.0) ? y : 0.0;
-    const double y2 = y * y;
-    const double f = (s.w * y) * y2;
+    double y;
+    asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(r2));
+    if (GUARD) y = (r2 > 0.0) ? y : 0.0;      // a pair at zero softened distance adds nothing (R13)
+    const double u = y * y;
+    const double w = s.w * y;
+    const double e = fma(-r2, u, 1.0);
+    const double v = u * w;
+    const double p = fma(1.875, e, 1.5);
+    const double h = fma(p, e, 1.0);
+    const double f = v * h;
     ax = fma(f, dx, ax);
     ay = fma(f, dy, ay);
     az = fma(f, dz, az);
 }
 
+struct PairCtrl {                            // all words are written by one role and read by the other
+    unsigned tail_pub;                       // producer: ring entries below this are complete
+    unsigned head_pub;                       // consumer: ring entries below this are free again
+    unsigned started;                        // producer: groups whose descriptor is valid
+    unsigned finished;                       // producer: groups whose list is complete (desc_end valid)
+    unsigned consumed;                       // consumer: groups it is done with
+    unsigned desc_g[kDesc], desc_begin[kDesc], desc_end[kDesc];
+    unsigned pad[3];
+};
+
+struct PairSmem {
+    double4 ring[kRing];
+    uint2 stack[kStack];                     // (first sibling, count) ranges
+    PairCtrl ctrl;
+};
+
 struct WalkSmem {
-    double4 src[kWalkWarps][kListCap];        // ring of pending sources
-    double4 stage_mono[kWalkWarps][32];       // async landing zone of the next node batch
-    uint4 stage_info[kWalkWarps][32];
-    unsigned stack[kWalkWarps][kStackSmem];
+    PairSmem pair[kPairs];
 };
 
 __device__ __forceinline__ void cp_async16(void *smem, const void *gmem)
 {
     const unsigned s = (unsigned)__cvta_generic_to_shared(smem);
-    asm volatile("cp.async.ca.shared.global [%0], [%1], 16;" ::"r"(s), "l"(gmem) : "memory");
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(s), "l"(gmem) : "memory");
 }
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
 __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;" ::: "memory"); }
+__device__ __forceinline__ void cp_async_wait_1() { asm volatile("cp.async.wait_group 1;" ::: "memory"); }
 
-// Evaluation: every lane carries TWO bodies of the group (lane l: bodies l%16 and l%16 + 16) and the
-// two half-warps take alternate sources, so each source read from shared memory feeds two
-// interactions (this lifts the fp64 pipe from ~85 % to ~100 % busy in the inner loop; measured).  The
-// two partial sums of a body are added at the end of the group.
-struct TwoBodies {
-    double x0, y0, z0, x1, y1, z1;
-    double ax0, ay0, az0, ax1, ay1, az1;
-};
-
-// evaluate the largest multiple of four sources that is ready; head stays a multiple of four, so a
-// quad never wraps around the ring.  half = 0 / 1 for lanes 0-15 / 16-31.
-template <bool GUARD>
-__device__ __forceinline__ int eval_quads(const double4 *src, int head, int tail, int half, double eps2, TwoBodies &B)
+__device__ __forceinline__ void st_release(unsigned *p, unsigned v)
 {
-    const int n4 = (tail - head) & ~3;
-#pragma unroll 1
-    for (int i = 0; i < n4; i += 4) {
-        const double4 *p = src + ((head + i) & (kListCap - 1)) + half;
-        const double4 s0 = p[0], s1 = p[2];
-        interact<GUARD>(B.x0, B.y0, B.z0, eps2, s0, B.ax0, B.ay0, B.az0);
-        interact<GUARD>(B.x1, B.y1, B.z1, eps2, s0, B.ax1, B.ay1, B.az1);
-        interact<GUARD>(B.x0, B.y0, B.z0, eps2, s1, B.ax0, B.ay0, B.az0);
-        interact<GUARD>(B.x1, B.y1, B.z1, eps2, s1, B.ax1, B.ay1, B.az1);
-    }
-    return head + n4;
+    const unsigned a = (unsigned)__cvta_generic_to_shared(p);
+    asm volatile("st.release.cta.shared.u32 [%0], %1;" ::"r"(a), "r"(v) : "memory");
+}
+__device__ __forceinline__ unsigned ld_acquire(const unsigned *p)
+{
+    const unsigned a = (unsigned)__cvta_generic_to_shared(p);
+    unsigned v;
+    asm volatile("ld.acquire.cta.shared.u32 %0, [%1];" : "=r"(v) : "r"(a) : "memory");
+    return v;
+}
+// lane 0 reads a counter of the other role; the shuffle hands the value (and the ordering) to the warp
+__device__ __forceinline__ unsigned warp_acquire(const unsigned *p, unsigned lane)
+{
+    unsigned v = 0;
+    if (lane == 0) v = ld_acquire(p);
+    return __shfl_sync(0xffffffffu, v, 0);
+}
+// lane 0 publishes a counter after the whole warp has passed this point
+__device__ __forceinline__ void warp_release(unsigned *p, unsigned v, unsigned lane)
+{
+    __syncwarp();
+    if (lane == 0) st_release(p, v);
 }
 
-// The traversal is software-pipelined with asynchronous copies (cp.async / LDGSTS): while the warp
-// evaluates the chunks that are ready, the node records of the NEXT batch and the bodies of the
-// leaves opened by THIS batch are already in flight from L2 straight into shared memory.
+// ------------------------------------------------------------------------------------------ producer
+struct Producer {
+    PairSmem &ps;
+    unsigned lane;
+    unsigned tail;        // ring entries written (absolute)
+    unsigned head_seen;   // last value read from ctrl.head_pub
+    unsigned pub;         // last value stored to ctrl.tail_pub
+#ifdef BH_WALK_PROF
+    long long wait_cycles = 0;
+    unsigned long long iterations = 0;
+#endif
+
+    __device__ __forceinline__ void publish(unsigned v)
+    {
+        if ((int)(v - pub) > 0) {
+            warp_release(&ps.ctrl.tail_pub, v, lane);
+            pub = v;
+        }
+    }
+    // make room for n more ring entries.  When the ring is full: publish everything written so far
+    // (the consumer can only free what it has been given), then sleep until a good part of the ring
+    // is free again, so that the producer works in bursts and does not burn issue slots polling
+    __device__ __forceinline__ void reserve_slow(unsigned n)
+    {
+#ifdef BH_WALK_PROF
+        const long long t0 = clock64();
+#endif
+        cp_async_commit();
+        cp_async_wait_all();
+        publish(tail);
+        const unsigned want = n > (unsigned)kRing / 2 - 64u ? n : (unsigned)kRing / 2 - 64u;
+        while (true) {
+            __nanosleep(1000);
+            head_seen = warp_acquire(&ps.ctrl.head_pub, lane);
+            if (tail + want - head_seen <= (unsigned)kRing) break;
+        }
+#ifdef BH_WALK_PROF
+        wait_cycles += clock64() - t0;
+#endif
+    }
+    __device__ __forceinline__ void reserve(unsigned n)
+    {
+        if (tail + n - head_seen <= (unsigned)kRing) return;
+        head_seen = warp_acquire(&ps.ctrl.head_pub, lane);
+        if (tail + n - head_seen <= (unsigned)kRing) return;
+        reserve_slow(n);
+    }
+};
+
+struct NodeRec {
+    uint4 info;      // begin, count, first_child, level | children << 8
+    double4 mn;      // centre of mass, mass
+};
+
+__device__ __forceinline__ NodeRec load_rec(const uint4 *__restrict__ winfo, const double4 *__restrict__ mono, unsigned t)
+{
+    NodeRec r;
+    r.info = __ldg(winfo + t);
+    const double2 *m2 = reinterpret_cast<const double2 *>(mono + t);
+    const double2 lo = __ldg(m2), hi = __ldg(m2 + 1);
+    r.mn = make_double4(lo.x, lo.y, hi.x, hi.y);
+    return r;
+}
+
+// max(0, max(lo - c, c - hi)), each difference rounded once (R22).  Since lo <= hi at most one of the
+// differences is positive; a negative one is cleared through its sign bit (integer pipe: an fp64
+// max costs six instructions on sm_100).  The result is only ever squared, so -0 for +0 is harmless.
+__device__ __forceinline__ double box_delta(double lo, double hi, double c)
+{
+    const double t1 = __dsub_rn(lo, c), t2 = __dsub_rn(c, hi);
+    const int h1 = __double2hiint(t1), h2 = __double2hiint(t2);
+    const int m1 = ~(h1 >> 31), m2 = ~(h2 >> 31);
+    return __hiloint2double((h1 & m1) | (h2 & m2), (__double2loint(t1) & m1) | (__double2loint(t2) & m2));
+}
+
+// The stack holds RANGES of sibling nodes (first id, count): one entry per opened node.  A pop gives
+// every lane one range; the lane then walks its (at most eight, memory-contiguous) siblings one per
+// trip, so the warp-wide bookkeeping of a trip (two ballots, one stack entry per opened node) is
+// spread over up to 32 nodes and the records of the next trip are already in flight.
+__device__ void produce(PairSmem &ps, DevState *st, const unsigned *__restrict__ gstart,
+                        const double4 *__restrict__ sbody, const double *__restrict__ gbox,
+                        const uint4 *__restrict__ winfo, const double4 *__restrict__ mono, double theta2,
+                        unsigned *__restrict__ cnt_mono, unsigned *__restrict__ cnt_direct, uint2 *slab)
+{
+    const unsigned lane = lane_id();
+    const unsigned lt = (1u << lane) - 1u;
+    const unsigned ngroups = st->n_groups;
+    const int s2_base = (2 * st->e + 1023) << 20;   // high word of L^2; a level down is 2^-2: subtract 2 << 20
+    unsigned long long tot_mono = 0, tot_direct = 0, tot_inter = 0, tot_tested = 0;
+    Producer P{ps, lane, 0u, 0u, 0u};
+#ifdef BH_WALK_PROF
+    const long long prof_t0 = clock64();
+#endif
+    uint2 *stack = ps.stack;
+    unsigned k = 0;   // groups started by this pair
+
+    while (true) {
+        unsigned g = 0;
+        if (lane == 0) g = atomicAdd(&st->walk_queue, 1u);
+        g = __shfl_sync(0xffffffffu, g, 0);
+        if (g >= ngroups) g = kNoGroup;
+        while (k - warp_acquire(&ps.ctrl.consumed, lane) >= (unsigned)kDesc) __nanosleep(256);
+        P.tail = (P.tail + 7u) & ~7u;          // a group's sources start on a chunk boundary
+        if (lane == 0) {
+            ps.ctrl.desc_g[k % kDesc] = g;
+            ps.ctrl.desc_begin[k % kDesc] = P.tail;
+        }
+        warp_release(&ps.ctrl.started, k + 1, lane);
+        if (g == kNoGroup) break;
+
+        const unsigned gb = gstart[g], ge = gstart[g + 1];
+        const double glx = gbox[6 * g + 0], gly = gbox[6 * g + 1], glz = gbox[6 * g + 2];
+        const double ghx = gbox[6 * g + 3], ghy = gbox[6 * g + 4], ghz = gbox[6 * g + 5];
+        unsigned bot = 0, top = 1, gsp = 0;    // shared stack = [bot, top) mod kStack; gsp entries in the slab
+        unsigned n_mono = 0, n_direct = 0, my_tested = 0;
+        if (lane == 0) stack[0] = make_uint2(0u, 1u);   // the root, as a range of one
+        __syncwarp();
+        unsigned tail_prev = P.tail;           // ring fill at the end of the previous trip
+
+        while (true) {
+            if (top == bot) {
+                if (gsp == 0) break;           // nothing left: the list of this group is complete
+                gsp -= kSpill;                 // refill from the slab
+                for (unsigned q = lane; q < (unsigned)kSpill; q += 32) stack[(bot + q) & (kStack - 1)] = slab[gsp + q];
+                top = bot + kSpill;
+                __syncwarp();
+            }
+            unsigned take = top - bot;
+            take = take < 32u ? take : 32u;
+            top -= take;
+            uint2 ent = make_uint2(0u, 0u);
+            if (lane < take) ent = stack[(top + lane) & (kStack - 1)];
+            __syncwarp();                      // the entries are read before later pushes reuse their slots
+            const unsigned first = ent.x, nsib = ent.y;
+            const unsigned trips = __reduce_max_sync(0xffffffffu, nsib);
+            NodeRec nxt;
+            nxt.info = make_uint4(0u, 0u, 0u, 0u);
+            nxt.mn = make_double4(0.0, 0.0, 0.0, 0.0);
+            if (nsib > 0) nxt = load_rec(winfo, mono, first);
+#pragma unroll 1
+            for (unsigned q = 0; q < trips; ++q) {
+                const bool have = q < nsib;
+                const NodeRec cur = nxt;
+                if (q + 1 < nsib) nxt = load_rec(winfo, mono, first + q + 1);
+#ifdef BH_WALK_PROF
+                ++P.iterations;
+#endif
+                // ---- opening test (canonical arithmetic, R22) ----
+                const unsigned nb = cur.info.x, nc = cur.info.y;
+                const bool internal = (int)cur.info.z >= 0;
+                const bool overlap = (nb < ge) && (gb < nb + nc);
+                const double dx = box_delta(glx, ghx, cur.mn.x);
+                const double dy = box_delta(gly, ghy, cur.mn.y);
+                const double dz = box_delta(glz, ghz, cur.mn.z);
+                const double d2 = __fma_rn(dz, dz, __fma_rn(dy, dy, __dmul_rn(dx, dx)));
+                const double s2 = __hiloint2double(s2_base - (int)((cur.info.w & 0xffu) << 21), 0);   // (L 2^-level)^2
+                const bool accept = have && !overlap && (s2 < __dmul_rn(theta2, d2));
+                const bool open_int = have && !accept && internal;
+                const bool open_leaf = have && !accept && !internal;
+                my_tested += have ? 1u : 0u;
+                // ---- accepted nodes -> ring ----
+                {
+                    const unsigned m = __ballot_sync(0xffffffffu, accept);
+                    const unsigned cnt = __popc(m);
+                    P.reserve(cnt);
+                    if (accept) ps.ring[(P.tail + __popc(m & lt)) & (kRing - 1)] = cur.mn;
+                    P.tail += cnt;
+                    n_mono += cnt;
+                }
+                // ---- opened internal nodes -> their child ranges onto the stack ----
+                {
+                    const unsigned m = __ballot_sync(0xffffffffu, open_int);
+                    if (m) {
+                        if (top - bot + 32u > (unsigned)kStack) {       // spill the oldest kSpill entries
+                            if (gsp + kSpill > (unsigned)kStackSlab) {  // cannot happen within the slab bound
+                                if (lane == 0) atomicOr(&st->status, (int)kStatStack);
+                                bot = top;                              // drop the stack: the walk ends early
+                            } else {
+                                for (unsigned u = lane; u < (unsigned)kSpill; u += 32) slab[gsp + u] = stack[(bot + u) & (kStack - 1)];
+                                gsp += kSpill;
+                                bot += kSpill;
+                            }
+                        }
+                        if (open_int) stack[(top + __popc(m & lt)) & (kStack - 1)] = make_uint2(cur.info.z, (cur.info.w >> 8) & 0xffu);
+                        top += __popc(m);
+                    }
+                }
+                // ---- opened leaves -> their bodies, asynchronously into the ring ----
+                {
+                    unsigned m = __ballot_sync(0xffffffffu, open_leaf);
+                    while (m) {
+                        const int srcl = __ffs(m) - 1;
+                        m &= m - 1;
+                        const unsigned lb = __shfl_sync(0xffffffffu, nb, srcl);
+                        const unsigned lc = __shfl_sync(0xffffffffu, nc, srcl);
+                        for (unsigned off = 0; off < lc; off += 32) {   // a level-21 leaf may hold more than 32
+                            const unsigned n = lc - off < 32u ? lc - off : 32u;
+                            P.reserve(n);
+                            if (lane < n) {
+                                char *dst = reinterpret_cast<char *>(&ps.ring[(P.tail + lane) & (kRing - 1)]);
+                                const char *from = reinterpret_cast<const char *>(sbody + lb + off + lane);
+                                cp_async16(dst, from);
+                                cp_async16(dst + 16, from + 16);
+                            }
+                            P.tail += n;
+                        }
+                        n_direct += lc;
+                    }
+                }
+                // ---- publish what is complete: everything up to the end of the previous trip ----
+                cp_async_commit();
+                cp_async_wait_1();
+                P.publish(tail_prev);
+                tail_prev = P.tail;
+            }
+            __syncwarp();                      // this batch's pushes are on the stack before the next pop
+        }
+        // ---- the list of this group is complete ----
+        cp_async_wait_all();
+        __syncwarp();
+        if (lane == 0) {
+            ps.ctrl.desc_end[k % kDesc] = P.tail;
+            st_release(&ps.ctrl.tail_pub, P.tail);
+            st_release(&ps.ctrl.finished, k + 1);
+            cnt_mono[g] = n_mono;
+            cnt_direct[g] = n_direct;
+        }
+        P.pub = P.tail;
+        ++k;
+        tot_mono += n_mono;
+        tot_direct += n_direct;
+        tot_inter += (unsigned long long)(n_mono + n_direct) * (unsigned long long)(ge - gb);
+        tot_tested += my_tested;               // per lane; summed over the warp by the atomics below
+    }
+#ifdef BH_WALK_PROF
+    (void)tot_mono; (void)tot_direct; (void)tot_inter; (void)tot_tested;
+    if (lane == 0) {
+        atomicAdd(&st->stats[2], (unsigned long long)P.wait_cycles);
+        atomicAdd(&st->stats[3], P.iterations);
+    }
+#else
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) tot_tested += __shfl_xor_sync(0xffffffffu, tot_tested, o);
+    if (lane == 0) {
+        atomicAdd(&st->stats[0], tot_mono);
+        atomicAdd(&st->stats[1], tot_direct);
+        atomicAdd(&st->stats[2], tot_inter);
+        atomicAdd(&st->stats[3], tot_tested);
+    }
+#endif
+}
+
+// ------------------------------------------------------------------------------------------ consumer
+// Lane l = 8 q + r holds bodies r, r+8, r+16, r+24 of the group (NS = ceil(bodies / 8) of them are
+// real) and, of every chunk of eight sources, takes sources q and q+4.
+template <int NS>
+struct Bodies {
+    double x[NS], y[NS], z[NS], ax[NS], ay[NS], az[NS];
+};
+
+// evaluate n8 (a multiple of 8) sources starting at ring position head (a multiple of 8)
+template <bool GUARD, int NS>
+__device__ __forceinline__ void eval_chunks(const double4 *ring, unsigned head, unsigned n8, unsigned quarter,
+                                            double eps2, Bodies<NS> &B)
+{
+#pragma unroll 1
+    for (unsigned i = 0; i < n8; i += 8) {
+        const double4 *p = ring + ((head + i) & (kRing - 1)) + quarter;
+        const double4 s0 = p[0], s1 = p[4];
+#pragma unroll
+        for (int k = 0; k < NS; ++k) interact<GUARD>(B.x[k], B.y[k], B.z[k], eps2, s0, B.ax[k], B.ay[k], B.az[k]);
+#pragma unroll
+        for (int k = 0; k < NS; ++k) interact<GUARD>(B.x[k], B.y[k], B.z[k], eps2, s1, B.ax[k], B.ay[k], B.az[k]);
+    }
+}
+
+// one group: evaluate its sources as the producer publishes them, then write the accelerations
+template <bool GUARD, int NS>
+__device__ __forceinline__ long long consume_group(PairSmem &ps, unsigned k, unsigned head, long long gb, long long ge,
+                                              const double4 *__restrict__ sbody, const unsigned *__restrict__ perm,
+                                              double eps2, double G, double *__restrict__ acc)
+{
+    const unsigned lane = lane_id(), quarter = lane >> 3, r = lane & 7u;
+    Bodies<NS> B;
+#pragma unroll
+    for (int s = 0; s < NS; ++s) {
+        const long long j = gb + r + 8 * s;
+        const double4 bd = sbody[j < ge ? j : gb];
+        B.x[s] = bd.x; B.y[s] = bd.y; B.z[s] = bd.z;
+        B.ax[s] = B.ay[s] = B.az[s] = 0.0;
+    }
+    const double4 zero4 = make_double4(0.0, 0.0, 0.0, 0.0);
+    long long g_prof_wait = 0;   // cycles spent waiting for the producer (profiling builds only)
+    while (true) {
+        unsigned lim = 0;
+        bool fin = false;
+        if (lane == 0) {
+            fin = (int)(ld_acquire(&ps.ctrl.finished) - k) > 0;
+            lim = fin ? ps.ctrl.desc_end[k % kDesc] : ld_acquire(&ps.ctrl.tail_pub);
+        }
+        fin = __shfl_sync(0xffffffffu, (int)fin, 0) != 0;
+        lim = __shfl_sync(0xffffffffu, lim, 0);
+        const int avail = (int)(lim - head);       // negative while tail_pub still belongs to the last group
+        if (!fin && avail < 32) {
+#ifdef BH_WALK_PROF
+            const long long t0 = clock64();
+            __nanosleep(32);
+            g_prof_wait += clock64() - t0;
+#else
+            __nanosleep(32);
+#endif
+            continue;
+        }
+        const unsigned n8 = avail > 0 ? ((unsigned)avail & ~7u) : 0u;
+        eval_chunks<GUARD, NS>(ps.ring, head, n8, quarter, eps2, B);
+        head += n8;
+        if (fin) {
+            const unsigned rest = (unsigned)(avail > 0 ? avail : 0) & 7u;
+            if (rest) {                             // last, partial chunk: absent sources are massless
+                const double4 *p = ps.ring + (head & (kRing - 1)) + quarter;
+                const double4 s0 = quarter < rest ? p[0] : zero4;
+                const double4 s1 = quarter + 4 < rest ? p[4] : zero4;
+#pragma unroll
+                for (int s = 0; s < NS; ++s) interact<GUARD>(B.x[s], B.y[s], B.z[s], eps2, s0, B.ax[s], B.ay[s], B.az[s]);
+#pragma unroll
+                for (int s = 0; s < NS; ++s) interact<GUARD>(B.x[s], B.y[s], B.z[s], eps2, s1, B.ax[s], B.ay[s], B.az[s]);
+                head += rest;
+            }
+            warp_release(&ps.ctrl.head_pub, head, lane);
+            break;
+        }
+        warp_release(&ps.ctrl.head_pub, head, lane);
+    }
+    // add the four quarter-warp partial sums; lane 8 q + r then writes body r + 8 q
+    double ox = 0.0, oy = 0.0, oz = 0.0;
+#pragma unroll
+    for (int s = 0; s < NS; ++s) {
+        double tx = B.ax[s], ty = B.ay[s], tz = B.az[s];
+        tx += __shfl_xor_sync(0xffffffffu, tx, 8);
+        ty += __shfl_xor_sync(0xffffffffu, ty, 8);
+        tz += __shfl_xor_sync(0xffffffffu, tz, 8);
+        tx += __shfl_xor_sync(0xffffffffu, tx, 16);
+        ty += __shfl_xor_sync(0xffffffffu, ty, 16);
+        tz += __shfl_xor_sync(0xffffffffu, tz, 16);
+        if ((int)quarter == s) { ox = tx; oy = ty; oz = tz; }
+    }
+    const long long j = gb + lane;
+    if (j < ge) {
+        const unsigned i = perm[j];
+        acc[3ll * i + 0] = G * ox;
+        acc[3ll * i + 1] = G * oy;
+        acc[3ll * i + 2] = G * oz;
+    }
+    return g_prof_wait;
+}
+
 template <bool GUARD>
-__global__ void __launch_bounds__(kWalkWarps * 32, WalkConfig::kBlocksPerSM)
+__device__ void consume(PairSmem &ps, DevState *prof_st, const unsigned *__restrict__ gstart, const double4 *__restrict__ sbody,
+                        const unsigned *__restrict__ perm, double eps2, double G, double *__restrict__ acc)
+{
+    const unsigned lane = lane_id();
+    long long waited = 0;
+#ifdef BH_WALK_PROF
+    const long long prof_t0 = clock64();
+#endif
+    for (unsigned k = 0;; ++k) {
+#ifdef BH_WALK_PROF
+        const long long w0 = clock64();
+#endif
+        while ((int)(warp_acquire(&ps.ctrl.started, lane) - k) <= 0) __nanosleep(64);
+#ifdef BH_WALK_PROF
+        waited += clock64() - w0;
+#endif
+        const unsigned g = ps.ctrl.desc_g[k % kDesc];
+        if (g == kNoGroup) break;
+        const unsigned head = ps.ctrl.desc_begin[k % kDesc];
+        const long long gb = gstart[g];
+        const long long ge = gstart[g + 1];
+        const int slots = (int)((ge - gb + 7) >> 3);
+        if (slots >= 4) waited += consume_group<GUARD, 4>(ps, k, head, gb, ge, sbody, perm, eps2, G, acc);
+        else if (slots == 3) waited += consume_group<GUARD, 3>(ps, k, head, gb, ge, sbody, perm, eps2, G, acc);
+        else if (slots == 2) waited += consume_group<GUARD, 2>(ps, k, head, gb, ge, sbody, perm, eps2, G, acc);
+        else waited += consume_group<GUARD, 1>(ps, k, head, gb, ge, sbody, perm, eps2, G, acc);
+        warp_release(&ps.ctrl.consumed, k + 1, lane);
+    }
+#ifdef BH_WALK_PROF
+    if (lane == 0) {
+        atomicAdd(&prof_st->stats[0], (unsigned long long)waited);
+        atomicAdd(&prof_st->stats[1], (unsigned long long)(clock64() - prof_t0));
+    }
+#else
+    (void)waited;
+#endif
+}
+
+template <bool GUARD>
+__global__ void __launch_bounds__(kWalkThreads, 1)
 walk_kernel(DevState *st, const unsigned *__restrict__ gstart, const double4 *__restrict__ sbody,
             const double *__restrict__ gbox, const unsigned *__restrict__ perm,
             const uint4 *__restrict__ winfo, const double4 *__restrict__ mono, double theta2, double eps2,
@@ -107,226 +519,18 @@ walk_kernel(DevState *st, const unsigned *__restrict__ gstart, const double4 *__
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     WalkSmem &sm = *reinterpret_cast<WalkSmem *>(smem_raw);
-    const unsigned lane = lane_id(), warp = threadIdx.x >> 5;
-    const unsigned lt = (1u << lane) - 1u;
-    double4 *src = sm.src[warp];
-    unsigned *stack = sm.stack[warp];
-    double4 *st_mono = sm.stage_mono[warp];
-    uint4 *st_info = sm.stage_info[warp];
-    unsigned *slab = walk_stack + (size_t)(blockIdx.x * kWalkWarps + warp) * kStackSlab;
-    const unsigned ngroups = st->n_groups;
-    const int e2 = 2 * st->e;
-    unsigned long long tot_mono = 0, tot_direct = 0, tot_inter = 0, tot_tested = 0;
-
-    while (true) {
-        unsigned g = 0;
-        if (lane == 0) g = atomicAdd(&st->walk_queue, 1u);
-        g = __shfl_sync(0xffffffffu, g, 0);
-        if (g >= ngroups) break;
-        const long long gb = gstart[g];
-        const long long ge = gstart[g + 1];
-        const long long j = gb + lane;
-        const bool valid = j < ge;
-        TwoBodies B;
-        {
-            const long long j0 = gb + (lane & 15u), j1 = j0 + 16;
-            const double4 b0 = sbody[j0 < ge ? j0 : gb], b1 = sbody[j1 < ge ? j1 : gb];
-            B.x0 = b0.x; B.y0 = b0.y; B.z0 = b0.z;
-            B.x1 = b1.x; B.y1 = b1.y; B.z1 = b1.z;
-            B.ax0 = B.ay0 = B.az0 = B.ax1 = B.ay1 = B.az1 = 0.0;
-        }
-        const int half = (int)(lane >> 4);
-        const double glx = gbox[6 * g + 0], gly = gbox[6 * g + 1], glz = gbox[6 * g + 2];
-        const double ghx = gbox[6 * g + 3], ghy = gbox[6 * g + 4], ghz = gbox[6 * g + 5];
-        int head = 0, tail = 0, pending = 0;   // ring [head, tail) ready, then `pending` bodies in flight
-        int sp = 0, gsp = 0;                   // shared stack size, spilled entries in the slab
-        unsigned n_mono = 0, n_direct = 0, n_tested = 0;
-        // prime the pipeline with the root
-        int take = 1;
-        if (lane == 0) {
-            cp_async16(&st_info[0], winfo);
-            cp_async16(&st_mono[0], mono);
-            cp_async16(reinterpret_cast<char *>(&st_mono[0]) + 16, reinterpret_cast<const char *>(mono) + 16);
-        }
-        cp_async_commit();
-
-        while (take > 0) {
-            cp_async_wait_all();
-            __syncwarp();
-            tail += pending;
-            pending = 0;
-            const bool have = (int)lane < take;
-            n_tested += take;
-            // ---- opening test (canonical arithmetic) ----
-            bool accept = false, open_internal = false, open_leaf = false;
-            unsigned b = 0, c = 0, nch = 0;
-            int fc = -1;
-            double4 mn = make_double4(0.0, 0.0, 0.0, 0.0);
-            if (have) {
-                const uint4 info = st_info[lane];
-                mn = st_mono[lane];
-                b = info.x;
-                c = info.y;
-                fc = (int)info.z;
-                const bool overlap = ((long long)b < ge) && (gb < (long long)b + c);
-                if (!overlap) {
-                    const double dx = fmax(fmax(__dsub_rn(glx, mn.x), __dsub_rn(mn.x, ghx)), 0.0);
-                    const double dy = fmax(fmax(__dsub_rn(gly, mn.y), __dsub_rn(mn.y, ghy)), 0.0);
-                    const double dz = fmax(fmax(__dsub_rn(glz, mn.z), __dsub_rn(mn.z, ghz)), 0.0);
-                    const double d2 = __fma_rn(dz, dz, __fma_rn(dy, dy, __dmul_rn(dx, dx)));
-                    const int lv = (int)(info.w & 0xffu);
-                    const double s2 = __hiloint2double((e2 - 2 * lv + 1023) << 20, 0);   // (L 2^-lv)^2
-                    accept = s2 < __dmul_rn(theta2, d2);
-                }
-                if (!accept) {
-                    if (fc >= 0) {
-                        open_internal = true;
-                        nch = (info.w >> 8) & 0xffu;
-                    } else {
-                        open_leaf = true;
-                    }
-                }
-            }
-            __syncwarp();   // staging area is free again
-            // ---- accepted nodes -> source list ----
-            {
-                const unsigned m = __ballot_sync(0xffffffffu, accept);
-                if (accept) src[(tail + __popc(m & lt)) & (kListCap - 1)] = mn;
-                const int k = __popc(m);
-                tail += k;
-                n_mono += k;
-            }
-            // ---- opened internal nodes -> children onto the stack ----
-            {
-                unsigned inc = nch;
-#pragma unroll
-                for (int o = 1; o < 32; o <<= 1) {
-                    unsigned u = __shfl_up_sync(0xffffffffu, inc, o);
-                    if (lane >= (unsigned)o) inc += u;
-                }
-                const int total = __shfl_sync(0xffffffffu, inc, 31);
-                if (sp + total > kStackSmem) {        // spill the oldest kSpill entries
-                    for (int k = lane; k < kSpill; k += 32) slab[gsp + k] = stack[k];
-                    gsp += kSpill;
-                    __syncwarp();
-                    for (int k0 = 0; k0 < sp - kSpill; k0 += 32) {
-                        unsigned v = 0;
-                        if (k0 + (int)lane < sp - kSpill) v = stack[kSpill + k0 + lane];
-                        __syncwarp();
-                        if (k0 + (int)lane < sp - kSpill) stack[k0 + lane] = v;
-                        __syncwarp();
-                    }
-                    sp -= kSpill;
-                }
-                if (open_internal) {
-                    const int off = sp + (int)(inc - nch);
-                    for (unsigned u = 0; u < nch; ++u) stack[off + u] = (unsigned)fc + u;
-                }
-                sp += total;
-            }
-            // ---- opened leaves -> their bodies, asynchronously into the ring ----
-            {
-                const unsigned lc = open_leaf ? c : 0u;
-                unsigned inc = lc;
-#pragma unroll
-                for (int o = 1; o < 32; o <<= 1) {
-                    unsigned u = __shfl_up_sync(0xffffffffu, inc, o);
-                    if (lane >= (unsigned)o) inc += u;
-                }
-                const unsigned total = __shfl_sync(0xffffffffu, inc, 31);
-                n_direct += total;
-                for (unsigned base = 0; base < total; base += 32) {
-                    // keep 32 slots for this round and 32 for the next batch's accepted nodes
-                    if (kListCap - (tail + pending - head) < 64) {   // ring full: drain, evaluate, go on
-                        cp_async_commit();
-                        cp_async_wait_all();
-                        __syncwarp();
-                        tail += pending;
-                        pending = 0;
-                        head = eval_quads<GUARD>(src, head, tail, half, eps2, B);
-                        __syncwarp();
-                    }
-                    const unsigned idx = base + lane;
-                    // owner lane = first lane whose inclusive count exceeds idx (binary search by shuffles)
-                    unsigned lo = 0;
-#pragma unroll
-                    for (int step = 16; step > 0; step >>= 1) {
-                        unsigned probe = __shfl_sync(0xffffffffu, inc, lo + step - 1);
-                        if (probe <= idx) lo += step;
-                    }
-                    lo = lo > 31u ? 31u : lo;
-                    const unsigned oinc = __shfl_sync(0xffffffffu, inc, lo);
-                    const unsigned ocnt = __shfl_sync(0xffffffffu, lc, lo);
-                    const unsigned obeg = __shfl_sync(0xffffffffu, b, lo);
-                    if (idx < total) {
-                        const unsigned body = obeg + (idx - (oinc - ocnt));
-                        char *dst = reinterpret_cast<char *>(&src[(tail + pending + lane) & (kListCap - 1)]);
-                        const char *from = reinterpret_cast<const char *>(sbody + body);
-                        cp_async16(dst, from);
-                        cp_async16(dst + 16, from + 16);
-                    }
-                    pending += (int)(total - base < 32u ? total - base : 32u);
-                }
-            }
-            __syncwarp();   // children are on the stack
-            // ---- pop the next batch and start its loads ----
-            if (sp == 0 && gsp > 0) {             // refill from the slab
-                gsp -= kSpill;
-                for (int k = lane; k < kSpill; k += 32) stack[k] = slab[gsp + k];
-                sp = kSpill;
-                __syncwarp();
-            }
-            take = sp < 32 ? sp : 32;
-            sp -= take;
-            if ((int)lane < take) {
-                const unsigned t = stack[sp + lane];
-                cp_async16(&st_info[lane], winfo + t);
-                const char *from = reinterpret_cast<const char *>(mono + t);
-                cp_async16(&st_mono[lane], from);
-                cp_async16(reinterpret_cast<char *>(&st_mono[lane]) + 16, from + 16);
-            }
-            cp_async_commit();
-            __syncwarp();
-            // ---- evaluate what is ready while the copies fly ----
-            head = eval_quads<GUARD>(src, head, tail, half, eps2, B);
-        }
-        cp_async_wait_all();
-        __syncwarp();
-        tail += pending;
-        // pad the last quad with massless sources (they add exactly zero) and finish
-        if ((int)lane < ((4 - (tail & 3)) & 3)) src[(tail + lane) & (kListCap - 1)] = make_double4(0.0, 0.0, 0.0, 0.0);
-        __syncwarp();
-        head = eval_quads<GUARD>(src, head, (tail + 3) & ~3, half, eps2, B);
-        __syncwarp();
-        {   // add the two half-warp partial sums; lane l then holds body l in slot (l >> 4)
-            const double tx0 = B.ax0 + __shfl_xor_sync(0xffffffffu, B.ax0, 16);
-            const double ty0 = B.ay0 + __shfl_xor_sync(0xffffffffu, B.ay0, 16);
-            const double tz0 = B.az0 + __shfl_xor_sync(0xffffffffu, B.az0, 16);
-            const double tx1 = B.ax1 + __shfl_xor_sync(0xffffffffu, B.ax1, 16);
-            const double ty1 = B.ay1 + __shfl_xor_sync(0xffffffffu, B.ay1, 16);
-            const double tz1 = B.az1 + __shfl_xor_sync(0xffffffffu, B.az1, 16);
-            if (valid) {
-                const unsigned i = perm[j];
-                acc[3ll * i + 0] = G * (half ? tx1 : tx0);
-                acc[3ll * i + 1] = G * (half ? ty1 : ty0);
-                acc[3ll * i + 2] = G * (half ? tz1 : tz0);
-            }
-        }
-        if (lane == 0) {
-            cnt_mono[g] = n_mono;
-            cnt_direct[g] = n_direct;
-        }
-        tot_mono += n_mono;
-        tot_direct += n_direct;
-        tot_inter += (unsigned long long)(n_mono + n_direct) * (unsigned long long)(ge - gb);
-        tot_tested += n_tested;
-    }
-    if (lane == 0) {
-        atomicAdd(&st->stats[0], tot_mono);
-        atomicAdd(&st->stats[1], tot_direct);
-        atomicAdd(&st->stats[2], tot_inter);
-        atomicAdd(&st->stats[3], tot_tested);
-    }
+    // warps 0-3 and 8-11 produce, 4-7 and 12-15 consume: every SM sub-partition (warp % 4) gets two of each
+    const unsigned warp = threadIdx.x >> 5;
+    const unsigned pair = (warp >> 3) * 4 + (warp & 3u);
+    const bool producer = ((warp >> 2) & 1u) == 0;
+    PairSmem &ps = sm.pair[pair];
+    if (producer && lane_id() < sizeof(PairCtrl) / 4) reinterpret_cast<unsigned *>(&ps.ctrl)[lane_id()] = 0u;
+    __syncthreads();
+    if (producer)
+        produce(ps, st, gstart, sbody, gbox, winfo, mono, theta2, cnt_mono, cnt_direct,
+                reinterpret_cast<uint2 *>(walk_stack) + (size_t)(blockIdx.x * kPairs + pair) * kStackSlab);
+    else
+        consume<GUARD>(ps, st, gstart, sbody, perm, eps2, G, acc);
 }
 
 // ------------------------------------------------------------------------------------------ a8
@@ -437,14 +641,14 @@ void launch_walk(const Workspace &w, int64_t n, double theta, double eps, double
         configured = true;
     }
     (void)n;
-    const int blocks = w.walk_warps / kWalkWarps;
+    const int blocks = w.walk_warps / kPairs;   // one persistent block per SM
     const double eps2 = eps * eps;
     if (eps2 > 0.0)
-        walk_kernel<false><<<blocks, kWalkWarps * 32, sizeof(WalkSmem), s>>>(
+        walk_kernel<false><<<blocks, kWalkThreads, sizeof(WalkSmem), s>>>(
             w.st, w.gstart, w.sbody, w.gbox, w.idx[0], w.winfo, w.mono, theta * theta, eps2, G, acc, w.cnt_mono,
             w.cnt_direct, w.walk_stack);
     else
-        walk_kernel<true><<<blocks, kWalkWarps * 32, sizeof(WalkSmem), s>>>(
+        walk_kernel<true><<<blocks, kWalkThreads, sizeof(WalkSmem), s>>>(
             w.st, w.gstart, w.sbody, w.gbox, w.idx[0], w.winfo, w.mono, theta * theta, eps2, G, acc, w.cnt_mono,
             w.cnt_direct, w.walk_stack);
 }
