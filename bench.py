@@ -36,6 +36,9 @@ METRIC = "BH accel evals/s (build+walk) N=1M theta=0.5 fp64; speedup vs direct N
 UNIT = "body-accelerations/s"
 FLOPS_PER_INTERACTION = 20.0
 FP64_PEAK_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12      # derived: SMs x fp64 FMA lanes x 2 x max SM clock
+# dram__bytes_read.sum + dram__bytes_write.sum of one walk_kernel launch, from the committed ncu --set full
+# capture (profiles/r01_walk_ncu_full.md: 65.31 MB + 15.43 MB); a profiler figure, not measured by this run
+WALK_TRAFFIC_NCU = {"c4": 80.74e6}
 
 
 def workload_desc(w):
@@ -245,7 +248,8 @@ def run_own(args):
                 "peak_measured_dfma": peak_meas, "frac_of_measured_dfma": achieved / peak_meas,
                 "flops_per_interaction": FLOPS_PER_INTERACTION, "interactions_per_launch": inter_avg,
                 "interactions_per_s": inter_avg / (walk_avg_ms * 1e-3), "kernel_ms": walk_avg_ms,
-                "traffic": args.walk_traffic}
+                "traffic": args.walk_traffic if args.walk_traffic is not None else WALK_TRAFFIC_NCU.get(w.name),
+                "traffic_source": "profiles/r01_walk_ncu_full.md (ncu --set full, bytes per launch)"}
     # build kernels against HBM: algorithmic bytes per body over the build time
     build_ms = sum(phases[k] for k in ("cube", "keys", "sort", "gather", "tree", "monopoles"))
     build_bytes = 390.0 * w.n
