@@ -72,6 +72,7 @@ struct PairCtrl {                            // all words are written by one rol
 struct PairSmem {
     double4 ring[kRing];
     uint2 stack[kStack];                     // (first sibling, count) ranges
+    unsigned leaf_src[32];                   // producer scratch: (first body - offset in the run) per opened leaf
     PairCtrl ctrl;
 };
 
@@ -179,14 +180,18 @@ __device__ __forceinline__ NodeRec load_rec(const uint4 *__restrict__ winfo, con
 }
 
 // max(0, max(lo - c, c - hi)), each difference rounded once (R22).  Since lo <= hi at most one of the
-// differences is positive; a negative one is cleared through its sign bit (integer pipe: an fp64
-// max costs six instructions on sm_100).  The result is only ever squared, so -0 for +0 is harmless.
+// differences is positive, so the result is picked on the integer pipe (an fp64 max costs six
+// instructions on sm_100, and every instruction of a producer takes an issue slot from the fp64
+// warps): high word = max(h1, h2, 0) as signed integers, low word = that of t1 if t1 >= 0, else of
+// t2.  When neither difference is positive the high word is 0 and the low word arbitrary: a
+// subnormal whose square rounds to zero, and the result is only ever squared (so is -0 for +0).
 __device__ __forceinline__ double box_delta(double lo, double hi, double c)
 {
     const double t1 = __dsub_rn(lo, c), t2 = __dsub_rn(c, hi);
     const int h1 = __double2hiint(t1), h2 = __double2hiint(t2);
-    const int m1 = ~(h1 >> 31), m2 = ~(h2 >> 31);
-    return __hiloint2double((h1 & m1) | (h2 & m2), (__double2loint(t1) & m1) | (__double2loint(t2) & m2));
+    const int h = __vimax3_s32(h1, h2, 0);
+    const int l = h1 >= 0 ? __double2loint(t1) : __double2loint(t2);
+    return __hiloint2double(h, l);
 }
 
 // The stack holds RANGES of sibling nodes (first id, count): one entry per opened node.  A pop gives
@@ -302,25 +307,42 @@ __device__ void produce(PairSmem &ps, DevState *st, const unsigned *__restrict__
                     }
                 }
                 // ---- opened leaves -> their bodies, asynchronously into the ring ----
+                // All opened leaves of the trip are expanded together: a warp scan gives every leaf its
+                // offset in the run of bodies, the leaves leave (first body - offset) in a scratch row,
+                // and every lane then copies one body per window of 32, finding its leaf by counting
+                // the leaf starts at or before its slot.
                 {
-                    unsigned m = __ballot_sync(0xffffffffu, open_leaf);
-                    while (m) {
-                        const int srcl = __ffs(m) - 1;
-                        m &= m - 1;
-                        const unsigned lb = __shfl_sync(0xffffffffu, nb, srcl);
-                        const unsigned lc = __shfl_sync(0xffffffffu, nc, srcl);
-                        for (unsigned off = 0; off < lc; off += 32) {   // a level-21 leaf may hold more than 32
-                            const unsigned n = lc - off < 32u ? lc - off : 32u;
+                    const unsigned m = __ballot_sync(0xffffffffu, open_leaf);
+                    if (m) {
+                        const unsigned c = open_leaf ? nc : 0u;
+                        unsigned inc = c;
+#pragma unroll
+                        for (int o = 1; o < 32; o <<= 1) {
+                            const unsigned t = __shfl_up_sync(0xffffffffu, inc, o);
+                            if (lane >= (unsigned)o) inc += t;
+                        }
+                        const unsigned total = __shfl_sync(0xffffffffu, inc, 31);
+                        const unsigned excl = inc - c;
+                        if (open_leaf) ps.leaf_src[__popc(m & lt)] = nb - excl;
+                        __syncwarp();
+                        unsigned owners = 0;                           // leaves that start before this window
+                        for (unsigned base = 0; base < total; base += 32) {
+                            const unsigned rel = excl - base;
+                            const unsigned heads = __reduce_or_sync(0xffffffffu, (open_leaf && rel < 32u) ? 1u << rel : 0u);
+                            const unsigned k = owners + __popc(heads & (lt | (1u << lane))) - 1u;
+                            owners += __popc(heads);
+                            const unsigned n = total - base < 32u ? total - base : 32u;
                             P.reserve(n);
                             if (lane < n) {
                                 char *dst = reinterpret_cast<char *>(&ps.ring[(P.tail + lane) & (kRing - 1)]);
-                                const char *from = reinterpret_cast<const char *>(sbody + lb + off + lane);
+                                const char *from = reinterpret_cast<const char *>(sbody + (ps.leaf_src[k] + base + lane));
                                 cp_async16(dst, from);
                                 cp_async16(dst + 16, from + 16);
                             }
                             P.tail += n;
                         }
-                        n_direct += lc;
+                        n_direct += total;
+                        __syncwarp();                                  // the scratch row is read before it is rewritten
                     }
                 }
                 // ---- publish what is complete: everything up to the end of the previous trip ----
