@@ -34,6 +34,24 @@ constexpr int kStack = 512;                 // sibling ranges per producer in sh
 constexpr int kSpill = 128;                 // spill / refill unit
 constexpr int kDesc = 4;                    // group descriptors in flight per pair
 constexpr unsigned kNoGroup = 0xffffffffu;
+#ifndef BH_SLEEP_FULL
+#define BH_SLEEP_FULL 1000                  // ns a producer sleeps per poll while its ring is full
+#endif
+#ifndef BH_TRIP_UNROLL
+#define BH_TRIP_UNROLL 1
+#endif
+#ifndef BH_EVAL_UNROLL
+#define BH_EVAL_UNROLL 4
+#endif
+#ifndef BH_REG_PROD
+#define BH_REG_PROD 96                      // registers per thread of the producer warpgroups ...
+#define BH_REG_CONS 160                     // ... and of the consumer warpgroups (launch: 128)
+#endif
+constexpr int kTripUnroll = BH_TRIP_UNROLL;   // producer: trips of a pop unrolled
+constexpr int kEvalUnroll = BH_EVAL_UNROLL;   // consumer: chunks of eight sources unrolled
+#ifndef BH_PUB_MIN
+#define BH_PUB_MIN 0                        // a trip publishes only if at least this many entries are pending
+#endif
 
 // m / r^3 from r2 = |d|^2 + eps^2: MUFU.RSQ64H seed y (about 20 good bits), e = 1 - r2 y^2 and the
 // series (1-e)^(-3/2) = 1 + e (3/2 + 15/8 e) + O(e^3).  Every fp64 instruction except the three
@@ -147,7 +165,7 @@ struct Producer {
         publish(tail);
         const unsigned want = n > (unsigned)kRing / 2 - 64u ? n : (unsigned)kRing / 2 - 64u;
         while (true) {
-            __nanosleep(1000);
+            __nanosleep(BH_SLEEP_FULL);
             head_seen = warp_acquire(&ps.ctrl.head_pub, lane);
             if (tail + want - head_seen <= (unsigned)kRing) break;
         }
@@ -258,7 +276,7 @@ __device__ void produce(PairSmem &ps, DevState *st, const unsigned *__restrict__
             nxt.info = make_uint4(0u, 0u, 0u, 0u);
             nxt.mn = make_double4(0.0, 0.0, 0.0, 0.0);
             if (nsib > 0) nxt = load_rec(winfo, mono, first);
-#pragma unroll 1
+#pragma unroll kTripUnroll
             for (unsigned q = 0; q < trips; ++q) {
                 const bool have = q < nsib;
                 const NodeRec cur = nxt;
@@ -347,8 +365,10 @@ __device__ void produce(PairSmem &ps, DevState *st, const unsigned *__restrict__
                 }
                 // ---- publish what is complete: everything up to the end of the previous trip ----
                 cp_async_commit();
-                cp_async_wait_1();
-                P.publish(tail_prev);
+                if ((int)(tail_prev - P.pub) > BH_PUB_MIN) {
+                    cp_async_wait_1();
+                    P.publish(tail_prev);
+                }
                 tail_prev = P.tail;
             }
             __syncwarp();                      // this batch's pushes are on the stack before the next pop
@@ -401,7 +421,7 @@ template <bool GUARD, int NS>
 __device__ __forceinline__ void eval_chunks(const double4 *ring, unsigned head, unsigned n8, unsigned quarter,
                                             double eps2, Bodies<NS> &B)
 {
-#pragma unroll 1
+#pragma unroll kEvalUnroll
     for (unsigned i = 0; i < n8; i += 8) {
         const double4 *p = ring + ((head + i) & (kRing - 1)) + quarter;
         const double4 s0 = p[0], s1 = p[4];
@@ -548,6 +568,12 @@ walk_kernel(DevState *st, const unsigned *__restrict__ gstart, const double4 *__
     PairSmem &ps = sm.pair[pair];
     if (producer && lane_id() < sizeof(PairCtrl) / 4) reinterpret_cast<unsigned *>(&ps.ctrl)[lane_id()] = 0u;
     __syncthreads();
+#if BH_REG_PROD > 0
+    // the block is launched with 128 registers per thread; the producer warpgroups hand registers to
+    // the consumer warpgroups (warps 0-3 / 4-7 / 8-11 / 12-15 are the four warpgroups)
+    if (producer) asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(BH_REG_PROD));
+    else asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(BH_REG_CONS));
+#endif
     if (producer)
         produce(ps, st, gstart, sbody, gbox, winfo, mono, theta2, cnt_mono, cnt_direct,
                 reinterpret_cast<uint2 *>(walk_stack) + (size_t)(blockIdx.x * kPairs + pair) * kStackSlab);
