@@ -15,7 +15,12 @@
  * monopole against extended-precision totals; exact coverage of every walk list; theta=0 == direct
  * sum; a textbook per-body recursive Barnes-Hut (W=1, C=1); two-body / triangle / tetrahedron
  * closed forms; Newton's third law; brute force in exact rational arithmetic on tiny N; KDK
- * two-body orbit, dt^2 energy error, time reversal.  No function here is "parity unpinned".
+ * two-body orbit, dt^2 energy error, time reversal.  Rows "next" (O12-O16, tests/test_oracle_next.py):
+ * potential against the two-body closed form, exact-rational brute force and the finite-difference
+ * gradient (= minus the acceleration); theta=0 tree potential == direct potential; diagnostics against
+ * hand-computed systems; Eq. (7) on hand cases; Eq. (8) against the paper's "thousands of seconds";
+ * semi-implicit Euler: angular momentum exact for a central force, first-order energy error; the
+ * two-rate step against its closed form.  No function here is "parity unpinned".
  */
 #include <math.h>
 #include <stdint.h>
@@ -490,3 +495,129 @@ void orc_drift(double *pos, const double *vel, int64_t n, double dt)
 {
     for (int64_t i = 0; i < 3 * n; ++i) pos[i] = fma(vel[i], dt, pos[i]);
 }
+
+/* =============================================================================================
+ * Rows of SURVEY.md §8(f) ("next"): conservation diagnostics and the paper's stepping variants.
+ * ========================================================================================== */
+
+/* ---------------------------------------------------------------------------------------------
+ * O12  Gravitational potential with the lists of the walk (NEXT-1: "Conservation of
+ * energy, linear and angular momentum are checked for the purely gravitational case").  The paper
+ * prints no potential; the one consistent with the softened force of Eqs. (4)-(6) (its gradient is
+ * that force) is  phi_i = -G * sum_k m_k / sqrt(|d|^2 + eps^2),  nothing for a pair with r2 == 0,
+ * a body skips itself (reading R24).  Same groups, same opening test, same lists as O8.
+ * ------------------------------------------------------------------------------------------- */
+static inline void orc_pot_term(const long double p[3], const double *src, long double eps2, long double *s)
+{
+    long double dx = (long double)src[0] - p[0];
+    long double dy = (long double)src[1] - p[1];
+    long double dz = (long double)src[2] - p[2];
+    long double r2 = dx * dx + dy * dy + dz * dz + eps2;
+    if (r2 > 0.0L) *s += (long double)src[3] / sqrtl(r2);
+}
+
+void orc_potential(double L, int64_t n, const uint32_t *gstart, const uint8_t *level, const uint32_t *begin,
+                   const uint32_t *count, const int32_t *first_child, const uint8_t *child_mask,
+                   const double *mono, const double *sbody, const uint32_t *perm, const double *glo,
+                   const double *ghi, double theta, double eps, double G, int64_t g0, int64_t g1,
+                   double *phi)
+{
+    orc_tree_view T = {L, n, level, begin, count, first_child, child_mask, mono};
+    long double eps2 = (long double)eps * (long double)eps;
+#pragma omp parallel
+    {
+        orc_ivec lm = {0, 0, 0}, ld = {0, 0, 0};
+#pragma omp for schedule(dynamic, 4)
+        for (int64_t g = g0; g < g1; ++g) {
+            int64_t gb = gstart[g], ge = gstart[g + 1];
+            lm.n = 0;
+            ld.n = 0;
+            orc_visit(&T, 0, gb, ge, &glo[3 * g], &ghi[3 * g], theta * theta, &lm, &ld);
+            for (int64_t j = gb; j < ge; ++j) {
+                long double p[3] = {sbody[4 * j], sbody[4 * j + 1], sbody[4 * j + 2]};
+                long double s = 0.0L;
+                for (int64_t k = 0; k < lm.n; ++k) orc_pot_term(p, &mono[4 * (int64_t)lm.v[k]], eps2, &s);
+                for (int64_t k = 0; k < ld.n; ++k)
+                    if (ld.v[k] != j) orc_pot_term(p, &sbody[4 * (int64_t)ld.v[k]], eps2, &s);
+                phi[perm[j]] = (double)(-(long double)G * s);
+            }
+        }
+        free(lm.v);
+        free(ld.v);
+    }
+}
+
+/* O13  Direct potential: phi_i = -G sum_{k != i} m_k / sqrt(|R_ik|^2 + eps^2) (plain definition). */
+void orc_direct_potential(const double *pos, const double *mass, int64_t n, double eps, double G, double *phi)
+{
+    long double eps2 = (long double)eps * (long double)eps;
+#pragma omp parallel for schedule(dynamic, 16)
+    for (int64_t i = 0; i < n; ++i) {
+        long double p[3] = {pos[3 * i], pos[3 * i + 1], pos[3 * i + 2]};
+        long double s = 0.0L;
+        for (int64_t k = 0; k < n; ++k) {
+            if (k == i) continue;
+            double src[4] = {pos[3 * k], pos[3 * k + 1], pos[3 * k + 2], mass[k]};
+            orc_pot_term(p, src, eps2, &s);
+        }
+        phi[i] = (double)(-(long double)G * s);
+    }
+}
+
+/* ---------------------------------------------------------------------------------------------
+ * O14  Conserved quantities (energy, linear and angular momentum of the purely
+ * gravitational system).  out[0] = kinetic energy  1/2 sum m |v|^2;  out[1] = potential energy
+ * 1/2 sum m_i phi_i (every pair once; 0 if phi == NULL);  out[2..4] = linear momentum sum m v;
+ * out[5..7] = angular momentum sum m x cross v (about the origin).  Extended-precision sums.
+ * ------------------------------------------------------------------------------------------- */
+void orc_diagnostics(const double *pos, const double *vel, const double *mass, const double *phi, int64_t n,
+                     double out[8])
+{
+    long double ek = 0.0L, ep = 0.0L, P[3] = {0.0L, 0.0L, 0.0L}, Lm[3] = {0.0L, 0.0L, 0.0L};
+    for (int64_t i = 0; i < n; ++i) {
+        long double m = mass[i];
+        long double x = pos[3 * i], y = pos[3 * i + 1], z = pos[3 * i + 2];
+        long double vx = vel[3 * i], vy = vel[3 * i + 1], vz = vel[3 * i + 2];
+        ek += 0.5L * m * (vx * vx + vy * vy + vz * vz);
+        if (phi) ep += 0.5L * m * (long double)phi[i];
+        P[0] += m * vx;
+        P[1] += m * vy;
+        P[2] += m * vz;
+        Lm[0] += m * (y * vz - z * vy);
+        Lm[1] += m * (z * vx - x * vz);
+        Lm[2] += m * (x * vy - y * vx);
+    }
+    out[0] = (double)ek;
+    out[1] = (double)ep;
+    for (int c = 0; c < 3; ++c) {
+        out[2 + c] = (double)P[c];
+        out[5 + c] = (double)Lm[c];
+    }
+}
+
+/* ---------------------------------------------------------------------------------------------
+ * O15  Maximum relative position error, Eq. (7) PAPER.md:223:
+ *     e_i = |r_i - r_i,ref| / |r_i,ref| * 100   (per cent),   result = max_i e_i.
+ * Canonical arithmetic (compared bit for bit): d = r - r_ref per component (one rounding each);
+ * |.|^2 = fma(z, z, fma(y, y, x*x));  e_i = 100 * sqrt(|d|^2 / |r_ref|^2).  A reference position at
+ * the origin (|r_ref|^2 == 0) has no relative error and is skipped (reading R25).
+ * ------------------------------------------------------------------------------------------- */
+double orc_position_error(const double *pos, const double *ref, int64_t n)
+{
+    double worst = 0.0;
+    for (int64_t i = 0; i < n; ++i) {
+        double dx = pos[3 * i] - ref[3 * i], dy = pos[3 * i + 1] - ref[3 * i + 1], dz = pos[3 * i + 2] - ref[3 * i + 2];
+        double nd = fma(dz, dz, fma(dy, dy, dx * dx));
+        double nr = fma(ref[3 * i + 2], ref[3 * i + 2], fma(ref[3 * i + 1], ref[3 * i + 1], ref[3 * i] * ref[3 * i]));
+        if (nr == 0.0) continue;
+        double e = 100.0 * sqrt(nd / nr);
+        if (e > worst) worst = e;
+    }
+    return worst;
+}
+
+/* ---------------------------------------------------------------------------------------------
+ * O16  Gravity time-step bound, Eq. (8):  dt_g < T_g / 2 = 1 / (2 sqrt(G rho)).
+ * Returns the bound 1 / (2 sqrt(G rho)).
+ * ------------------------------------------------------------------------------------------- */
+double orc_gravity_dt(double G, double rho) { return 1.0 / (2.0 * sqrt(G * rho)); }

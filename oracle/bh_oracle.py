@@ -264,3 +264,90 @@ class Leapfrog:
         drift(self.pos, self.vel, dt)
         self.acc = self._eval()
         kick(self.vel, self.acc, dt * 0.5)
+
+
+# ------------------------------------------------------------------ rows "next" of SURVEY.md §8(f)
+def potential(t: Tree, theta: float, eps: float, G: float, g0: int = 0, g1: int | None = None):
+    """O12: tree potential of the bodies of groups [g0,g1) -> phi[n] in ORIGINAL order (others NaN)."""
+    if g1 is None:
+        g1 = t.ngroups
+    phi = np.full(t.n, np.nan)
+    lib().orc_potential(C.c_double(t.L), C.c_int64(t.n), _p(t.gstart), _p(t.level), _p(t.begin),
+                        _p(t.count), _p(t.first_child), _p(t.child_mask), _p(t.mono), _p(t.sbody),
+                        _p(t.perm), _p(t.glo), _p(t.ghi), C.c_double(theta), C.c_double(eps),
+                        C.c_double(G), C.c_int64(g0), C.c_int64(g1), _p(phi))
+    return phi
+
+
+def direct_potential(pos, mass, eps: float, G: float):
+    """O13: phi_i = -G sum_{k != i} m_k / sqrt(|R_ik|^2 + eps^2)."""
+    pos = np.ascontiguousarray(pos, dtype=np.float64)
+    mass = np.ascontiguousarray(mass, dtype=np.float64)
+    phi = np.zeros(pos.shape[0])
+    lib().orc_direct_potential(_p(pos), _p(mass), C.c_int64(pos.shape[0]), C.c_double(eps),
+                               C.c_double(G), _p(phi))
+    return phi
+
+
+def diagnostics(pos, vel, mass, phi=None):
+    """O14 -> dict(ekin, epot, P[3], L[3])."""
+    pos = np.ascontiguousarray(pos, dtype=np.float64)
+    vel = np.ascontiguousarray(vel, dtype=np.float64)
+    mass = np.ascontiguousarray(mass, dtype=np.float64)
+    out = np.zeros(8)
+    if phi is not None:
+        phi = np.ascontiguousarray(phi, dtype=np.float64)
+    lib().orc_diagnostics(_p(pos), _p(vel), _p(mass), _p(phi) if phi is not None else None,
+                          C.c_int64(pos.shape[0]), _p(out))
+    return {"ekin": out[0], "epot": out[1], "P": out[2:5].copy(), "L": out[5:8].copy()}
+
+
+def position_error(pos, ref) -> float:
+    """O15: Eq. (7), max over bodies, per cent."""
+    pos = np.ascontiguousarray(pos, dtype=np.float64)
+    ref = np.ascontiguousarray(ref, dtype=np.float64)
+    lib().orc_position_error.restype = C.c_double
+    return float(lib().orc_position_error(_p(pos), _p(ref), C.c_int64(pos.shape[0])))
+
+
+def gravity_dt(G: float, rho: float) -> float:
+    """O16: Eq. (8) bound 1 / (2 sqrt(G rho))."""
+    lib().orc_gravity_dt.restype = C.c_double
+    return float(lib().orc_gravity_dt(C.c_double(G), C.c_double(rho)))
+
+
+class Stepper:
+    """The paper's stepping variants (NEXT-2), composed of the C kick / drift / evaluation steps.
+
+    euler(dt): semi-implicit (symplectic) Euler, the paper's preferred stepper:
+        a = a(x_k);  v_{k+1} = fma(a, dt, v_k);  x_{k+1} = fma(v_{k+1}, dt, x_k).
+    multirate(dt_c, n_sub): PAPER.md:338-340 — "we advance the simulation of dt_c ... but we evaluate
+        gravity (through N^2 interactions or by building the octree) every dt_g": one evaluation
+        a = a(x_k), then n_sub semi-implicit Euler sub-steps of dt_c with that same a (dt_g = n_sub dt_c;
+        with contacts out of scope nothing else acts between evaluations).
+    """
+
+    def __init__(self, pos, vel, mass, theta, eps, G, leaf_cap, W=32, use_direct=False):
+        self.pos = np.array(pos, dtype=np.float64, order="C")
+        self.vel = np.array(vel, dtype=np.float64, order="C")
+        self.mass = np.ascontiguousarray(mass, dtype=np.float64)
+        self.theta, self.eps, self.G, self.C, self.W = theta, eps, G, leaf_cap, W
+        self.use_direct = use_direct
+        self.acc = None
+
+    def _eval(self):
+        if self.use_direct:
+            return direct(self.pos, self.mass, self.eps, self.G)
+        t = build(self.pos, self.mass, self.C, self.W)
+        return accel(t, self.theta, self.eps, self.G)[0]
+
+    def euler(self, dt: float):
+        self.acc = self._eval()
+        kick(self.vel, self.acc, dt)
+        drift(self.pos, self.vel, dt)
+
+    def multirate(self, dt_c: float, n_sub: int):
+        self.acc = self._eval()
+        for _ in range(n_sub):
+            kick(self.vel, self.acc, dt_c)
+            drift(self.pos, self.vel, dt_c)
