@@ -88,6 +88,52 @@ bh_status bh_bind_state(bh_ctx *ctx, double *pos_dev, double *vel_dev, const dou
 bh_status bh_kdk_step(bh_ctx *ctx, double dt);
 /* Device pointer to the accelerations [n][3] held by the bound state (valid after a step). */
 bh_status bh_get_state_acc(bh_ctx *ctx, const double **acc_dev);
+/* Copy the accelerations [n][3] of the last evaluation a stepper made (bh_kdk_step: a(x) at the new
+ * positions; bh_euler_step / bh_multirate_step: a(x_k) at the positions the step started from) into
+ * acc_dev.  BH_ERR_STATE before the first step. */
+bh_status bh_copy_state_acc(bh_ctx *ctx, double *acc_dev);
+
+/* ---- rows "next" of SURVEY.md 8(f): the paper's stepping variants and conservation diagnostics ---- */
+
+/* Semi-implicit (symplectic) Euler, the paper's preferred stepper, on the state of
+ * bh_bind_state:  rebuild tree;  a = accel(x_k);  v_k+1 = fma(a, dt, v_k);  x_k+1 = fma(v_k+1, dt, x_k).
+ * One evaluation per step.  Afterwards the context holds a(x_k), so a following bh_kdk_step starts by
+ * evaluating a(x) again. */
+bh_status bh_euler_step(bh_ctx *ctx, double dt);
+
+/* Two-rate stepping, PAPER.md:338-340 ("we advance the simulation of dt_c ... but we evaluate gravity
+ * (through N^2 interactions or by building the octree) every dt_g"): one evaluation a = accel(x_k), then
+ * n_sub >= 1 semi-implicit Euler sub-steps of dt_c with that same a (dt_g = n_sub dt_c; contacts are out
+ * of scope, so nothing else acts between evaluations).  Bit-identical to n_sub separate updates. */
+bh_status bh_multirate_step(bh_ctx *ctx, double dt_c, int n_sub);
+
+/* Gravitational potential of every body of the last build with the interaction lists of bh_accel
+ * (same groups, same opening test):  phi_i = -G sum_k m_k / sqrt(|d|^2 + eps^2), a body skips itself, a
+ * pair at zero softened distance adds nothing (R24: the potential whose gradient is the force of
+ * Eqs. (4)-(6) PAPER.md:90-101; the paper checks energy conservation, but prints no
+ * potential).  phi_dev is [n] in bh_build order.  Overwrites the counters read by bh_get_counts/stats. */
+bh_status bh_potential(bh_ctx *ctx, double theta, double eps, double G, double *phi_dev);
+
+/* Direct-sum potential over all ordered pairs (the plain definition of the same phi). phi_dev [n]. */
+bh_status bh_direct_potential(bh_ctx *ctx, double eps, double G, double *phi_dev);
+
+/* Synchronising. Conserved quantities of n bodies given as device arrays:
+ * out_host[0] = kinetic energy 1/2 sum m |v|^2;  [1] = potential energy 1/2 sum m_i phi_i (0 if phi_dev
+ * is NULL);  [2..4] = linear momentum sum m v;  [5..7] = angular momentum sum m x cross v about the
+ * origin.  Accumulated in double-double in a fixed order: reproducible run to run, and exact to fp64
+ * rounding of the true sum of the fp64 inputs.  Needs no prior build. */
+bh_status bh_diagnostics(bh_ctx *ctx, const double *pos_dev, const double *vel_dev, const double *mass_dev,
+                         const double *phi_dev, int64_t n, double out_host[8]);
+
+/* Synchronising. Maximum relative position error in per cent, Eq. (7) PAPER.md:223:
+ * max_i 100 |r_i - r_i,ref| / |r_i,ref|, with |.|^2 = fma(z,z,fma(y,y,x*x)), e_i = 100 sqrt(|d|^2/|r_ref|^2),
+ * every operation IEEE-rounded once (bit-reproducible); bodies with r_ref at the origin are skipped (R25).
+ * pos_dev, ref_dev are [n][3]. */
+bh_status bh_position_error(bh_ctx *ctx, const double *pos_dev, const double *ref_dev, int64_t n,
+                            double *err_host);
+
+/* Host helper. Upper bound of the gravity time step, Eq. (8): 1 / (2 sqrt(G rho)). */
+double bh_gravity_dt(double G, double rho);
 
 /* End-to-end evaluation from HOST buffers: copies pos_host [n][3] and mass_host [n] to the GPU,
  * builds, walks, copies acc_host [n][3] back and waits.  Pinned host memory makes the copies

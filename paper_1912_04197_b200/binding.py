@@ -41,6 +41,8 @@ def lib() -> C.CDLL:
         L.bh_last_error.restype = C.c_char_p
         L.bh_last_error.argtypes = [vp]
         L.bh_version.restype = C.c_char_p
+        L.bh_gravity_dt.restype = dbl
+        L.bh_gravity_dt.argtypes = [dbl, dbl]
         sigs = {
             "bh_create": [C.POINTER(vp), i64, i32, i32, vp, C.c_size_t, vp],
             "bh_destroy": [vp], "bh_set_stream": [vp, vp],
@@ -51,6 +53,13 @@ def lib() -> C.CDLL:
             "bh_bind_state": [vp, vp, vp, vp, i64, dbl, dbl, dbl],
             "bh_kdk_step": [vp, dbl],
             "bh_get_state_acc": [vp, C.POINTER(vp)],
+            "bh_copy_state_acc": [vp, vp],
+            "bh_euler_step": [vp, dbl],
+            "bh_multirate_step": [vp, dbl, i32],
+            "bh_potential": [vp, dbl, dbl, dbl, vp],
+            "bh_direct_potential": [vp, dbl, dbl, vp],
+            "bh_diagnostics": [vp, vp, vp, vp, vp, i64, C.POINTER(dbl)],
+            "bh_position_error": [vp, vp, vp, i64, C.POINTER(dbl)],
             "bh_eval_host": [vp, vp, vp, i64, dbl, dbl, dbl, vp],
             "bh_synchronize": [vp],
             "bh_get_cube": [vp, C.POINTER(dbl), C.POINTER(dbl)],
@@ -79,7 +88,9 @@ EXPORTS = ("bh_workspace_bytes", "bh_create", "bh_destroy", "bh_set_stream", "bh
            "bh_eval_host", "bh_synchronize", "bh_get_cube", "bh_get_keys", "bh_get_node_count",
            "bh_get_nodes", "bh_get_groups", "bh_get_bodies", "bh_get_counts", "bh_get_stats", "bh_get_launches",
            "bh_set_timing",
-           "bh_get_phase_ms", "bh_measure_fp64_peak", "bh_last_error", "bh_version")
+           "bh_get_phase_ms", "bh_measure_fp64_peak", "bh_last_error", "bh_version",
+           "bh_euler_step", "bh_multirate_step", "bh_potential", "bh_direct_potential", "bh_diagnostics",
+           "bh_position_error", "bh_gravity_dt", "bh_copy_state_acc")
 
 
 def _check(ctx, status: int):
@@ -155,6 +166,45 @@ def bh_bind_state(ctx, pos, vel, mass, theta: float, eps: float, G: float):
 
 def bh_kdk_step(ctx, dt: float):
     _check(ctx, lib().bh_kdk_step(ctx, dt))
+
+
+def bh_copy_state_acc(ctx, acc: torch.Tensor):
+    _check(ctx, lib().bh_copy_state_acc(ctx, _dev(acc, torch.float64, "acc")))
+
+
+def bh_euler_step(ctx, dt: float):
+    _check(ctx, lib().bh_euler_step(ctx, dt))
+
+
+def bh_multirate_step(ctx, dt_c: float, n_sub: int):
+    _check(ctx, lib().bh_multirate_step(ctx, dt_c, n_sub))
+
+
+def bh_potential(ctx, theta: float, eps: float, G: float, phi: torch.Tensor):
+    _check(ctx, lib().bh_potential(ctx, theta, eps, G, _dev(phi, torch.float64, "phi")))
+
+
+def bh_direct_potential(ctx, eps: float, G: float, phi: torch.Tensor):
+    _check(ctx, lib().bh_direct_potential(ctx, eps, G, _dev(phi, torch.float64, "phi")))
+
+
+def bh_diagnostics(ctx, pos, vel, mass, phi=None):
+    out = (C.c_double * 8)()
+    _check(ctx, lib().bh_diagnostics(ctx, _dev(pos, torch.float64, "pos"), _dev(vel, torch.float64, "vel"),
+                                     _dev(mass, torch.float64, "mass"), _dev(phi, torch.float64, "phi"),
+                                     pos.shape[0], out))
+    return {"ekin": out[0], "epot": out[1], "P": [out[2], out[3], out[4]], "L": [out[5], out[6], out[7]]}
+
+
+def bh_position_error(ctx, pos, ref) -> float:
+    v = C.c_double()
+    _check(ctx, lib().bh_position_error(ctx, _dev(pos, torch.float64, "pos"), _dev(ref, torch.float64, "ref"),
+                                        pos.shape[0], C.byref(v)))
+    return v.value
+
+
+def bh_gravity_dt(G: float, rho: float) -> float:
+    return float(lib().bh_gravity_dt(G, rho))
 
 
 def bh_eval_host(ctx, pos_host, mass_host, theta, eps, G, acc_host):
@@ -278,6 +328,16 @@ class Context:
         else:
             out = torch.empty((targets.numel(), 3), dtype=torch.float64, device=self.device) if out is None else out
             bh_direct_targets(self.ctx, targets, eps, G, out)
+        return out
+
+    def potential(self, theta, eps, G, out=None):
+        out = torch.empty(self.n, dtype=torch.float64, device=self.device) if out is None else out
+        bh_potential(self.ctx, theta, eps, G, out)
+        return out
+
+    def direct_potential(self, eps, G, out=None):
+        out = torch.empty(self.n, dtype=torch.float64, device=self.device) if out is None else out
+        bh_direct_potential(self.ctx, eps, G, out)
         return out
 
     def tree(self):

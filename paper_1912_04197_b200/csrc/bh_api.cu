@@ -1,4 +1,5 @@
 // bh_api.cu — the C ABI declared in include/bh.h: context, workspace carving, call sequencing.
+#include <cmath>
 #include <cstdio>
 #include <cstring>
 #include <new>
@@ -22,11 +23,13 @@ struct bh_ctx {
     int64_t bound_n = 0;
     double theta = 0, eps = 0, G = 0;
     bool bound = false, have_acc = false;
+    bool acc_filled = false;   // ws.acc holds the accelerations of the last stepper evaluation
     // timing
     bool timing = false;
     cudaEvent_t ev[BH_NUM_PHASES][2]{};
     bool ev_set[BH_NUM_PHASES]{};
     DevState *host_state = nullptr;   // pinned mirror for synchronising getters
+    double *host_diag = nullptr;      // pinned, 16 doubles, after host_state
     uint64_t launches = 0;            // kernels launched so far (bench.py's gpu_launches)
     char err[256] = "";
 };
@@ -129,7 +132,7 @@ bh_status do_build(bh_ctx *c, const double *pos, const double *mass, int64_t n)
     return BH_OK;
 }
 
-bh_status do_accel(bh_ctx *c, double theta, double eps, double G, double *acc)
+bh_status do_accel(bh_ctx *c, double theta, double eps, double G, double *acc, bool potential = false)
 {
     const Workspace &w = c->ws;
     // reset the group queue and the counters of this evaluation
@@ -137,7 +140,7 @@ bh_status do_accel(bh_ctx *c, double theta, double eps, double G, double *acc)
     cudaMemsetAsync(&w.st->stats[0], 0, 4 * sizeof(unsigned long long), c->stream);
     {
         Phase p(c, 6);
-        launch_walk(w, c->n, theta, eps, G, acc, c->stream);
+        launch_walk(w, c->n, theta, eps, G, acc, potential, c->stream);
     }
     bh_status st = cuda_check(c, cudaGetLastError(), "bh_accel launch");
     if (st == BH_OK) {
@@ -197,6 +200,9 @@ Workspace carve(char *base, int64_t max_n, int leaf_cap)
     w.stage_doubles = 3 * n;
     w.stage_mass = cv.take<double>(n);
     w.peak_sink = cv.take<double>(32);
+    w.diag_part = cv.take<double>((size_t)kDiagBlocks * 16);
+    w.diag_out = cv.take<double>(16);
+    w.diag_ticket = base ? &w.st->ticket_diag : nullptr;
     w.total_bytes = cv.off;
     return w;
 }
@@ -238,7 +244,9 @@ bh_status bh_create(bh_ctx **out, int64_t max_n, int leaf_cap, int group_size, v
     c->leaf_cap = leaf_cap;
     c->stream = (cudaStream_t)cuda_stream;
     c->ws = w;
-    cudaError_t e = cudaMallocHost((void **)&c->host_state, sizeof(DevState));
+    const size_t hs = (sizeof(DevState) + 63) & ~(size_t)63;
+    cudaError_t e = cudaMallocHost((void **)&c->host_state, hs + 16 * sizeof(double));
+    if (e == cudaSuccess) c->host_diag = reinterpret_cast<double *>(reinterpret_cast<char *>(c->host_state) + hs);
     if (e == cudaSuccess) e = cudaMemsetAsync(w.st, 0, sizeof(DevState), c->stream);
     for (int p = 0; p < BH_NUM_PHASES && e == cudaSuccess; ++p) {
         e = cudaEventCreate(&c->ev[p][0]);
@@ -300,7 +308,7 @@ bh_status bh_direct(bh_ctx *c, double eps, double G, double *acc_dev)
     if (!(eps >= 0.0)) return fail(c, BH_ERR_INVALID_ARG, "bh_direct: eps negative");
     {
         Phase p(c, 7);
-        c->launches += launch_direct(c->ws, c->n, nullptr, c->n, eps, G, acc_dev, c->stream);
+        c->launches += launch_direct(c->ws, c->n, nullptr, c->n, eps, G, acc_dev, false, c->stream);
     }
     return cuda_check(c, cudaGetLastError(), "bh_direct launch");
 }
@@ -313,7 +321,7 @@ bh_status bh_direct_targets(bh_ctx *c, const int32_t *tgt_dev, int64_t nt, doubl
     if (nt < 1 || !(eps >= 0.0)) return fail(c, BH_ERR_INVALID_ARG, "bh_direct_targets: nt < 1 or eps negative");
     {
         Phase p(c, 7);
-        c->launches += launch_direct(c->ws, c->n, tgt_dev, nt, eps, G, acc_dev, c->stream);
+        c->launches += launch_direct(c->ws, c->n, tgt_dev, nt, eps, G, acc_dev, false, c->stream);
     }
     return cuda_check(c, cudaGetLastError(), "bh_direct_targets launch");
 }
@@ -334,6 +342,7 @@ bh_status bh_bind_state(bh_ctx *c, double *pos_dev, double *vel_dev, const doubl
     c->G = G;
     c->bound = true;
     c->have_acc = false;
+    c->acc_filled = false;
     return BH_OK;
 }
 
@@ -356,9 +365,97 @@ bh_status bh_kdk_step(bh_ctx *c, double dt)
     if ((st = do_build(c, c->pos, c->mass, c->bound_n)) != BH_OK) return st;
     if ((st = do_accel(c, c->theta, c->eps, c->G, c->ws.acc)) != BH_OK) return st;
     launch_kick(c->vel, c->ws.acc, c->bound_n, dt * 0.5, c->stream);
+    c->acc_filled = true;
     c->launches += 2;   // kick+drift, kick
     return cuda_check(c, cudaGetLastError(), "bh_kdk_step launch");
 }
+
+/* ---- rows "next": paper's stepping variants and conservation diagnostics ---- */
+static bh_status euler_like(bh_ctx *c, double dt, int n_sub, const char *who)
+{
+    if (!c) return BH_ERR_INVALID_ARG;
+    if (!c->bound) return fail(c, BH_ERR_STATE, "stepper called before bh_bind_state");
+    if (n_sub < 1) return fail(c, BH_ERR_INVALID_ARG, "n_sub < 1");
+    bh_status st;
+    if ((st = do_build(c, c->pos, c->mass, c->bound_n)) != BH_OK) return st;
+    if ((st = do_accel(c, c->theta, c->eps, c->G, c->ws.acc)) != BH_OK) return st;
+    c->have_acc = false;   // acc is a(x_k), not a(x_k+1): a later bh_kdk_step re-evaluates
+    c->acc_filled = true;
+    if (c->timing) cudaEventRecord(c->ev[8][0], c->stream);
+    launch_euler_sub(c->pos, c->vel, c->ws.acc, c->bound_n, dt, n_sub, c->stream);
+    if (c->timing) {
+        cudaEventRecord(c->ev[8][1], c->stream);
+        c->ev_set[8] = true;
+    }
+    c->launches += 1;
+    return cuda_check(c, cudaGetLastError(), who);
+}
+
+bh_status bh_euler_step(bh_ctx *c, double dt) { return euler_like(c, dt, 1, "bh_euler_step launch"); }
+
+bh_status bh_multirate_step(bh_ctx *c, double dt_c, int n_sub)
+{
+    return euler_like(c, dt_c, n_sub, "bh_multirate_step launch");
+}
+
+bh_status bh_potential(bh_ctx *c, double theta, double eps, double G, double *phi_dev)
+{
+    if (!c) return BH_ERR_INVALID_ARG;
+    if (!c->built) return fail(c, BH_ERR_STATE, "bh_potential before bh_build");
+    if (!phi_dev) return fail(c, BH_ERR_INVALID_ARG, "bh_potential: null pointer");
+    if (!(theta >= 0.0) || !(eps >= 0.0)) return fail(c, BH_ERR_INVALID_ARG, "bh_potential: theta or eps negative");
+    return do_accel(c, theta, eps, G, phi_dev, true);
+}
+
+bh_status bh_direct_potential(bh_ctx *c, double eps, double G, double *phi_dev)
+{
+    if (!c) return BH_ERR_INVALID_ARG;
+    if (!c->built) return fail(c, BH_ERR_STATE, "bh_direct_potential before bh_build");
+    if (!phi_dev) return fail(c, BH_ERR_INVALID_ARG, "bh_direct_potential: null pointer");
+    if (!(eps >= 0.0)) return fail(c, BH_ERR_INVALID_ARG, "bh_direct_potential: eps negative");
+    {
+        Phase p(c, 7);
+        c->launches += launch_direct(c->ws, c->n, nullptr, c->n, eps, G, phi_dev, true, c->stream);
+    }
+    return cuda_check(c, cudaGetLastError(), "bh_direct_potential launch");
+}
+
+static bh_status read_diag(bh_ctx *c, int first, int count, double *out_host)
+{
+    cudaError_t e = cudaMemcpyAsync(c->host_diag, c->ws.diag_out + first, count * sizeof(double),
+                                    cudaMemcpyDeviceToHost, c->stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
+    if (e != cudaSuccess) return cuda_check(c, e, "diagnostics readback");
+    for (int k = 0; k < count; ++k) out_host[k] = c->host_diag[k];
+    return BH_OK;
+}
+
+bh_status bh_diagnostics(bh_ctx *c, const double *pos_dev, const double *vel_dev, const double *mass_dev,
+                         const double *phi_dev, int64_t n, double out_host[8])
+{
+    if (!c) return BH_ERR_INVALID_ARG;
+    if (!pos_dev || !vel_dev || !mass_dev || !out_host) return fail(c, BH_ERR_INVALID_ARG, "bh_diagnostics: null pointer");
+    if (n < 1) return fail(c, BH_ERR_INVALID_ARG, "bh_diagnostics: n < 1");
+    launch_diagnostics(c->ws, pos_dev, vel_dev, mass_dev, phi_dev, n, c->stream);
+    c->launches += 1;
+    bh_status st = cuda_check(c, cudaGetLastError(), "bh_diagnostics launch");
+    if (st != BH_OK) return st;
+    return read_diag(c, 0, 8, out_host);
+}
+
+bh_status bh_position_error(bh_ctx *c, const double *pos_dev, const double *ref_dev, int64_t n, double *err_host)
+{
+    if (!c) return BH_ERR_INVALID_ARG;
+    if (!pos_dev || !ref_dev || !err_host) return fail(c, BH_ERR_INVALID_ARG, "bh_position_error: null pointer");
+    if (n < 1) return fail(c, BH_ERR_INVALID_ARG, "bh_position_error: n < 1");
+    launch_position_error(c->ws, pos_dev, ref_dev, n, c->stream);
+    c->launches += 1;
+    bh_status st = cuda_check(c, cudaGetLastError(), "bh_position_error launch");
+    if (st != BH_OK) return st;
+    return read_diag(c, 8, 1, err_host);
+}
+
+double bh_gravity_dt(double G, double rho) { return 1.0 / (2.0 * sqrt(G * rho)); }
 
 bh_status bh_get_state_acc(bh_ctx *c, const double **acc_dev)
 {
@@ -366,6 +463,14 @@ bh_status bh_get_state_acc(bh_ctx *c, const double **acc_dev)
     if (!c->bound || !c->have_acc) return fail(c, BH_ERR_STATE, "no accelerations yet");
     *acc_dev = c->ws.acc;
     return BH_OK;
+}
+
+bh_status bh_copy_state_acc(bh_ctx *c, double *acc_dev)
+{
+    if (!c || !acc_dev) return BH_ERR_INVALID_ARG;
+    if (!c->bound || !c->acc_filled) return fail(c, BH_ERR_STATE, "no stepper evaluation yet");
+    return cuda_check(c, cudaMemcpyAsync(acc_dev, c->ws.acc, (size_t)c->bound_n * 24, cudaMemcpyDeviceToDevice,
+                                         c->stream), "bh_copy_state_acc");
 }
 
 bh_status bh_eval_host(bh_ctx *c, const double *pos_host, const double *mass_host, int64_t n, double theta,
@@ -384,6 +489,7 @@ bh_status bh_eval_host(bh_ctx *c, const double *pos_host, const double *mass_hos
     if ((st = do_build(c, w.stage_pos, w.stage_mass, n)) != BH_OK) return st;
     if ((st = do_accel(c, theta, eps, G, w.acc)) != BH_OK) return st;
     c->have_acc = false;   // the internal acc buffer no longer belongs to the bound state
+    c->acc_filled = false;
     e = cudaMemcpyAsync(acc_host, w.acc, 3 * n * sizeof(double), cudaMemcpyDeviceToHost, c->stream);
     if (e != cudaSuccess) return cuda_check(c, e, "bh_eval_host D2H");
     return fetch_state(c);

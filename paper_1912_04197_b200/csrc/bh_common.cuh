@@ -19,6 +19,7 @@ constexpr int kSortThreads = 256;
 constexpr int kSortItems = 16;            // keys per thread
 constexpr int kSortTile = kSortThreads * kSortItems;   // 4096 keys per tile
 constexpr int kTreeTile = 1024;           // bodies per block in the tree kernels
+constexpr int kDiagBlocks = 148 * 4;       // diagnostics: most blocks (fixed, so the reduction order is fixed)
 constexpr int kStackSlab = 22 * 256;      // walk: spill entries (8 bytes each) per producer warp: <= 32 x 7 ranges per level; overflow sets kStatStack
 
 enum StatusBits : int { kStatNonFinite = 1, kStatCapacity = 2, kStatStack = 4 };
@@ -36,6 +37,7 @@ struct DevState {
     unsigned lvl_start[kLevels + 1];   // first node id of each level (lvl_start[kLevels] = M)
     unsigned ticket_bbox;  // last-block election
     unsigned walk_queue;   // dynamic group counter of the walk
+    unsigned ticket_diag;  // last-block election of the diagnostics reduction (resets itself)
     unsigned long long stats[4];       // n_mono, n_direct, interactions, nodes tested
 };
 
@@ -73,6 +75,9 @@ struct Workspace {
     int64_t stage_doubles;        // capacity of stage_pos in doubles
     double *stage_mass;           // [n]
     double *peak_sink;            // fp64 microbenchmark sink
+    double *diag_part;            // [kDiagBlocks][8][2] double-double partial sums of the diagnostics
+    double *diag_out;             // [8] conserved quantities, [8] bits of the Eq. (7) maximum
+    unsigned *diag_ticket;        // = &st->ticket_diag
     int64_t node_cap;
     int64_t sort_tiles;
     int64_t tree_tiles;
@@ -97,13 +102,20 @@ void launch_sort(const Workspace &w, int64_t n, cudaStream_t s);   // result in 
 void launch_gather(const Workspace &w, const double *pos, const double *mass, int64_t n, cudaStream_t s);
 void launch_tree(const Workspace &w, int64_t n, int leaf_cap, cudaStream_t s);
 void launch_monopoles(const Workspace &w, int64_t n, cudaStream_t s);
-void launch_walk(const Workspace &w, int64_t n, double theta, double eps, double G, double *acc, cudaStream_t s);
+// potential = false: acc [n][3] accelerations; true: acc [n] potential (NEXT-1)
+void launch_walk(const Workspace &w, int64_t n, double theta, double eps, double G, double *acc, bool potential,
+                 cudaStream_t s);
 int launch_direct(const Workspace &w, int64_t n, const int32_t *tgt, int64_t nt, double eps, double G,
-                  double *acc, cudaStream_t s);   // returns the number of kernels launched
+                  double *acc, bool potential, cudaStream_t s);   // returns the number of kernels launched
 void launch_kick_drift(double *pos, double *vel, const double *acc, int64_t n, double dt, cudaStream_t s);
 void launch_kick(double *vel, const double *acc, int64_t n, double h, cudaStream_t s);
 void launch_unpack_mask(const Workspace &w, unsigned char *mask_out, int64_t cap, cudaStream_t s);
 double run_fp64_peak(const Workspace &w, cudaStream_t s);
+// rows "next" (bh_diag.cu): results land in w.diag_out
+void launch_diagnostics(const Workspace &w, const double *pos, const double *vel, const double *mass,
+                        const double *phi, int64_t n, cudaStream_t s);
+void launch_position_error(const Workspace &w, const double *pos, const double *ref, int64_t n, cudaStream_t s);
+void launch_euler_sub(double *pos, double *vel, const double *acc, int64_t n, double dt, int n_sub, cudaStream_t s);
 
 // ---- small device helpers ----
 __device__ __forceinline__ unsigned lane_id() { return threadIdx.x & 31u; }

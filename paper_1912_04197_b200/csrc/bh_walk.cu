@@ -77,6 +77,31 @@ __device__ __forceinline__ void interact(double px, double py, double pz, double
     az = fma(f, dz, az);
 }
 
+// m / r from the same seed (NEXT-1, potential of the softened force, R24): (1-e)^(-1/2) = 1 + e (1/2 + 3/8 e) + O(e^3)
+template <bool GUARD>
+__device__ __forceinline__ void interact_pot(double px, double py, double pz, double eps2, const double4 s, double &phi)
+{
+    const double dx = s.x - px, dy = s.y - py, dz = s.z - pz;
+    const double r2 = fma(dx, dx, fma(dy, dy, fma(dz, dz, eps2)));
+    double y;
+    asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(r2));
+    if (GUARD) y = (r2 > 0.0) ? y : 0.0;
+    const double u = y * y;
+    const double w = s.w * y;
+    const double e = fma(-r2, u, 1.0);
+    const double p = fma(0.375, e, 0.5);
+    const double h = fma(p, e, 1.0);
+    phi = fma(w, h, phi);
+}
+
+template <bool GUARD, bool POT>
+__device__ __forceinline__ void interact_any(double px, double py, double pz, double eps2, const double4 s,
+                                             double &ax, double &ay, double &az)
+{
+    if constexpr (POT) interact_pot<GUARD>(px, py, pz, eps2, s, ax);
+    else interact<GUARD>(px, py, pz, eps2, s, ax, ay, az);
+}
+
 struct PairCtrl {                            // all words are written by one role and read by the other
     unsigned tail_pub;                       // producer: ring entries below this are complete
     unsigned head_pub;                       // consumer: ring entries below this are free again
@@ -216,6 +241,9 @@ __device__ __forceinline__ double box_delta(double lo, double hi, double c)
 // every lane one range; the lane then walks its (at most eight, memory-contiguous) siblings one per
 // trip, so the warp-wide bookkeeping of a trip (two ballots, one stack entry per opened node) is
 // spread over up to 32 nodes and the records of the next trip are already in flight.
+// POT (potential walk): the group's own bodies enter the ring with zero mass; the consumer adds the
+// pairs inside the group itself, where a body can be told from its coincident neighbours (R24).
+template <bool POT>
 __device__ void produce(PairSmem &ps, DevState *st, const unsigned *__restrict__ gstart,
                         const double4 *__restrict__ sbody, const double *__restrict__ gbox,
                         const uint4 *__restrict__ winfo, const double4 *__restrict__ mono, double theta2,
@@ -353,9 +381,14 @@ __device__ void produce(PairSmem &ps, DevState *st, const unsigned *__restrict__
                             P.reserve(n);
                             if (lane < n) {
                                 char *dst = reinterpret_cast<char *>(&ps.ring[(P.tail + lane) & (kRing - 1)]);
-                                const char *from = reinterpret_cast<const char *>(sbody + (ps.leaf_src[k] + base + lane));
-                                cp_async16(dst, from);
-                                cp_async16(dst + 16, from + 16);
+                                const unsigned src = ps.leaf_src[k] + base + lane;
+                                const char *from = reinterpret_cast<const char *>(sbody + src);
+                                if (POT && src >= gb && src < ge) {
+                                    ps.ring[(P.tail + lane) & (kRing - 1)] = make_double4(0.0, 0.0, 0.0, 0.0);
+                                } else {
+                                    cp_async16(dst, from);
+                                    cp_async16(dst + 16, from + 16);
+                                }
                             }
                             P.tail += n;
                         }
@@ -417,7 +450,7 @@ struct Bodies {
 };
 
 // evaluate n8 (a multiple of 8) sources starting at ring position head (a multiple of 8)
-template <bool GUARD, int NS>
+template <bool GUARD, int NS, bool POT>
 __device__ __forceinline__ void eval_chunks(const double4 *ring, unsigned head, unsigned n8, unsigned quarter,
                                             double eps2, Bodies<NS> &B)
 {
@@ -426,14 +459,14 @@ __device__ __forceinline__ void eval_chunks(const double4 *ring, unsigned head, 
         const double4 *p = ring + ((head + i) & (kRing - 1)) + quarter;
         const double4 s0 = p[0], s1 = p[4];
 #pragma unroll
-        for (int k = 0; k < NS; ++k) interact<GUARD>(B.x[k], B.y[k], B.z[k], eps2, s0, B.ax[k], B.ay[k], B.az[k]);
+        for (int k = 0; k < NS; ++k) interact_any<GUARD, POT>(B.x[k], B.y[k], B.z[k], eps2, s0, B.ax[k], B.ay[k], B.az[k]);
 #pragma unroll
-        for (int k = 0; k < NS; ++k) interact<GUARD>(B.x[k], B.y[k], B.z[k], eps2, s1, B.ax[k], B.ay[k], B.az[k]);
+        for (int k = 0; k < NS; ++k) interact_any<GUARD, POT>(B.x[k], B.y[k], B.z[k], eps2, s1, B.ax[k], B.ay[k], B.az[k]);
     }
 }
 
 // one group: evaluate its sources as the producer publishes them, then write the accelerations
-template <bool GUARD, int NS>
+template <bool GUARD, int NS, bool POT>
 __device__ __forceinline__ long long consume_group(PairSmem &ps, unsigned k, unsigned head, long long gb, long long ge,
                                               const double4 *__restrict__ sbody, const unsigned *__restrict__ perm,
                                               double eps2, double G, double *__restrict__ acc)
@@ -470,7 +503,7 @@ __device__ __forceinline__ long long consume_group(PairSmem &ps, unsigned k, uns
             continue;
         }
         const unsigned n8 = avail > 0 ? ((unsigned)avail & ~7u) : 0u;
-        eval_chunks<GUARD, NS>(ps.ring, head, n8, quarter, eps2, B);
+        eval_chunks<GUARD, NS, POT>(ps.ring, head, n8, quarter, eps2, B);
         head += n8;
         if (fin) {
             const unsigned rest = (unsigned)(avail > 0 ? avail : 0) & 7u;
@@ -479,15 +512,27 @@ __device__ __forceinline__ long long consume_group(PairSmem &ps, unsigned k, uns
                 const double4 s0 = quarter < rest ? p[0] : zero4;
                 const double4 s1 = quarter + 4 < rest ? p[4] : zero4;
 #pragma unroll
-                for (int s = 0; s < NS; ++s) interact<GUARD>(B.x[s], B.y[s], B.z[s], eps2, s0, B.ax[s], B.ay[s], B.az[s]);
+                for (int s = 0; s < NS; ++s) interact_any<GUARD, POT>(B.x[s], B.y[s], B.z[s], eps2, s0, B.ax[s], B.ay[s], B.az[s]);
 #pragma unroll
-                for (int s = 0; s < NS; ++s) interact<GUARD>(B.x[s], B.y[s], B.z[s], eps2, s1, B.ax[s], B.ay[s], B.az[s]);
+                for (int s = 0; s < NS; ++s) interact_any<GUARD, POT>(B.x[s], B.y[s], B.z[s], eps2, s1, B.ax[s], B.ay[s], B.az[s]);
                 head += rest;
             }
             warp_release(&ps.ctrl.head_pub, head, lane);
             break;
         }
         warp_release(&ps.ctrl.head_pub, head, lane);
+    }
+    if constexpr (POT) {
+        // pairs inside the group: quarter q takes the group's bodies gb + q, gb + q + 4, ...; a body skips itself
+        for (long long k = gb + quarter; k < ge; k += 4) {
+            const double4 sk = sbody[k];
+#pragma unroll
+            for (int s = 0; s < NS; ++s) {
+                double4 src = sk;
+                if (k == gb + r + 8 * s) src.w = 0.0;
+                interact_pot<true>(B.x[s], B.y[s], B.z[s], eps2, src, B.ax[s]);
+            }
+        }
     }
     // add the four quarter-warp partial sums; lane 8 q + r then writes body r + 8 q
     double ox = 0.0, oy = 0.0, oz = 0.0;
@@ -505,14 +550,18 @@ __device__ __forceinline__ long long consume_group(PairSmem &ps, unsigned k, uns
     const long long j = gb + lane;
     if (j < ge) {
         const unsigned i = perm[j];
-        acc[3ll * i + 0] = G * ox;
-        acc[3ll * i + 1] = G * oy;
-        acc[3ll * i + 2] = G * oz;
+        if constexpr (POT) {
+            acc[i] = -G * ox;                       // phi, one value per body
+        } else {
+            acc[3ll * i + 0] = G * ox;
+            acc[3ll * i + 1] = G * oy;
+            acc[3ll * i + 2] = G * oz;
+        }
     }
     return g_prof_wait;
 }
 
-template <bool GUARD>
+template <bool GUARD, bool POT>
 __device__ void consume(PairSmem &ps, DevState *prof_st, const unsigned *__restrict__ gstart, const double4 *__restrict__ sbody,
                         const unsigned *__restrict__ perm, double eps2, double G, double *__restrict__ acc)
 {
@@ -535,10 +584,10 @@ __device__ void consume(PairSmem &ps, DevState *prof_st, const unsigned *__restr
         const long long gb = gstart[g];
         const long long ge = gstart[g + 1];
         const int slots = (int)((ge - gb + 7) >> 3);
-        if (slots >= 4) waited += consume_group<GUARD, 4>(ps, k, head, gb, ge, sbody, perm, eps2, G, acc);
-        else if (slots == 3) waited += consume_group<GUARD, 3>(ps, k, head, gb, ge, sbody, perm, eps2, G, acc);
-        else if (slots == 2) waited += consume_group<GUARD, 2>(ps, k, head, gb, ge, sbody, perm, eps2, G, acc);
-        else waited += consume_group<GUARD, 1>(ps, k, head, gb, ge, sbody, perm, eps2, G, acc);
+        if (slots >= 4) waited += consume_group<GUARD, 4, POT>(ps, k, head, gb, ge, sbody, perm, eps2, G, acc);
+        else if (slots == 3) waited += consume_group<GUARD, 3, POT>(ps, k, head, gb, ge, sbody, perm, eps2, G, acc);
+        else if (slots == 2) waited += consume_group<GUARD, 2, POT>(ps, k, head, gb, ge, sbody, perm, eps2, G, acc);
+        else waited += consume_group<GUARD, 1, POT>(ps, k, head, gb, ge, sbody, perm, eps2, G, acc);
         warp_release(&ps.ctrl.consumed, k + 1, lane);
     }
 #ifdef BH_WALK_PROF
@@ -551,7 +600,7 @@ __device__ void consume(PairSmem &ps, DevState *prof_st, const unsigned *__restr
 #endif
 }
 
-template <bool GUARD>
+template <bool GUARD, bool POT>
 __global__ void __launch_bounds__(kWalkThreads, 1)
 walk_kernel(DevState *st, const unsigned *__restrict__ gstart, const double4 *__restrict__ sbody,
             const double *__restrict__ gbox, const unsigned *__restrict__ perm,
@@ -575,10 +624,10 @@ walk_kernel(DevState *st, const unsigned *__restrict__ gstart, const double4 *__
     else asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(BH_REG_CONS));
 #endif
     if (producer)
-        produce(ps, st, gstart, sbody, gbox, winfo, mono, theta2, cnt_mono, cnt_direct,
+        produce<POT>(ps, st, gstart, sbody, gbox, winfo, mono, theta2, cnt_mono, cnt_direct,
                 reinterpret_cast<uint2 *>(walk_stack) + (size_t)(blockIdx.x * kPairs + pair) * kStackSlab);
     else
-        consume<GUARD>(ps, st, gstart, sbody, perm, eps2, G, acc);
+        consume<GUARD, POT>(ps, st, gstart, sbody, perm, eps2, G, acc);
 }
 
 // ------------------------------------------------------------------------------------------ a8
@@ -589,7 +638,7 @@ walk_kernel(DevState *st, const unsigned *__restrict__ gstart, const double4 *__
 constexpr int kDirectThreads = 256;
 constexpr int kDirectTargets = 2 * kDirectThreads;
 
-template <bool GUARD>
+template <bool GUARD, bool POT>
 __global__ void __launch_bounds__(kDirectThreads)
 direct_kernel(long long n, const double4 *__restrict__ sbody, const unsigned *__restrict__ perm,
               const unsigned *__restrict__ iperm, const int32_t *__restrict__ tgt, long long nt, double eps2,
@@ -612,12 +661,29 @@ direct_kernel(long long n, const double4 *__restrict__ sbody, const unsigned *__
 #pragma unroll 4
         for (int q = 0; q < kDirectThreads; ++q) {
             const double4 sq = tile[q];
-            interact<GUARD>(p0.x, p0.y, p0.z, eps2, sq, ax0, ay0, az0);
-            interact<GUARD>(p1.x, p1.y, p1.z, eps2, sq, ax1, ay1, az1);
+            if constexpr (POT) {                 // a body skips itself: its own term m/eps is not zero
+                double4 s0 = sq, s1 = sq;
+                if (t0 + q == j0) s0.w = 0.0;
+                if (t0 + q == j1) s1.w = 0.0;
+                interact_pot<GUARD>(p0.x, p0.y, p0.z, eps2, s0, ax0);
+                interact_pot<GUARD>(p1.x, p1.y, p1.z, eps2, s1, ax1);
+            } else {
+                interact<GUARD>(p0.x, p0.y, p0.z, eps2, sq, ax0, ay0, az0);
+                interact<GUARD>(p1.x, p1.y, p1.z, eps2, sq, ax1, ay1, az1);
+            }
         }
         __syncthreads();
     }
-    if (gridDim.y == 1) {
+    if constexpr (POT) {                     // one value per body: phi = -G sum m / r
+        if (gridDim.y == 1) {
+            if (r0 < nt) acc[tgt ? r0 : (long long)perm[r0]] = -G * ax0;
+            if (r1 < nt) acc[tgt ? r1 : (long long)perm[r1]] = -G * ax1;
+        } else {
+            double *p = partial + (size_t)blockIdx.y * nt;
+            if (r0 < nt) p[r0] = ax0;
+            if (r1 < nt) p[r1] = ax1;
+        }
+    } else if (gridDim.y == 1) {
         if (r0 < nt) {
             const long long o = tgt ? r0 : (long long)perm[r0];
             acc[3 * o + 0] = G * ax0; acc[3 * o + 1] = G * ay0; acc[3 * o + 2] = G * az0;
@@ -633,16 +699,18 @@ direct_kernel(long long n, const double4 *__restrict__ sbody, const unsigned *__
     }
 }
 
-__global__ void direct_reduce_kernel(const double *__restrict__ partial, long long nt, int splits, double G,
-                                     const unsigned *__restrict__ perm, bool sampled, double *__restrict__ acc)
+// ncomp = 3 (accelerations, scale G) or 1 (potential, scale -G)
+__global__ void direct_reduce_kernel(const double *__restrict__ partial, long long nt, int splits, double scale,
+                                     int ncomp, const unsigned *__restrict__ perm, bool sampled,
+                                     double *__restrict__ acc)
 {
-    for (long long k = (long long)blockIdx.x * blockDim.x + threadIdx.x; k < 3 * nt;
+    for (long long k = (long long)blockIdx.x * blockDim.x + threadIdx.x; k < ncomp * nt;
          k += (long long)gridDim.x * blockDim.x) {
         double s = 0.0;
-        for (int q = 0; q < splits; ++q) s += partial[(size_t)q * nt * 3 + k];
-        const long long r = k / 3, c = k - 3 * r;
+        for (int q = 0; q < splits; ++q) s += partial[(size_t)q * nt * ncomp + k];
+        const long long r = k / ncomp, c = k - ncomp * r;
         const long long o = sampled ? r : (long long)perm[r];
-        acc[3 * o + c] = G * s;
+        acc[ncomp * o + c] = scale * s;
     }
 }
 
@@ -680,29 +748,36 @@ __global__ void __launch_bounds__(256) fp64_peak_kernel(double *sink, int iters,
 }
 
 // ------------------------------------------------------------------------------------------ launchers
-void launch_walk(const Workspace &w, int64_t n, double theta, double eps, double G, double *acc, cudaStream_t s)
+template <bool GUARD, bool POT>
+static void launch_walk_t(const Workspace &w, double theta, double eps2, double G, double *out, cudaStream_t s)
 {
     static bool configured = false;
     if (!configured) {
-        cudaFuncSetAttribute(walk_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(WalkSmem));
-        cudaFuncSetAttribute(walk_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(WalkSmem));
+        cudaFuncSetAttribute(walk_kernel<GUARD, POT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(WalkSmem));
         configured = true;
     }
-    (void)n;
     const int blocks = w.walk_warps / kPairs;   // one persistent block per SM
+    walk_kernel<GUARD, POT><<<blocks, kWalkThreads, sizeof(WalkSmem), s>>>(
+        w.st, w.gstart, w.sbody, w.gbox, w.idx[0], w.winfo, w.mono, theta * theta, eps2, G, out, w.cnt_mono,
+        w.cnt_direct, w.walk_stack);
+}
+
+void launch_walk(const Workspace &w, int64_t n, double theta, double eps, double G, double *acc, bool potential,
+                 cudaStream_t s)
+{
+    (void)n;
     const double eps2 = eps * eps;
-    if (eps2 > 0.0)
-        walk_kernel<false><<<blocks, kWalkThreads, sizeof(WalkSmem), s>>>(
-            w.st, w.gstart, w.sbody, w.gbox, w.idx[0], w.winfo, w.mono, theta * theta, eps2, G, acc, w.cnt_mono,
-            w.cnt_direct, w.walk_stack);
-    else
-        walk_kernel<true><<<blocks, kWalkThreads, sizeof(WalkSmem), s>>>(
-            w.st, w.gstart, w.sbody, w.gbox, w.idx[0], w.winfo, w.mono, theta * theta, eps2, G, acc, w.cnt_mono,
-            w.cnt_direct, w.walk_stack);
+    if (potential) {
+        if (eps2 > 0.0) launch_walk_t<false, true>(w, theta, eps2, G, acc, s);
+        else launch_walk_t<true, true>(w, theta, eps2, G, acc, s);
+    } else {
+        if (eps2 > 0.0) launch_walk_t<false, false>(w, theta, eps2, G, acc, s);
+        else launch_walk_t<true, false>(w, theta, eps2, G, acc, s);
+    }
 }
 
 int launch_direct(const Workspace &w, int64_t n, const int32_t *tgt, int64_t nt, double eps, double G,
-                  double *acc, cudaStream_t s)
+                  double *acc, bool potential, cudaStream_t s)
 {
     const int64_t rows = tgt ? nt : n;
     const int tblocks = (int)((rows + kDirectTargets - 1) / kDirectTargets);
@@ -717,14 +792,20 @@ int launch_direct(const Workspace &w, int64_t n, const int32_t *tgt, int64_t nt,
     splits = (tiles + tps - 1) / tps;
     const double eps2 = eps * eps;
     dim3 grid(tblocks, splits);
-    if (eps2 > 0.0)
-        direct_kernel<false><<<grid, kDirectThreads, 0, s>>>(n, w.sbody, w.idx[0], w.iperm, tgt, rows, eps2, G, acc,
-                                                            w.stage_pos, tps);
-    else
-        direct_kernel<true><<<grid, kDirectThreads, 0, s>>>(n, w.sbody, w.idx[0], w.iperm, tgt, rows, eps2, G, acc,
-                                                           w.stage_pos, tps);
+#define BH_DIRECT(GUARD, POT)                                                                                      \
+    direct_kernel<GUARD, POT><<<grid, kDirectThreads, 0, s>>>(n, w.sbody, w.idx[0], w.iperm, tgt, rows, eps2, G,   \
+                                                              acc, w.stage_pos, tps)
+    if (potential) {
+        if (eps2 > 0.0) BH_DIRECT(false, true);
+        else BH_DIRECT(true, true);
+    } else {
+        if (eps2 > 0.0) BH_DIRECT(false, false);
+        else BH_DIRECT(true, false);
+    }
+#undef BH_DIRECT
     if (splits > 1)
-        direct_reduce_kernel<<<148 * 2, 256, 0, s>>>(w.stage_pos, rows, splits, G, w.idx[0], tgt != nullptr, acc);
+        direct_reduce_kernel<<<148 * 2, 256, 0, s>>>(w.stage_pos, rows, splits, potential ? -G : G,
+                                                     potential ? 1 : 3, w.idx[0], tgt != nullptr, acc);
     return splits > 1 ? 2 : 1;
 }
 

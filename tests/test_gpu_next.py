@@ -1,0 +1,191 @@
+"""GPU parity for the rows "next" of SURVEY.md 8(f) (NEXT-1, NEXT-2): tree / direct potential, conserved
+quantities, Eq. (7) position error, semi-implicit Euler and two-rate stepping, against the CPU oracle
+(O12-O16 of oracle/bh_oracle.c) on the same seeded inputs.
+
+Bit-exact: Eq. (7) maximum (canonical arithmetic), the updates of the steppers given the same
+accelerations, the two-rate step against n_sub separate updates.  Floating point: potential within
+1e-11 relative per body (the bound north_star sets for accelerations); conserved quantities within
+1e-15 of the sum of |terms| (they cancel, so a relative bound on the result would be meaningless).
+"""
+import numpy as np
+import pytest
+import torch
+
+from oracle import bh_oracle as orc
+from paper_1912_04197_b200 import binding as bh
+from paper_1912_04197_b200 import workloads as wl
+
+pytestmark = pytest.mark.gpu
+TOL = 1e-11
+
+
+def dev(a, dtype=torch.float64):
+    return torch.as_tensor(np.ascontiguousarray(a), dtype=dtype).cuda()
+
+
+@pytest.mark.parametrize("name,n,C", [("c1", 1024, 8), ("c2", 16384, 16), ("c4", 30000, 16), ("c3", 777, 1),
+                                       ("c5", 20000, 32), ("c3", 5, 16)])
+def test_tree_potential(name, n, C):
+    w = wl.make(name, n)
+    t = orc.build(w.pos, w.mass, C)
+    ctx = bh.Context(n, C)
+    ctx.build(dev(w.pos), dev(w.mass))
+    for theta in (w.theta, 0.0) if n <= 20000 else (w.theta,):
+        ref = orc.potential(t, theta, w.eps, w.G)
+        phi = ctx.potential(theta, w.eps, w.G).cpu().numpy()
+        assert np.abs(phi - ref).max() <= TOL * np.abs(ref).min(), (theta, np.abs((phi - ref) / ref).max())
+        # the lists are those of the acceleration walk
+        _, nm, nd, _ = orc.accel(t, theta, w.eps, w.G, 0, 1)
+        gm, gd = ctx.counts()
+        assert gm[0].item() == nm[0] and gd[0].item() == nd[0]
+    ctx.close()
+
+
+@pytest.mark.parametrize("name,n,C", [("c1", 1024, 8), ("c2", 16384, 16), ("c4", 3001, 16)])
+def test_direct_potential(name, n, C):
+    w = wl.make(name, n)
+    ref = orc.direct_potential(w.pos, w.mass, w.eps, w.G)
+    ctx = bh.Context(n, C)
+    ctx.build(dev(w.pos), dev(w.mass))
+    phi = ctx.direct_potential(w.eps, w.G).cpu().numpy()
+    assert np.abs((phi - ref) / ref).max() <= TOL
+    ctx.close()
+
+
+def test_potential_coincident_bodies_eps0():
+    # R13/R24: a pair at zero softened distance adds nothing; a lone body has potential 0
+    pos = np.array([[0.0, 0, 0], [0.0, 0, 0], [2.0, 0, 0]])
+    mass = np.array([1.0, 3.0, 5.0])
+    ctx = bh.Context(3, 1)
+    ctx.build(dev(pos), dev(mass))
+    for phi in (ctx.potential(0.5, 0.0, 1.0).cpu().numpy(), ctx.direct_potential(0.0, 1.0).cpu().numpy()):
+        assert np.allclose(phi, np.array([-2.5, -2.5, -2.0]), rtol=1e-14, atol=0.0)
+    ctx.close()
+    ctx = bh.Context(1, 4)
+    ctx.build(dev(np.array([[1.0, 2.0, 3.0]])), dev(np.array([7.0])))
+    assert ctx.potential(0.5, 0.0, 1.0).item() == 0.0 and ctx.direct_potential(0.0, 1.0).item() == 0.0
+    ctx.close()
+
+
+def _sum_abs_terms(pos, vel, mass, phi):
+    m = mass[:, None]
+    lx = np.abs(pos[:, [1, 2, 0]] * vel[:, [2, 0, 1]]) + np.abs(pos[:, [2, 0, 1]] * vel[:, [1, 2, 0]])
+    return dict(ekin=(0.5 * mass * (vel ** 2).sum(1)).sum(), epot=np.abs(0.5 * mass * phi).sum(),
+                P=np.abs(m * vel).sum(0), L=(m * lx).sum(0))
+
+
+@pytest.mark.parametrize("name,n", [("c4", 100000), ("c5", 65537), ("c1", 1024), ("c4", 1)])
+def test_diagnostics(name, n):
+    w = wl.make(name, n)
+    rng = np.random.default_rng(7)
+    if w.vel is None:
+        w.vel = rng.standard_normal((n, 3))
+    phi = -rng.random(n) - 0.1
+    ctx = bh.Context(n, 16)
+    ref = orc.diagnostics(w.pos, w.vel, w.mass, phi)
+    scale = _sum_abs_terms(w.pos, w.vel, w.mass, phi)
+    d1 = bh.bh_diagnostics(ctx.ctx, dev(w.pos), dev(w.vel), dev(w.mass), dev(phi))
+    d2 = bh.bh_diagnostics(ctx.ctx, dev(w.pos), dev(w.vel), dev(w.mass), dev(phi))
+    assert d1 == d2                                    # fixed reduction order: reproducible bit for bit
+    for k in ("ekin", "epot"):
+        assert abs(d1[k] - ref[k]) <= 1e-15 * scale[k] + 1e-300
+    for k in ("P", "L"):
+        assert (np.abs(np.array(d1[k]) - ref[k]) <= 1e-15 * scale[k] + 1e-300).all()
+    d0 = bh.bh_diagnostics(ctx.ctx, dev(w.pos), dev(w.vel), dev(w.mass), None)
+    assert d0["epot"] == 0.0 and d0["ekin"] == d1["ekin"]
+    ctx.close()
+
+
+def test_diagnostics_exact_cancellation():
+    # momentum of +-v pairs cancels to ~2^-100 of the sum of |terms| (double-double accumulation), where a
+    # plain fp64 sum of terms spanning 16 decades would keep nothing
+    rng = np.random.default_rng(11)
+    n = 50000
+    v = rng.standard_normal((n, 3)) * 10.0 ** rng.integers(-8, 8, (n, 1))
+    x = rng.standard_normal((n, 3))
+    pos, vel, mass = np.concatenate([x, x]), np.concatenate([v, -v]), np.full(2 * n, 0.37)
+    ctx = bh.Context(2 * n, 16)
+    d = bh.bh_diagnostics(ctx.ctx, dev(pos), dev(vel), dev(mass), None)
+    sc = _sum_abs_terms(pos, vel, mass, np.zeros(2 * n))
+    assert (np.abs(d["P"]) <= 1e-28 * sc["P"]).all() and (np.abs(d["L"]) <= 1e-28 * sc["L"]).all()
+    ctx.close()
+
+
+@pytest.mark.parametrize("n", [1, 33, 100000])
+def test_position_error_bit_exact(n):
+    rng = np.random.default_rng(n)
+    ref = rng.standard_normal((n, 3))
+    pos = ref + 1e-6 * rng.standard_normal((n, 3))
+    if n > 10:
+        ref[3] = 0.0            # R25: skipped
+        pos[5] = ref[5]         # zero error
+    ctx = bh.Context(n, 16)
+    e = bh.bh_position_error(ctx.ctx, dev(pos), dev(ref))
+    assert e == orc.position_error(pos, ref)
+    assert bh.bh_position_error(ctx.ctx, dev(ref), dev(ref)) == 0.0
+    ctx.close()
+
+
+def test_gravity_dt():
+    for G, rho in [(6.674e-11, 3000.0), (1.0, 0.24), (6.674e-11, 2000.0)]:
+        assert bh.bh_gravity_dt(G, rho) == orc.gravity_dt(G, rho)
+
+
+@pytest.mark.parametrize("name,n,C", [("c4", 20000, 16), ("c5", 10000, 32)])
+def test_euler_and_multirate_steps(name, n, C):
+    """Per evaluation on bit-identical inputs: the oracle advances from the GPU's own
+    positions of the previous step; accelerations within 1e-11, and the update itself bit-exact when fed
+    the GPU's accelerations."""
+    w = wl.make(name, n)
+    dt = 1e-3
+    ctx = bh.Context(n, C)
+    pos, vel, mass = dev(w.pos), dev(w.vel), dev(w.mass)
+    bh.bh_bind_state(ctx.ctx, pos, vel, mass, w.theta, w.eps, w.G)
+    for kind, n_sub in (("euler", 1), ("multirate", 5), ("euler", 1)):
+        p0, v0 = pos.cpu().numpy().copy(), vel.cpu().numpy().copy()
+        if kind == "euler":
+            bh.bh_euler_step(ctx.ctx, dt)
+        else:
+            bh.bh_multirate_step(ctx.ctx, dt, n_sub)
+        bh.bh_synchronize(ctx.ctx)
+        # the accelerations the step used: a(x_k)
+        a_dev = torch.empty((n, 3), dtype=torch.float64, device="cuda")
+        bh.bh_copy_state_acc(ctx.ctx, a_dev)
+        a_gpu = a_dev.cpu().numpy()
+        t = orc.build(p0, w.mass, C)
+        a_ref = orc.accel(t, w.theta, w.eps, w.G)[0]
+        e = np.linalg.norm(a_gpu - a_ref, axis=1) / np.linalg.norm(a_ref, axis=1)
+        assert e.max() <= TOL
+        # oracle update from the GPU's accelerations: bit for bit
+        pr, vr = p0.copy(), v0.copy()
+        for _ in range(n_sub):
+            orc.kick(vr, a_gpu, dt)
+            orc.drift(pr, vr, dt)
+        assert np.array_equal(vel.cpu().numpy(), vr) and np.array_equal(pos.cpu().numpy(), pr)
+        # and the whole oracle step (its own accelerations) agrees to the tolerance of the accelerations
+        s = orc.Stepper(p0, v0, w.mass, w.theta, w.eps, w.G, C)
+        s.euler(dt) if kind == "euler" else s.multirate(dt, n_sub)
+        assert np.abs(vel.cpu().numpy() - s.vel).max() <= TOL * np.abs(a_ref).max() * dt * n_sub * 10
+    ctx.close()
+
+
+def test_stepper_state_errors():
+    ctx = bh.Context(100, 8)
+    with pytest.raises(bh.BhError) as ei:
+        bh.bh_euler_step(ctx.ctx, 1e-3)
+    assert ei.value.status == bh.BH_ERR_STATE
+    w = wl.make("c1", 100)
+    pos, vel, mass = dev(w.pos), dev(np.zeros((100, 3))), dev(w.mass)
+    bh.bh_bind_state(ctx.ctx, pos, vel, mass, 0.5, 1e-3, 1.0)
+    with pytest.raises(bh.BhError) as ei:
+        bh.bh_multirate_step(ctx.ctx, 1e-3, 0)
+    assert ei.value.status == bh.BH_ERR_INVALID_ARG
+    # Euler then KDK: the KDK step re-evaluates a(x) (the Euler step leaves a(x_k) behind)
+    bh.bh_euler_step(ctx.ctx, 1e-3)
+    p0, v0 = pos.cpu().numpy().copy(), vel.cpu().numpy().copy()
+    bh.bh_kdk_step(ctx.ctx, 1e-3)
+    bh.bh_synchronize(ctx.ctx)
+    lf = orc.Leapfrog(p0, v0, w.mass, 0.5, 1e-3, 1.0, 8)
+    lf.step(1e-3)
+    assert np.abs(pos.cpu().numpy() - lf.pos).max() <= 1e-13
+    ctx.close()
