@@ -95,6 +95,12 @@ bh_status bh_copy_state_acc(bh_ctx *ctx, double *acc_dev);
 
 /* ---- rows "next" of SURVEY.md 8(f): the paper's stepping variants and conservation diagnostics ---- */
 
+/* How the steppers (bh_kdk_step, bh_euler_step, bh_multirate_step) evaluate gravity
+ * "through N^2 interactions or by building the octree" (direct for few bodies, octree for
+ * many): method 0 = Barnes-Hut tree (default), 1 = direct N^2 sum, Eq. (1), without building a tree.
+ * After a direct evaluation the context holds no tree: bh_accel etc. need a new bh_build. */
+bh_status bh_set_gravity_method(bh_ctx *ctx, int method);
+
 /* Semi-implicit (symplectic) Euler, the paper's preferred stepper, on the state of
  * bh_bind_state:  rebuild tree;  a = accel(x_k);  v_k+1 = fma(a, dt, v_k);  x_k+1 = fma(v_k+1, dt, x_k).
  * One evaluation per step.  Afterwards the context holds a(x_k), so a following bh_kdk_step starts by

@@ -54,6 +54,7 @@ def lib() -> C.CDLL:
             "bh_kdk_step": [vp, dbl],
             "bh_get_state_acc": [vp, C.POINTER(vp)],
             "bh_copy_state_acc": [vp, vp],
+            "bh_set_gravity_method": [vp, i32],
             "bh_euler_step": [vp, dbl],
             "bh_multirate_step": [vp, dbl, i32],
             "bh_potential": [vp, dbl, dbl, dbl, vp],
@@ -90,7 +91,7 @@ EXPORTS = ("bh_workspace_bytes", "bh_create", "bh_destroy", "bh_set_stream", "bh
            "bh_set_timing",
            "bh_get_phase_ms", "bh_measure_fp64_peak", "bh_last_error", "bh_version",
            "bh_euler_step", "bh_multirate_step", "bh_potential", "bh_direct_potential", "bh_diagnostics",
-           "bh_position_error", "bh_gravity_dt", "bh_copy_state_acc")
+           "bh_position_error", "bh_gravity_dt", "bh_copy_state_acc", "bh_set_gravity_method")
 
 
 def _check(ctx, status: int):
@@ -170,6 +171,10 @@ def bh_kdk_step(ctx, dt: float):
 
 def bh_copy_state_acc(ctx, acc: torch.Tensor):
     _check(ctx, lib().bh_copy_state_acc(ctx, _dev(acc, torch.float64, "acc")))
+
+
+def bh_set_gravity_method(ctx, method: int):
+    _check(ctx, lib().bh_set_gravity_method(ctx, method))
 
 
 def bh_euler_step(ctx, dt: float):

@@ -23,6 +23,7 @@ struct bh_ctx {
     int64_t bound_n = 0;
     double theta = 0, eps = 0, G = 0;
     bool bound = false, have_acc = false;
+    bool use_direct = false;   // steppers evaluate gravity by the direct N^2 sum instead of the tree
     bool acc_filled = false;   // ws.acc holds the accelerations of the last stepper evaluation
     // timing
     bool timing = false;
@@ -148,6 +149,26 @@ bh_status do_accel(bh_ctx *c, double theta, double eps, double G, double *acc, b
         c->launches += 1;
     }
     return st;
+}
+
+// One gravity evaluation of the bound state into ws.acc, by the method bh_set_gravity_method chose
+// ("through N^2 interactions or by building the octree").
+bh_status do_eval_state(bh_ctx *c)
+{
+    if (!c->use_direct) {
+        bh_status st = do_build(c, c->pos, c->mass, c->bound_n);
+        if (st != BH_OK) return st;
+        return do_accel(c, c->theta, c->eps, c->G, c->ws.acc);
+    }
+    // direct sum: no tree, bodies packed in their own order
+    c->built = false;
+    c->walked = false;
+    launch_pack(c->ws, c->pos, c->mass, c->bound_n, c->stream);
+    {
+        Phase p(c, 7);
+        c->launches += 1 + launch_direct(c->ws, c->bound_n, nullptr, c->bound_n, c->eps, c->G, c->ws.acc, false, c->stream);
+    }
+    return cuda_check(c, cudaGetLastError(), "direct evaluation launch");
 }
 
 }  // namespace
@@ -352,8 +373,7 @@ bh_status bh_kdk_step(bh_ctx *c, double dt)
     if (!c->bound) return fail(c, BH_ERR_STATE, "bh_kdk_step before bh_bind_state");
     bh_status st;
     if (!c->have_acc) {   // a(x0), once
-        if ((st = do_build(c, c->pos, c->mass, c->bound_n)) != BH_OK) return st;
-        if ((st = do_accel(c, c->theta, c->eps, c->G, c->ws.acc)) != BH_OK) return st;
+        if ((st = do_eval_state(c)) != BH_OK) return st;
         c->have_acc = true;
     }
     if (c->timing) cudaEventRecord(c->ev[8][0], c->stream);
@@ -362,8 +382,7 @@ bh_status bh_kdk_step(bh_ctx *c, double dt)
         cudaEventRecord(c->ev[8][1], c->stream);
         c->ev_set[8] = true;
     }
-    if ((st = do_build(c, c->pos, c->mass, c->bound_n)) != BH_OK) return st;
-    if ((st = do_accel(c, c->theta, c->eps, c->G, c->ws.acc)) != BH_OK) return st;
+    if ((st = do_eval_state(c)) != BH_OK) return st;
     launch_kick(c->vel, c->ws.acc, c->bound_n, dt * 0.5, c->stream);
     c->acc_filled = true;
     c->launches += 2;   // kick+drift, kick
@@ -377,8 +396,7 @@ static bh_status euler_like(bh_ctx *c, double dt, int n_sub, const char *who)
     if (!c->bound) return fail(c, BH_ERR_STATE, "stepper called before bh_bind_state");
     if (n_sub < 1) return fail(c, BH_ERR_INVALID_ARG, "n_sub < 1");
     bh_status st;
-    if ((st = do_build(c, c->pos, c->mass, c->bound_n)) != BH_OK) return st;
-    if ((st = do_accel(c, c->theta, c->eps, c->G, c->ws.acc)) != BH_OK) return st;
+    if ((st = do_eval_state(c)) != BH_OK) return st;
     c->have_acc = false;   // acc is a(x_k), not a(x_k+1): a later bh_kdk_step re-evaluates
     c->acc_filled = true;
     if (c->timing) cudaEventRecord(c->ev[8][0], c->stream);
@@ -389,6 +407,15 @@ static bh_status euler_like(bh_ctx *c, double dt, int n_sub, const char *who)
     }
     c->launches += 1;
     return cuda_check(c, cudaGetLastError(), who);
+}
+
+bh_status bh_set_gravity_method(bh_ctx *c, int method)
+{
+    if (!c) return BH_ERR_INVALID_ARG;
+    if (method != 0 && method != 1) return fail(c, BH_ERR_INVALID_ARG, "bh_set_gravity_method: method must be 0 or 1");
+    c->use_direct = method == 1;
+    c->have_acc = false;
+    return BH_OK;
 }
 
 bh_status bh_euler_step(bh_ctx *c, double dt) { return euler_like(c, dt, 1, "bh_euler_step launch"); }

@@ -100,6 +100,8 @@ void launch_cube(const Workspace &w, const double *pos, int64_t n, cudaStream_t 
 void launch_keys(const Workspace &w, const double *pos, int64_t n, cudaStream_t s);
 void launch_sort(const Workspace &w, int64_t n, cudaStream_t s);   // result in key[0]/idx[0]
 void launch_gather(const Workspace &w, const double *pos, const double *mass, int64_t n, cudaStream_t s);
+// (x,y,z,m) in the caller's body order with the identity permutation: input of a direct sum without a tree
+void launch_pack(const Workspace &w, const double *pos, const double *mass, int64_t n, cudaStream_t s);
 void launch_tree(const Workspace &w, int64_t n, int leaf_cap, cudaStream_t s);
 void launch_monopoles(const Workspace &w, int64_t n, cudaStream_t s);
 // potential = false: acc [n][3] accelerations; true: acc [n] potential (NEXT-1)

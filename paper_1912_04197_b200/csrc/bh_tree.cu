@@ -41,6 +41,17 @@ __global__ void __launch_bounds__(256) gather_kernel(const double *__restrict__ 
     iperm[i] = (unsigned)j;
 }
 
+__global__ void __launch_bounds__(256) pack_kernel(const double *__restrict__ pos, const double *__restrict__ mass,
+                                                   long long n, double4 *__restrict__ sbody,
+                                                   unsigned *__restrict__ perm, unsigned *__restrict__ iperm)
+{
+    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    sbody[i] = make_double4(pos[3 * i], pos[3 * i + 1], pos[3 * i + 2], mass[i]);
+    perm[i] = (unsigned)i;
+    iperm[i] = (unsigned)i;
+}
+
 // exact bounding box of every walk group (one warp per group, lanes stride over its bodies)
 __global__ void __launch_bounds__(256) group_box_kernel(const DevState *__restrict__ st,
                                                         const unsigned *__restrict__ gstart,
@@ -402,6 +413,11 @@ void launch_gather(const Workspace &w, const double *pos, const double *mass, in
 {
     int blocks = (int)((n + 255) / 256);
     gather_kernel<<<blocks, 256, 0, s>>>(pos, mass, w.idx[0], n, w.sbody, w.iperm);
+}
+
+void launch_pack(const Workspace &w, const double *pos, const double *mass, int64_t n, cudaStream_t s)
+{
+    pack_kernel<<<(int)((n + 255) / 256), 256, 0, s>>>(pos, mass, n, w.sbody, w.idx[0], w.iperm);
 }
 
 void launch_tree(const Workspace &w, int64_t n, int leaf_cap, cudaStream_t s)

@@ -189,3 +189,41 @@ def test_stepper_state_errors():
     lf.step(1e-3)
     assert np.abs(pos.cpu().numpy() - lf.pos).max() <= 1e-13
     ctx.close()
+
+
+def test_steppers_with_direct_gravity():
+    """bh_set_gravity_method(1): the steppers evaluate Eq. (1) directly, no tree."""
+    w = wl.make("c1", 600)
+    rng = np.random.default_rng(5)
+    v0 = 0.1 * rng.standard_normal((600, 3))
+    ctx = bh.Context(600, 8)
+    pos, vel, mass = dev(w.pos), dev(v0), dev(w.mass)
+    bh.bh_bind_state(ctx.ctx, pos, vel, mass, w.theta, w.eps, w.G)
+    bh.bh_set_gravity_method(ctx.ctx, 1)
+    lf = orc.Leapfrog(w.pos, v0, w.mass, w.theta, w.eps, w.G, 8, use_direct=True)
+    for _ in range(3):
+        bh.bh_kdk_step(ctx.ctx, 1e-3)
+        lf.step(1e-3)
+    bh.bh_synchronize(ctx.ctx)
+    assert np.abs(pos.cpu().numpy() - lf.pos).max() <= 1e-13
+    assert np.abs(vel.cpu().numpy() - lf.vel).max() <= 1e-12
+    a = torch.empty((600, 3), dtype=torch.float64, device="cuda")
+    bh.bh_copy_state_acc(ctx.ctx, a)
+    ref = orc.direct(lf.pos, w.mass, w.eps, w.G)
+    assert (np.linalg.norm(a.cpu().numpy() - ref, axis=1) / np.linalg.norm(ref, axis=1)).max() <= 1e-10
+    # no tree after a direct evaluation
+    with pytest.raises(bh.BhError) as ei:
+        ctx.n = 600
+        ctx.accel(0.5, 1e-3, 1.0)
+    assert ei.value.status == bh.BH_ERR_STATE
+    # Euler with direct gravity, then back to the tree
+    st = orc.Stepper(lf.pos, lf.vel, w.mass, w.theta, w.eps, w.G, 8, use_direct=True)
+    bh.bh_euler_step(ctx.ctx, 1e-3)
+    st.euler(1e-3)
+    bh.bh_synchronize(ctx.ctx)
+    assert np.abs(pos.cpu().numpy() - st.pos).max() <= 1e-13
+    bh.bh_set_gravity_method(ctx.ctx, 0)
+    bh.bh_euler_step(ctx.ctx, 1e-3)
+    bh.bh_synchronize(ctx.ctx)
+    assert bh.bh_get_node_count(ctx.ctx)[0] > 1
+    ctx.close()
