@@ -621,3 +621,143 @@ double orc_position_error(const double *pos, const double *ref, int64_t n)
  * Returns the bound 1 / (2 sqrt(G rho)).
  * ------------------------------------------------------------------------------------------- */
 double orc_gravity_dt(double G, double rho) { return 1.0 / (2.0 * sqrt(G * rho)); }
+
+/* =============================================================================================
+ * Rows NEXT-3 and NEXT-4 of SURVEY.md §8(f): broad-phase collision detection and aggregate
+ * identification.
+ * ========================================================================================== */
+
+/* ---------------------------------------------------------------------------------------------
+ * O17  Broad phase: "pairs of bodies whose geometrical boundaries are close enough are
+ * identified.  The bounding volume of a body is estimated based on its velocity and integration time
+ * step.  If the bounding volume of two bodies overlap, the narrow phase is performed".
+ * Reading R26: the bounding volume of body i is the sphere about its centre of radius
+ *     b_i = fma(|v_i|, dt, R_i),   |v_i| = sqrt(fma(vz, vz, fma(vy, vy, vx*vx)))
+ * (R_i the radius of the body's circumscribed sphere; within one step its boundary cannot leave that
+ * sphere), and two volumes overlap iff  |x_j - x_i|^2 <= (b_i + b_j)^2  (touching counts), evaluated as
+ *     d = x_j - x_i per component;  d2 = fma(dz, dz, fma(dy, dy, dx*dx));  s = b_i + b_j;  d2 <= s*s
+ * with every operation rounded once, so that the set of pairs is reproducible bit for bit.
+ * Plain definition: all i < j are tested.  orc_bound_radius fills b[n] (vel may be NULL: b = R).
+ * orc_broadphase returns the number of pairs and writes the first `cap` of them, (i, j) with i < j, in
+ * lexicographic order.
+ * ------------------------------------------------------------------------------------------- */
+void orc_bound_radius(const double *vel, const double *radius, int64_t n, double dt, double *b)
+{
+    for (int64_t i = 0; i < n; ++i) {
+        if (!vel) {
+            b[i] = radius[i];
+            continue;
+        }
+        double vx = vel[3 * i], vy = vel[3 * i + 1], vz = vel[3 * i + 2];
+        double sp = sqrt(fma(vz, vz, fma(vy, vy, vx * vx)));
+        b[i] = fma(sp, dt, radius[i]);
+    }
+}
+
+static inline int orc_overlap(const double *pos, const double *b, int64_t i, int64_t j)
+{
+    double dx = pos[3 * j] - pos[3 * i], dy = pos[3 * j + 1] - pos[3 * i + 1], dz = pos[3 * j + 2] - pos[3 * i + 2];
+    double d2 = fma(dz, dz, fma(dy, dy, dx * dx));
+    double s = b[i] + b[j];
+    return d2 <= s * s;
+}
+
+int64_t orc_broadphase(const double *pos, const double *b, int64_t n, int32_t *pairs, int64_t cap)
+{
+    /* per-row counts in parallel, then rows are written in order */
+    int64_t *cnt = (int64_t *)calloc((size_t)n + 1, sizeof(int64_t));
+#pragma omp parallel for schedule(dynamic, 64)
+    for (int64_t i = 0; i < n; ++i) {
+        int64_t c = 0;
+        for (int64_t j = i + 1; j < n; ++j) c += orc_overlap(pos, b, i, j);
+        cnt[i + 1] = c;
+    }
+    for (int64_t i = 0; i < n; ++i) cnt[i + 1] += cnt[i];
+    int64_t total = cnt[n];
+#pragma omp parallel for schedule(dynamic, 64)
+    for (int64_t i = 0; i < n; ++i) {
+        int64_t at = cnt[i];
+        if (at == cnt[i + 1]) continue;
+        for (int64_t j = i + 1; j < n; ++j)
+            if (orc_overlap(pos, b, i, j)) {
+                if (at < cap) {
+                    pairs[2 * at] = (int32_t)i;
+                    pairs[2 * at + 1] = (int32_t)j;
+                }
+                ++at;
+            }
+    }
+    free(cnt);
+    return total;
+}
+
+/* ---------------------------------------------------------------------------------------------
+ * O18  Aggregate identification: bodies are the vertices of a graph, contacts its
+ * edges ("a contact container is filled with pairs ID_i, ID_j"); "aggregates obtained correspond to
+ * the connected subgraphs"; "the number of aggregates is defined as the number of connected
+ * components ... with a size greater than one"; "a Depth First Search (DFS) algorithm ... complexity
+ * of O(N+E)".  Followed as written: adjacency lists from the pairs, DFS with an explicit stack from
+ * every unvisited vertex in increasing id.  label[v] = id of the DFS root = smallest vertex of the
+ * component (canonical, so it can be compared exactly); size[r] and mass[r] (sum of the members' masses
+ * in increasing vertex id; mass_in may be NULL) are set at roots r and are 0 elsewhere.
+ * counts[0] = connected components, counts[1] = aggregates (components with more than one body).
+ * Self-pairs and repeated pairs are allowed and change nothing.  Returns 0, or -1 if a pair names a
+ * vertex outside [0, n).
+ * ------------------------------------------------------------------------------------------- */
+int orc_aggregates(int64_t n, const int32_t *pairs, int64_t n_pairs, const double *mass_in, int32_t *label,
+                   int32_t *size, double *mass, int64_t counts[2])
+{
+    int64_t *off = (int64_t *)calloc((size_t)n + 1, sizeof(int64_t));
+    for (int64_t e = 0; e < n_pairs; ++e) {
+        int32_t a = pairs[2 * e], b = pairs[2 * e + 1];
+        if (a < 0 || b < 0 || a >= n || b >= n) {
+            free(off);
+            return -1;
+        }
+        ++off[a + 1];
+        ++off[b + 1];
+    }
+    for (int64_t v = 0; v < n; ++v) off[v + 1] += off[v];
+    int32_t *adj = (int32_t *)malloc(sizeof(int32_t) * (size_t)(2 * n_pairs + 1));
+    int64_t *fill = (int64_t *)malloc(sizeof(int64_t) * (size_t)(n + 1));
+    memcpy(fill, off, sizeof(int64_t) * (size_t)(n + 1));
+    for (int64_t e = 0; e < n_pairs; ++e) {
+        int32_t a = pairs[2 * e], b = pairs[2 * e + 1];
+        adj[fill[a]++] = b;
+        adj[fill[b]++] = a;
+    }
+    int32_t *stack = (int32_t *)malloc(sizeof(int32_t) * (size_t)(2 * n_pairs + n + 1));
+    for (int64_t v = 0; v < n; ++v) {
+        label[v] = -1;
+        if (size) size[v] = 0;
+        if (mass) mass[v] = 0.0;
+    }
+    counts[0] = counts[1] = 0;
+    for (int64_t r = 0; r < n; ++r) {
+        if (label[r] >= 0) continue;
+        int64_t top = 0, members = 0;
+        stack[top++] = (int32_t)r;
+        label[r] = (int32_t)r;
+        while (top > 0) {
+            int32_t v = stack[--top];
+            ++members;
+            for (int64_t k = off[v]; k < off[v + 1]; ++k) {
+                int32_t u = adj[k];
+                if (label[u] < 0) {
+                    label[u] = (int32_t)r;
+                    stack[top++] = u;
+                }
+            }
+        }
+        if (size) size[r] = (int32_t)members;
+        ++counts[0];
+        if (members > 1) ++counts[1];
+    }
+    if (mass && mass_in)
+        for (int64_t v = 0; v < n; ++v) mass[label[v]] += mass_in[v];
+    free(off);
+    free(adj);
+    free(fill);
+    free(stack);
+    return 0;
+}

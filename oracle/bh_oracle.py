@@ -351,3 +351,45 @@ class Stepper:
         for _ in range(n_sub):
             kick(self.vel, self.acc, dt_c)
             drift(self.pos, self.vel, dt_c)
+
+
+# ------------------------------------------------------------------ rows NEXT-3 / NEXT-4
+def bound_radius(vel, radius, dt: float) -> np.ndarray:
+    """O17 (R26): b_i = fma(|v_i|, dt, R_i); vel may be None (b = R)."""
+    radius = np.ascontiguousarray(radius, dtype=np.float64)
+    b = np.zeros_like(radius)
+    if vel is not None:
+        vel = np.ascontiguousarray(vel, dtype=np.float64)
+    lib().orc_bound_radius(_p(vel) if vel is not None else None, _p(radius), C.c_int64(radius.shape[0]),
+                           C.c_double(dt), _p(b))
+    return b
+
+
+def broadphase(pos, b) -> np.ndarray:
+    """O17: all pairs i < j with |x_j - x_i|^2 <= (b_i + b_j)^2 -> int32 [P,2], lexicographic."""
+    pos = np.ascontiguousarray(pos, dtype=np.float64)
+    b = np.ascontiguousarray(b, dtype=np.float64)
+    n = pos.shape[0]
+    f = lib().orc_broadphase
+    f.restype = C.c_int64
+    total = f(_p(pos), _p(b), C.c_int64(n), None, C.c_int64(0))
+    pairs = np.zeros((max(total, 1), 2), dtype=np.int32)
+    f(_p(pos), _p(b), C.c_int64(n), _p(pairs), C.c_int64(total))
+    return pairs[:total]
+
+
+def aggregates(n: int, pairs, mass=None):
+    """O18 -> dict(label[n], size[n], mass[n] or None, components, aggregates)."""
+    pairs = np.ascontiguousarray(pairs, dtype=np.int32).reshape(-1, 2)
+    label = np.zeros(n, dtype=np.int32)
+    size = np.zeros(n, dtype=np.int32)
+    out_mass = np.zeros(n) if mass is not None else None
+    if mass is not None:
+        mass = np.ascontiguousarray(mass, dtype=np.float64)
+    counts = np.zeros(2, dtype=np.int64)
+    rc = lib().orc_aggregates(C.c_int64(n), _p(pairs) if pairs.size else None, C.c_int64(pairs.shape[0]),
+                              _p(mass) if mass is not None else None, _p(label), _p(size),
+                              _p(out_mass) if mass is not None else None, _p(counts))
+    if rc != 0:
+        raise ValueError("pair index out of range")
+    return dict(label=label, size=size, mass=out_mass, components=int(counts[0]), aggregates=int(counts[1]))

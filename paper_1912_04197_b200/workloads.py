@@ -119,7 +119,8 @@ def c2(n: int = 16384, seed: int = BASE_SEED + 2) -> Workload:
     r = (a - u * (a - b)) ** -0.5
     mass = 2000.0 * (4.0 / 3.0) * math.pi * r ** 3
     return Workload("c2", pos, mass, None, 6.674e-11, 0.0, 0.5, 16, seed=seed,
-                    note="ball R=1000 m, radii power law r^-3 on [5,50] m, rho=2000 kg/m^3")
+                    note="ball R=1000 m, radii power law r^-3 on [5,50] m, rho=2000 kg/m^3",
+                    extra={"radius": r})
 
 
 def c3(n: int = 131072, seed: int = BASE_SEED + 3) -> Workload:
@@ -174,6 +175,21 @@ def c5(n: int = 4194304, seed: int = BASE_SEED + 5) -> Workload:
         vel[:, a] += 0.05 * _gauss(seed, 8 + a, n)
     return Workload("c5", pos, mass, vel, 1.0, 1e-3, 0.6, 32, dt=1e-3, steps=50, seed=seed,
                     note="uniform ball R=10, m=1/N, spin 0.3 critical + sigma=0.05")
+
+
+def spheres(n: int, seed: int = BASE_SEED + 6, mean_contacts: float = 1.5, speed: float = 0.0) -> Workload:
+    """Cloud of finite-size bodies for the broad phase / aggregate rows:
+    centres uniform in the unit ball, bounding radii uniform in [0.5, 1.5] r0 with r0 chosen so that a
+    body's sphere overlaps `mean_contacts` others on average (N (2 r0)^3 = mean_contacts) — around the
+    percolation threshold, so aggregates of every size appear, as at the end of the paper's transient
+    phase.  Optional random velocities of typical magnitude `speed`."""
+    pos = _ball(seed, 0, n, 1.0)
+    r0 = 0.5 * (mean_contacts / n) ** (1.0 / 3.0)
+    radius = r0 * (0.5 + uniform(seed, 1, 0, n))
+    vel = _isotropic(seed, 2, n) * (speed * uniform(seed, 3, 0, n))[:, None] if speed > 0 else None
+    mass = (4.0 / 3.0) * math.pi * radius ** 3
+    return Workload("spheres", pos, mass, vel, 1.0, 0.0, 0.5, 16, seed=seed,
+                    note=f"unit ball, radii U[0.5,1.5] r0, r0={r0:.3e}", extra={"radius": radius})
 
 
 CONFIGS = {"c1": c1, "c2": c2, "c3": c3, "c4": c4, "c5": c5}
