@@ -138,6 +138,28 @@ bh_status bh_diagnostics(bh_ctx *ctx, const double *pos_dev, const double *vel_d
 bh_status bh_position_error(bh_ctx *ctx, const double *pos_dev, const double *ref_dev, int64_t n,
                             double *err_host);
 
+/* Synchronising. Broad phase of the collision detection over the bodies of the last
+ * bh_build, on its octree: the bounding volume of body i is the sphere of radius
+ * b_i = fma(|v_i|, dt, R_i) about its centre (R26: "estimated based on its velocity and integration time
+ * step"; radius_dev [n] = circumscribed radius R_i, vel_dev [n][3] or NULL for b = R, both in bh_build
+ * order); a pair i < j is reported iff |x_j - x_i|^2 <= (b_i + b_j)^2 (touching counts) with
+ * d2 = fma(dz, dz, fma(dy, dy, dx*dx)) and every operation rounded once.  Pairs (i, j), i < j, are written
+ * to pairs_dev [capacity][2] in no particular order, each once; *count_host = number found.  capacity 0
+ * (pairs_dev may be NULL) only counts.  BH_ERR_CAPACITY if count > capacity > 0 (the first `capacity`
+ * slots are filled, *count_host is valid: call again with a larger buffer). */
+bh_status bh_broadphase(bh_ctx *ctx, const double *radius_dev, const double *vel_dev, double dt,
+                        int32_t *pairs_dev, int64_t capacity, int64_t *count_host);
+
+/* Synchronising. Aggregate identification: connected components of the graph whose
+ * vertices are the n bodies and whose edges are the n_pairs contacts pairs_dev [n_pairs][2] (any order,
+ * repeats and self-pairs allowed).  label_dev [n] = smallest body id of the body's component;
+ * size_dev [n] (may be NULL) = number of bodies, at the component's label, 0 elsewhere; agg_mass_dev [n]
+ * (may be NULL; needs mass_dev [n]) = total mass, same layout (atomic sums: order not fixed, ~n ulp).
+ * counts_host[0] = components, [1] = aggregates = components with more than one body.
+ * Needs no build; n <= max_n.  BH_ERR_INVALID_ARG if a pair names a body outside [0, n). */
+bh_status bh_aggregates(bh_ctx *ctx, int64_t n, const int32_t *pairs_dev, int64_t n_pairs, const double *mass_dev,
+                        int32_t *label_dev, int32_t *size_dev, double *agg_mass_dev, int64_t counts_host[2]);
+
 /* Host helper. Upper bound of the gravity time step, Eq. (8): 1 / (2 sqrt(G rho)). */
 double bh_gravity_dt(double G, double rho);
 

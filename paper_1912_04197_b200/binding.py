@@ -61,6 +61,8 @@ def lib() -> C.CDLL:
             "bh_direct_potential": [vp, dbl, dbl, vp],
             "bh_diagnostics": [vp, vp, vp, vp, vp, i64, C.POINTER(dbl)],
             "bh_position_error": [vp, vp, vp, i64, C.POINTER(dbl)],
+            "bh_broadphase": [vp, vp, vp, dbl, vp, i64, C.POINTER(i64)],
+            "bh_aggregates": [vp, i64, vp, i64, vp, vp, vp, vp, C.POINTER(i64)],
             "bh_eval_host": [vp, vp, vp, i64, dbl, dbl, dbl, vp],
             "bh_synchronize": [vp],
             "bh_get_cube": [vp, C.POINTER(dbl), C.POINTER(dbl)],
@@ -91,7 +93,8 @@ EXPORTS = ("bh_workspace_bytes", "bh_create", "bh_destroy", "bh_set_stream", "bh
            "bh_set_timing",
            "bh_get_phase_ms", "bh_measure_fp64_peak", "bh_last_error", "bh_version",
            "bh_euler_step", "bh_multirate_step", "bh_potential", "bh_direct_potential", "bh_diagnostics",
-           "bh_position_error", "bh_gravity_dt", "bh_copy_state_acc", "bh_set_gravity_method")
+           "bh_position_error", "bh_gravity_dt", "bh_copy_state_acc", "bh_set_gravity_method",
+           "bh_broadphase", "bh_aggregates")
 
 
 def _check(ctx, status: int):
@@ -206,6 +209,29 @@ def bh_position_error(ctx, pos, ref) -> float:
     _check(ctx, lib().bh_position_error(ctx, _dev(pos, torch.float64, "pos"), _dev(ref, torch.float64, "ref"),
                                         pos.shape[0], C.byref(v)))
     return v.value
+
+
+def bh_broadphase(ctx, radius, vel, dt: float, pairs: torch.Tensor | None) -> int:
+    """Returns the number of pairs found; raises BhError(BH_ERR_CAPACITY) if `pairs` is too small
+    (the exception's .count holds the number found)."""
+    cnt = C.c_int64()
+    cap = 0 if pairs is None else pairs.shape[0]
+    st = lib().bh_broadphase(ctx, _dev(radius, torch.float64, "radius"), _dev(vel, torch.float64, "vel"), dt,
+                             _dev(pairs, torch.int32, "pairs"), cap, C.byref(cnt))
+    if st != BH_OK:
+        err = BhError(st, lib().bh_last_error(ctx).decode())
+        err.count = cnt.value
+        raise err
+    return cnt.value
+
+
+def bh_aggregates(ctx, n: int, pairs: torch.Tensor | None, mass, label, size=None, agg_mass=None):
+    counts = (C.c_int64 * 2)()
+    npairs = 0 if pairs is None else pairs.shape[0]
+    _check(ctx, lib().bh_aggregates(ctx, n, _dev(pairs, torch.int32, "pairs") if npairs else None, npairs,
+                                    _dev(mass, torch.float64, "mass"), _dev(label, torch.int32, "label"),
+                                    _dev(size, torch.int32, "size"), _dev(agg_mass, torch.float64, "agg_mass"), counts))
+    return counts[0], counts[1]
 
 
 def bh_gravity_dt(G: float, rho: float) -> float:

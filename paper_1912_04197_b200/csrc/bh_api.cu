@@ -224,6 +224,11 @@ Workspace carve(char *base, int64_t max_n, int leaf_cap)
     w.diag_part = cv.take<double>((size_t)kDiagBlocks * 16);
     w.diag_out = cv.take<double>(16);
     w.diag_ticket = base ? &w.st->ticket_diag : nullptr;
+    w.bsort = cv.take<double>(n);
+    w.box_lo = cv.take<double4>(w.node_cap);
+    w.box_hi = cv.take<double4>(w.node_cap);
+    w.bp_cnt = cv.take<unsigned>(w.node_cap);
+    w.agg_size = cv.take<int>(n);
     w.total_bytes = cv.off;
     return w;
 }
@@ -480,6 +485,43 @@ bh_status bh_position_error(bh_ctx *c, const double *pos_dev, const double *ref_
     bh_status st = cuda_check(c, cudaGetLastError(), "bh_position_error launch");
     if (st != BH_OK) return st;
     return read_diag(c, 8, 1, err_host);
+}
+
+bh_status bh_broadphase(bh_ctx *c, const double *radius_dev, const double *vel_dev, double dt, int32_t *pairs_dev,
+                        int64_t capacity, int64_t *count_host)
+{
+    if (!c) return BH_ERR_INVALID_ARG;
+    if (!c->built) return fail(c, BH_ERR_STATE, "bh_broadphase before bh_build");
+    if (!radius_dev || !count_host) return fail(c, BH_ERR_INVALID_ARG, "bh_broadphase: null pointer");
+    if (capacity < 0 || (capacity > 0 && !pairs_dev)) return fail(c, BH_ERR_INVALID_ARG, "bh_broadphase: bad pair buffer");
+    if (!(dt >= 0.0)) return fail(c, BH_ERR_INVALID_ARG, "bh_broadphase: dt negative");
+    c->launches += launch_broadphase(c->ws, c->n, radius_dev, vel_dev, dt, pairs_dev, capacity, c->stream);
+    bh_status st = cuda_check(c, cudaGetLastError(), "bh_broadphase launch");
+    if (st != BH_OK) return st;
+    if ((st = fetch_state(c)) != BH_OK) return st;
+    *count_host = (int64_t)c->host_state->pair_count;
+    if (capacity > 0 && *count_host > capacity) return fail(c, BH_ERR_CAPACITY, "bh_broadphase: pair buffer too small");
+    return BH_OK;
+}
+
+bh_status bh_aggregates(bh_ctx *c, int64_t n, const int32_t *pairs_dev, int64_t n_pairs, const double *mass_dev,
+                        int32_t *label_dev, int32_t *size_dev, double *agg_mass_dev, int64_t counts_host[2])
+{
+    if (!c) return BH_ERR_INVALID_ARG;
+    if (!label_dev || !counts_host) return fail(c, BH_ERR_INVALID_ARG, "bh_aggregates: null pointer");
+    if (n < 1 || n > c->max_n) return fail(c, BH_ERR_INVALID_ARG, "bh_aggregates: n out of range");
+    if (n_pairs < 0 || (n_pairs > 0 && !pairs_dev)) return fail(c, BH_ERR_INVALID_ARG, "bh_aggregates: bad pair list");
+    if (agg_mass_dev && !mass_dev) return fail(c, BH_ERR_INVALID_ARG, "bh_aggregates: agg_mass without mass");
+    c->launches += launch_aggregates(c->ws, n, pairs_dev, n_pairs, mass_dev, label_dev, size_dev, agg_mass_dev, c->stream);
+    bh_status st = cuda_check(c, cudaGetLastError(), "bh_aggregates launch");
+    if (st != BH_OK) return st;
+    cudaError_t e = cudaMemcpyAsync(c->host_state, c->ws.st, sizeof(DevState), cudaMemcpyDeviceToHost, c->stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
+    if (e != cudaSuccess) return cuda_check(c, e, "bh_aggregates readback");
+    if (c->host_state->agg_counts[2]) return fail(c, BH_ERR_INVALID_ARG, "bh_aggregates: a pair names a body outside [0, n)");
+    counts_host[0] = (int64_t)c->host_state->agg_counts[0];
+    counts_host[1] = (int64_t)c->host_state->agg_counts[1];
+    return BH_OK;
 }
 
 double bh_gravity_dt(double G, double rho) { return 1.0 / (2.0 * sqrt(G * rho)); }

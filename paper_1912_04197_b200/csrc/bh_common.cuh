@@ -38,6 +38,8 @@ struct DevState {
     unsigned ticket_bbox;  // last-block election
     unsigned walk_queue;   // dynamic group counter of the walk
     unsigned ticket_diag;  // last-block election of the diagnostics reduction (resets itself)
+    unsigned long long pair_count;     // broad phase: candidate pairs found (may exceed the caller's capacity)
+    unsigned long long agg_counts[3];  // aggregates: connected components, aggregates (size > 1), bad pairs
     unsigned long long stats[4];       // n_mono, n_direct, interactions, nodes tested
 };
 
@@ -78,6 +80,12 @@ struct Workspace {
     double *diag_part;            // [kDiagBlocks][8][2] double-double partial sums of the diagnostics
     double *diag_out;             // [8] conserved quantities, [8] bits of the Eq. (7) maximum
     unsigned *diag_ticket;        // = &st->ticket_diag
+    // rows NEXT-3 / NEXT-4 (bh_contact.cu)
+    double *bsort;                // [n] bounding radius b of the sorted bodies
+    double4 *box_lo;              // [cap] per node: min x,y,z of its bodies' centres, max b
+    double4 *box_hi;              // [cap] per node: max x,y,z
+    unsigned *bp_cnt;             // [cap] arrival counters of the node-box pass
+    int *agg_size;                // [n] component sizes when the caller wants none
     int64_t node_cap;
     int64_t sort_tiles;
     int64_t tree_tiles;
@@ -117,6 +125,11 @@ double run_fp64_peak(const Workspace &w, cudaStream_t s);
 void launch_diagnostics(const Workspace &w, const double *pos, const double *vel, const double *mass,
                         const double *phi, int64_t n, cudaStream_t s);
 void launch_position_error(const Workspace &w, const double *pos, const double *ref, int64_t n, cudaStream_t s);
+// rows NEXT-3 / NEXT-4 (bh_contact.cu); each returns the number of kernels launched
+int launch_broadphase(const Workspace &w, int64_t n, const double *radius, const double *vel, double dt,
+                      int32_t *pairs, int64_t cap, cudaStream_t s);   // count lands in st->pair_count
+int launch_aggregates(const Workspace &w, int64_t n, const int32_t *pairs, int64_t n_pairs, const double *mass_in,
+                      int32_t *label, int32_t *size, double *mass, cudaStream_t s);   // counts in st->agg_counts
 void launch_euler_sub(double *pos, double *vel, const double *acc, int64_t n, double dt, int n_sub, cudaStream_t s);
 
 // ---- small device helpers ----
