@@ -168,6 +168,70 @@ def aggregate(total_ms: float, bodies_per_rank: int, steps: int, world: int, dev
     return tmax, world * bodies_per_rank * steps / (tmax * 1e-3)
 
 
+# ------------------------------------------------------------------------------------------ rows "next"
+def next_rows(ctx, w, pos, vel, mass, dev, hbm_peak):
+    """SURVEY.md 8(f) rows NEXT-1..4 timed beside the headline (CUDA events on the library's stream, median of
+    3, inputs resident): tree potential, conserved quantities, Eq. (7), semi-implicit Euler step on the
+    headline workload; broad phase + aggregate identification on a cloud of N finite-size bodies."""
+    import torch
+    from paper_1912_04197_b200 import binding as bh
+    from paper_1912_04197_b200 import workloads as wl
+    stream = torch.cuda.current_stream()
+
+    def timed(fn, reps=3):
+        ts = []
+        for _ in range(reps):
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record(stream)
+            r = fn()
+            b.record(stream)
+            torch.cuda.synchronize()
+            ts.append(a.elapsed_time(b))
+        return statistics.median(ts), r
+
+    out = {}
+    n = w.n
+    ctx.build(pos, mass)
+    phi = torch.empty(n, dtype=torch.float64, device=dev)
+    bh.bh_potential(ctx.ctx, w.theta, w.eps, w.G, phi)
+    ms, _ = timed(lambda: bh.bh_potential(ctx.ctx, w.theta, w.eps, w.G, phi))
+    inter = bh.bh_get_stats(ctx.ctx)["interactions"]
+    out["potential_walk"] = {"ms": ms, "interactions_per_s": inter / (ms * 1e-3),
+                             "fp64_instr_per_interaction": 12}
+    ms, d = timed(lambda: bh.bh_diagnostics(ctx.ctx, pos, vel, mass, phi))
+    out["diagnostics"] = {"ms": ms, "GB_per_s": 64.0 * n / (ms * 1e-3) / 1e9, "frac_of_hbm_peak": 64.0 * n / (ms * 1e-3) / 1e9 / hbm_peak,
+                          "bytes_per_body": 64, "virial_2K_over_W": -2.0 * d["ekin"] / d["epot"]}
+    ref = pos.clone()
+    ms, _ = timed(lambda: bh.bh_position_error(ctx.ctx, pos, ref))
+    out["position_error"] = {"ms": ms, "GB_per_s": 48.0 * n / (ms * 1e-3) / 1e9, "bytes_per_body": 48}
+    p2, v2 = pos.clone(), vel.clone()
+    bh.bh_bind_state(ctx.ctx, p2, v2, mass, w.theta, w.eps, w.G)
+    bh.bh_euler_step(ctx.ctx, w.dt or 1e-3)
+    ms, _ = timed(lambda: bh.bh_euler_step(ctx.ctx, w.dt or 1e-3))
+    out["euler_step"] = {"ms": ms, "body_accelerations_per_s": n / (ms * 1e-3)}
+    ms, _ = timed(lambda: bh.bh_multirate_step(ctx.ctx, (w.dt or 1e-3) / 8, 8))
+    out["multirate_step_8_substeps"] = {"ms": ms}
+
+    # broad phase + aggregates: N finite-size bodies around the percolation threshold (workloads.spheres)
+    sp = wl.spheres(n, mean_contacts=3.0, speed=0.01)
+    sctx = bh.Context(n, 16, device=dev)
+    spos, smass = torch.as_tensor(sp.pos).to(dev), torch.as_tensor(sp.mass).to(dev)
+    srad, svel = torch.as_tensor(sp.extra["radius"]).to(dev), torch.as_tensor(sp.vel).to(dev)
+    sctx.build(spos, smass)
+    count = bh.bh_broadphase(sctx.ctx, srad, svel, 0.1, None)
+    pairs = torch.empty((max(count, 1), 2), dtype=torch.int32, device=dev)
+    ms, _ = timed(lambda: bh.bh_broadphase(sctx.ctx, srad, svel, 0.1, pairs))
+    out["broadphase"] = {"workload": f"spheres N={n} mean_contacts=3 speed=0.01 dt=0.1", "ms": ms, "pairs": count,
+                         "bodies_per_s": n / (ms * 1e-3), "pairs_per_s": count / (ms * 1e-3)}
+    label = torch.empty(n, dtype=torch.int32, device=dev)
+    size = torch.empty(n, dtype=torch.int32, device=dev)
+    ms, (comps, aggs) = timed(lambda: bh.bh_aggregates(sctx.ctx, n, pairs[:count], None, label, size, None))
+    out["aggregates"] = {"ms": ms, "edges": count, "edges_per_s": count / (ms * 1e-3), "components": comps,
+                         "aggregates": aggs, "largest": int(size.max().item())}
+    sctx.close()
+    return out
+
+
 # ------------------------------------------------------------------------------------------ own arm
 def run_own(args):
     import numpy as np
@@ -307,6 +371,10 @@ def run_own(args):
         out["e2e"] = {"value": w.n / te, "unit": UNIT, "h2d_bytes_per_step": 32 * w.n, "d2h_bytes_per_step": 24 * w.n,
                       "ms_per_step": te * 1e3, "call": "bh_eval_host (pinned host pos+mass in, acc out)"}
 
+        # ---- rows "next" of SURVEY.md 8(f), timed beside the headline ----
+        if not args.no_next:
+            out["next_rows"] = next_rows(ctx, w, pos0, vel0, mass, dev, hbm_peak)
+
         # ---- the oracle on the host cores, bounded sample ----
         if not args.no_cpu:
             v, desc, cores = oracle_sample(w, args.cpu_budget)
@@ -328,6 +396,7 @@ def main():
     ap.add_argument("--phases", action="store_true", help="read per-phase events after every step")
     ap.add_argument("--full-direct", action="store_true", help="time the direct kernel on all N targets")
     ap.add_argument("--no-cpu", action="store_true", help="skip the oracle leg")
+    ap.add_argument("--no-next", action="store_true", help="skip the timings of the SURVEY 8(f) 'next' rows")
     ap.add_argument("--cpu-budget", type=float, default=15.0, help="seconds of oracle work for cpu_baseline")
     ap.add_argument("--walk-traffic", type=float, default=None,
                     help="dram bytes per walk launch from the committed ncu capture (profiles/)")
