@@ -55,6 +55,7 @@ def lib() -> C.CDLL:
             "bh_get_state_acc": [vp, C.POINTER(vp)],
             "bh_copy_state_acc": [vp, vp],
             "bh_set_gravity_method": [vp, i32],
+            "bh_set_graph": [vp, i32],
             "bh_euler_step": [vp, dbl],
             "bh_multirate_step": [vp, dbl, i32],
             "bh_potential": [vp, dbl, dbl, dbl, vp],
@@ -94,7 +95,7 @@ EXPORTS = ("bh_workspace_bytes", "bh_create", "bh_destroy", "bh_set_stream", "bh
            "bh_get_phase_ms", "bh_measure_fp64_peak", "bh_last_error", "bh_version",
            "bh_euler_step", "bh_multirate_step", "bh_potential", "bh_direct_potential", "bh_diagnostics",
            "bh_position_error", "bh_gravity_dt", "bh_copy_state_acc", "bh_set_gravity_method",
-           "bh_broadphase", "bh_aggregates")
+           "bh_broadphase", "bh_aggregates", "bh_set_graph")
 
 
 def _check(ctx, status: int):
@@ -178,6 +179,10 @@ def bh_copy_state_acc(ctx, acc: torch.Tensor):
 
 def bh_set_gravity_method(ctx, method: int):
     _check(ctx, lib().bh_set_gravity_method(ctx, method))
+
+
+def bh_set_graph(ctx, enable: bool):
+    _check(ctx, lib().bh_set_graph(ctx, int(enable)))
 
 
 def bh_euler_step(ctx, dt: float):

@@ -29,6 +29,24 @@ struct bh_ctx {
     bool timing = false;
     cudaEvent_t ev[BH_NUM_PHASES][2]{};
     bool ev_set[BH_NUM_PHASES]{};
+    // CUDA graph of one stepper call (launch-bound at small N: 19 launches per step)
+    struct StepSig {
+        int kind = -1, n_sub = 0;
+        double dt = 0, theta = 0, eps = 0, G = 0;
+        const void *pos = nullptr, *vel = nullptr, *mass = nullptr;
+        int64_t n = 0;
+        bool direct = false;
+        cudaStream_t stream = nullptr;
+        bool operator==(const StepSig &o) const
+        {
+            return kind == o.kind && n_sub == o.n_sub && dt == o.dt && theta == o.theta && eps == o.eps && G == o.G &&
+                   pos == o.pos && vel == o.vel && mass == o.mass && n == o.n && direct == o.direct && stream == o.stream;
+        }
+    };
+    bool use_graph = false;
+    cudaGraphExec_t graph_exec = nullptr;
+    StepSig graph_sig{}, seen_sig{};
+    uint64_t graph_launches = 0;
     DevState *host_state = nullptr;   // pinned mirror for synchronising getters
     double *host_diag = nullptr;      // pinned, 16 doubles, after host_state
     uint64_t launches = 0;            // kernels launched so far (bench.py's gpu_launches)
@@ -171,6 +189,53 @@ bh_status do_eval_state(bh_ctx *c)
     return cuda_check(c, cudaGetLastError(), "direct evaluation launch");
 }
 
+// Run one stepper call, through a CUDA graph when bh_set_graph is on: the first call with a given
+// signature (stepper, dt, state pointers, parameters) runs plainly, the second is captured while it is
+// enqueued, later ones replay the graph.  All kernel arguments are pointers into the workspace or the
+// bound state and values of the signature, so a replay does exactly what a plain call would.
+template <typename F>
+bh_status run_stepper(bh_ctx *c, int kind, double dt, int n_sub, F enqueue)
+{
+    if (!c->use_graph || c->timing) return enqueue();
+    bh_ctx::StepSig sig;
+    sig.kind = kind; sig.n_sub = n_sub; sig.dt = dt; sig.theta = c->theta; sig.eps = c->eps; sig.G = c->G;
+    sig.pos = c->pos; sig.vel = c->vel; sig.mass = c->mass; sig.n = c->bound_n; sig.direct = c->use_direct;
+    sig.stream = c->stream;
+    if (c->graph_exec && sig == c->graph_sig) {
+        c->launches += c->graph_launches;
+        return cuda_check(c, cudaGraphLaunch(c->graph_exec, c->stream), "stepper graph launch");
+    }
+    if (!(sig == c->seen_sig)) {
+        c->seen_sig = sig;
+        return enqueue();
+    }
+    if (c->graph_exec) {
+        cudaGraphExecDestroy(c->graph_exec);
+        c->graph_exec = nullptr;
+    }
+    const uint64_t l0 = c->launches;
+    if (cudaStreamBeginCapture(c->stream, cudaStreamCaptureModeThreadLocal) != cudaSuccess) {
+        cudaGetLastError();
+        c->use_graph = false;
+        return enqueue();
+    }
+    bh_status st = enqueue();
+    cudaGraph_t g = nullptr;
+    cudaError_t e = cudaStreamEndCapture(c->stream, &g);
+    if (st == BH_OK && e == cudaSuccess && g) e = cudaGraphInstantiate(&c->graph_exec, g, 0);
+    if (g) cudaGraphDestroy(g);
+    if (st != BH_OK || e != cudaSuccess || !c->graph_exec) {   // capture failed: nothing ran; fall back for good
+        cudaGetLastError();
+        c->graph_exec = nullptr;
+        c->use_graph = false;
+        c->launches = l0;
+        return enqueue();
+    }
+    c->graph_sig = sig;
+    c->graph_launches = c->launches - l0;
+    return cuda_check(c, cudaGraphLaunch(c->graph_exec, c->stream), "stepper graph launch");
+}
+
 }  // namespace
 
 namespace bh {
@@ -296,6 +361,7 @@ bh_status bh_destroy(bh_ctx *c)
         if (c->ev[p][0]) cudaEventDestroy(c->ev[p][0]);
         if (c->ev[p][1]) cudaEventDestroy(c->ev[p][1]);
     }
+    if (c->graph_exec) cudaGraphExecDestroy(c->graph_exec);
     if (c->host_state) cudaFreeHost(c->host_state);
     delete c;
     return BH_OK;
@@ -372,10 +438,30 @@ bh_status bh_bind_state(bh_ctx *c, double *pos_dev, double *vel_dev, const doubl
     return BH_OK;
 }
 
+bh_status bh_set_graph(bh_ctx *c, int enable)
+{
+    if (!c) return BH_ERR_INVALID_ARG;
+    c->use_graph = enable != 0;
+    if (!c->use_graph && c->graph_exec) {
+        cudaGraphExecDestroy(c->graph_exec);
+        c->graph_exec = nullptr;
+    }
+    c->seen_sig = bh_ctx::StepSig{};
+    return BH_OK;
+}
+
+static bh_status kdk_enqueue(bh_ctx *c, double dt);
+
 bh_status bh_kdk_step(bh_ctx *c, double dt)
 {
     if (!c) return BH_ERR_INVALID_ARG;
     if (!c->bound) return fail(c, BH_ERR_STATE, "bh_kdk_step before bh_bind_state");
+    if (!c->have_acc) return kdk_enqueue(c, dt);   // the first step also evaluates a(x0): not the repeating pattern
+    return run_stepper(c, 0, dt, 0, [=]() { return kdk_enqueue(c, dt); });
+}
+
+static bh_status kdk_enqueue(bh_ctx *c, double dt)
+{
     bh_status st;
     if (!c->have_acc) {   // a(x0), once
         if ((st = do_eval_state(c)) != BH_OK) return st;
@@ -395,11 +481,22 @@ bh_status bh_kdk_step(bh_ctx *c, double dt)
 }
 
 /* ---- rows "next": paper's stepping variants and conservation diagnostics ---- */
+static bh_status euler_enqueue(bh_ctx *c, double dt, int n_sub, const char *who);
+
 static bh_status euler_like(bh_ctx *c, double dt, int n_sub, const char *who)
 {
     if (!c) return BH_ERR_INVALID_ARG;
     if (!c->bound) return fail(c, BH_ERR_STATE, "stepper called before bh_bind_state");
     if (n_sub < 1) return fail(c, BH_ERR_INVALID_ARG, "n_sub < 1");
+    bh_status st = run_stepper(c, 1, dt, n_sub, [=]() { return euler_enqueue(c, dt, n_sub, who); });
+    c->have_acc = false;   // whatever path ran: acc is a(x_k)
+    c->acc_filled = true;
+    if (!c->use_direct) { c->built = true; c->walked = true; c->n = c->bound_n; }
+    return st;
+}
+
+static bh_status euler_enqueue(bh_ctx *c, double dt, int n_sub, const char *who)
+{
     bh_status st;
     if ((st = do_eval_state(c)) != BH_OK) return st;
     c->have_acc = false;   // acc is a(x_k), not a(x_k+1): a later bh_kdk_step re-evaluates

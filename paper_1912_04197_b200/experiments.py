@@ -38,8 +38,8 @@ def cube_cloud(n: int, seed: int, half: float = 1.0) -> np.ndarray:
 
 
 def _time_steps(ctx, steps: int, dt: float) -> float:
-    bh.bh_euler_step(ctx.ctx, dt)   # warm-up
-    bh.bh_euler_step(ctx.ctx, dt)
+    for _ in range(3):               # warm-up (with bh_set_graph: plain, capture, replay)
+        bh.bh_euler_step(ctx.ctx, dt)
     torch.cuda.synchronize()
     a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     a.record()
@@ -51,7 +51,7 @@ def _time_steps(ctx, steps: int, dt: float) -> float:
     return a.elapsed_time(b) / steps
 
 
-def fig4(ns=None, leaf_cap: int = 16):
+def fig4(ns=None, leaf_cap: int = 16, graph: bool = False):
     ns = ns or [10, 30, 100, 300, 700, 1000, 2000, 3000, 5000, 10000, 30000, 100000, 300000, 1000000]
     dev = torch.device("cuda:0")
     print("| N | direct N^2 ms/step | " + " | ".join(f"BH theta={t:g} ms/step" for t in THETAS) + " | fastest |")
@@ -67,6 +67,7 @@ def fig4(ns=None, leaf_cap: int = 16):
             vel = torch.zeros_like(pos)
             bh.bh_bind_state(ctx.ctx, pos, vel, mass, theta, 1e-3, 1.0)
             bh.bh_set_gravity_method(ctx.ctx, method)
+            bh.bh_set_graph(ctx.ctx, graph)
             steps = 50 if n <= 100000 else (10 if method == 0 else 2)
             times.append(_time_steps(ctx, steps, 1e-6))
         ctx.close()
@@ -138,8 +139,8 @@ def fig5(n: int = 1000, eps: float = 0.05, leaf_cap: int = 16, steps: int = 3000
 
 if __name__ == "__main__":
     which = sys.argv[1] if len(sys.argv) > 1 else "fig4"
-    if which == "fig4":
-        fig4([int(x) for x in sys.argv[2:]] or None)
+    if which in ("fig4", "fig4-graph"):     # fig4-graph: the steps replayed through a CUDA graph (bh_set_graph)
+        fig4([int(x) for x in sys.argv[2:]] or None, graph=which == "fig4-graph")
     elif which == "fig5":
         fig5()
     else:

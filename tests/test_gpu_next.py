@@ -227,3 +227,32 @@ def test_steppers_with_direct_gravity():
     bh.bh_synchronize(ctx.ctx)
     assert bh.bh_get_node_count(ctx.ctx)[0] > 1
     ctx.close()
+
+
+@pytest.mark.parametrize("n,method", [(3000, 0), (500, 1), (40000, 0)])
+def test_cuda_graph_steppers_bit_identical(n, method):
+    """bh_set_graph: captured / replayed steps equal plain steps bit for bit, across steppers and dt changes."""
+    w = wl.make("c4", n)
+    outs = []
+    for graph in (False, True):
+        ctx = bh.Context(n, 16)
+        pos, vel, mass = dev(w.pos), dev(w.vel), dev(w.mass)
+        bh.bh_bind_state(ctx.ctx, pos, vel, mass, w.theta, w.eps, w.G)
+        bh.bh_set_gravity_method(ctx.ctx, method)
+        bh.bh_set_graph(ctx.ctx, graph)
+        l0 = bh.bh_get_launches(ctx.ctx)
+        for _ in range(6):
+            bh.bh_kdk_step(ctx.ctx, 1e-3)
+        for _ in range(4):
+            bh.bh_euler_step(ctx.ctx, 5e-4)
+        for _ in range(3):
+            bh.bh_multirate_step(ctx.ctx, 1e-4, 4)
+        for _ in range(3):
+            bh.bh_kdk_step(ctx.ctx, 2e-3)       # new dt: plain, capture, replay
+        bh.bh_synchronize(ctx.ctx)
+        outs.append((pos.cpu().numpy(), vel.cpu().numpy(), bh.bh_get_launches(ctx.ctx) - l0))
+        if method == 0:
+            assert bh.bh_get_node_count(ctx.ctx)[0] > 1
+        ctx.close()
+    assert np.array_equal(outs[0][0], outs[1][0]) and np.array_equal(outs[0][1], outs[1][1])
+    assert outs[0][2] == outs[1][2]             # the launch count is the same claim on both paths
