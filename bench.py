@@ -369,7 +369,8 @@ def run_own(args):
             bh.bh_eval_host(ctx.ctx, ph, mh, w.theta, w.eps, w.G, ah)   # synchronising call
         te = (time.perf_counter() - t0) / ke
         out["e2e"] = {"value": w.n / te, "unit": UNIT, "h2d_bytes_per_step": 32 * w.n, "d2h_bytes_per_step": 24 * w.n,
-                      "ms_per_step": te * 1e3, "call": "bh_eval_host (pinned host pos+mass in, acc out)"}
+                      "ms_per_step": te * 1e3, "call": "bh_eval_host (pinned host pos+mass in, acc out; mass upload beside the first build kernels, "
+                              "accelerations stored by the walk kernel straight into the pinned output)"}
 
         # ---- rows "next" of SURVEY.md 8(f), timed beside the headline ----
         if not args.no_next:

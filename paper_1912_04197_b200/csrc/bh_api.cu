@@ -1,6 +1,7 @@
 // bh_api.cu — the C ABI declared in include/bh.h: context, workspace carving, call sequencing.
 #include <cmath>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 
@@ -43,6 +44,9 @@ struct bh_ctx {
                    pos == o.pos && vel == o.vel && mass == o.mass && n == o.n && direct == o.direct && stream == o.stream;
         }
     };
+    cudaStream_t copy_stream = nullptr;   // bh_eval_host: mass upload beside the first build kernels
+    cudaEvent_t ev_copy[2]{};
+    bool host_direct = true;              // bh_eval_host: store accelerations straight into pinned host memory
     bool use_graph = false;
     cudaGraphExec_t graph_exec = nullptr;
     StepSig graph_sig{}, seen_sig{};
@@ -112,7 +116,7 @@ bh_status fetch_state(bh_ctx *c)   // synchronising
     return BH_OK;
 }
 
-bh_status do_build(bh_ctx *c, const double *pos, const double *mass, int64_t n)
+bh_status do_build(bh_ctx *c, const double *pos, const double *mass, int64_t n, cudaEvent_t mass_ready = nullptr)
 {
     const Workspace &w = c->ws;
     cudaStream_t s = c->stream;
@@ -133,6 +137,7 @@ bh_status do_build(bh_ctx *c, const double *pos, const double *mass, int64_t n)
     }
     {
         Phase p(c, 3);
+        if (mass_ready) cudaStreamWaitEvent(s, mass_ready, 0);   // masses copied on another stream
         launch_gather(w, pos, mass, n, s);
     }
     {
@@ -335,10 +340,13 @@ bh_status bh_create(bh_ctx **out, int64_t max_n, int leaf_cap, int group_size, v
     c->leaf_cap = leaf_cap;
     c->stream = (cudaStream_t)cuda_stream;
     c->ws = w;
+    if (const char *hd = getenv("BH_HOST_DIRECT")) c->host_direct = hd[0] != '0';   // A/B switch for measurements
     const size_t hs = (sizeof(DevState) + 63) & ~(size_t)63;
     cudaError_t e = cudaMallocHost((void **)&c->host_state, hs + 16 * sizeof(double));
     if (e == cudaSuccess) c->host_diag = reinterpret_cast<double *>(reinterpret_cast<char *>(c->host_state) + hs);
     if (e == cudaSuccess) e = cudaMemsetAsync(w.st, 0, sizeof(DevState), c->stream);
+    if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&c->copy_stream, cudaStreamNonBlocking);
+    for (int k = 0; k < 2 && e == cudaSuccess; ++k) e = cudaEventCreateWithFlags(&c->ev_copy[k], cudaEventDisableTiming);
     for (int p = 0; p < BH_NUM_PHASES && e == cudaSuccess; ++p) {
         e = cudaEventCreate(&c->ev[p][0]);
         if (e == cudaSuccess) e = cudaEventCreate(&c->ev[p][1]);
@@ -346,6 +354,9 @@ bh_status bh_create(bh_ctx **out, int64_t max_n, int leaf_cap, int group_size, v
     if (e != cudaSuccess) {
         snprintf(g_err, 256, "bh_create: %s", cudaGetErrorString(e));
         if (c->host_state) cudaFreeHost(c->host_state);
+        if (c->copy_stream) cudaStreamDestroy(c->copy_stream);
+        for (int k = 0; k < 2; ++k)
+            if (c->ev_copy[k]) cudaEventDestroy(c->ev_copy[k]);
         delete c;
         return BH_ERR_CUDA;
     }
@@ -362,6 +373,12 @@ bh_status bh_destroy(bh_ctx *c)
         if (c->ev[p][1]) cudaEventDestroy(c->ev[p][1]);
     }
     if (c->graph_exec) cudaGraphExecDestroy(c->graph_exec);
+    if (c->copy_stream) {
+        cudaStreamSynchronize(c->copy_stream);
+        cudaStreamDestroy(c->copy_stream);
+    }
+    for (int k = 0; k < 2; ++k)
+        if (c->ev_copy[k]) cudaEventDestroy(c->ev_copy[k]);
     if (c->host_state) cudaFreeHost(c->host_state);
     delete c;
     return BH_OK;
@@ -639,6 +656,17 @@ bh_status bh_copy_state_acc(bh_ctx *c, double *acc_dev)
                                          c->stream), "bh_copy_state_acc");
 }
 
+// device alias of a pinned (page-locked, mapped) host buffer, or nullptr for pageable memory
+static double *mapped_alias(const void *host)
+{
+    cudaPointerAttributes a{};
+    if (cudaPointerGetAttributes(&a, host) != cudaSuccess) {
+        cudaGetLastError();
+        return nullptr;
+    }
+    return a.type == cudaMemoryTypeHost ? static_cast<double *>(a.devicePointer) : nullptr;
+}
+
 bh_status bh_eval_host(bh_ctx *c, const double *pos_host, const double *mass_host, int64_t n, double theta,
                        double eps, double G, double *acc_host)
 {
@@ -647,17 +675,29 @@ bh_status bh_eval_host(bh_ctx *c, const double *pos_host, const double *mass_hos
     if (n < 1 || n > c->max_n) return fail(c, BH_ERR_INVALID_ARG, "bh_eval_host: n out of range");
     if (!(theta >= 0.0) || !(eps >= 0.0)) return fail(c, BH_ERR_INVALID_ARG, "bh_eval_host: theta or eps negative");
     const Workspace &w = c->ws;
+    // The masses are first needed by the gather (after the sort): their copy runs on a second stream,
+    // beside cube / keys / sort.  It may start once the previous user of the staging buffer is done.
+    // It starts after the positions have arrived (one transfer at a time gets the whole link) and after
+    // the previous user of the staging buffer (stream order of the main stream up to the event).
     cudaError_t e = cudaMemcpyAsync(w.stage_pos, pos_host, 3 * n * sizeof(double), cudaMemcpyHostToDevice, c->stream);
+    if (e == cudaSuccess) e = cudaEventRecord(c->ev_copy[0], c->stream);
+    if (e == cudaSuccess) e = cudaStreamWaitEvent(c->copy_stream, c->ev_copy[0], 0);
     if (e == cudaSuccess)
-        e = cudaMemcpyAsync(w.stage_mass, mass_host, n * sizeof(double), cudaMemcpyHostToDevice, c->stream);
+        e = cudaMemcpyAsync(w.stage_mass, mass_host, n * sizeof(double), cudaMemcpyHostToDevice, c->copy_stream);
+    if (e == cudaSuccess) e = cudaEventRecord(c->ev_copy[1], c->copy_stream);
     if (e != cudaSuccess) return cuda_check(c, e, "bh_eval_host H2D");
     bh_status st;
-    if ((st = do_build(c, w.stage_pos, w.stage_mass, n)) != BH_OK) return st;
-    if ((st = do_accel(c, theta, eps, G, w.acc)) != BH_OK) return st;
+    if ((st = do_build(c, w.stage_pos, w.stage_mass, n, c->ev_copy[1])) != BH_OK) return st;
+    // Pinned output: the walk stores the accelerations straight into host memory (24 bytes per body,
+    // over PCIe while the kernel computes), so no copy follows it.  Pageable output: staged in the workspace.
+    double *direct_out = c->host_direct ? mapped_alias(acc_host) : nullptr;
+    if ((st = do_accel(c, theta, eps, G, direct_out ? direct_out : w.acc)) != BH_OK) return st;
     c->have_acc = false;   // the internal acc buffer no longer belongs to the bound state
     c->acc_filled = false;
-    e = cudaMemcpyAsync(acc_host, w.acc, 3 * n * sizeof(double), cudaMemcpyDeviceToHost, c->stream);
-    if (e != cudaSuccess) return cuda_check(c, e, "bh_eval_host D2H");
+    if (!direct_out) {
+        e = cudaMemcpyAsync(acc_host, w.acc, 3 * n * sizeof(double), cudaMemcpyDeviceToHost, c->stream);
+        if (e != cudaSuccess) return cuda_check(c, e, "bh_eval_host D2H");
+    }
     return fetch_state(c);
 }
 

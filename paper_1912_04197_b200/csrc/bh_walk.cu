@@ -34,6 +34,9 @@ constexpr int kStack = 512;                 // sibling ranges per producer in sh
 constexpr int kSpill = 128;                 // spill / refill unit
 constexpr int kDesc = 4;                    // group descriptors in flight per pair
 constexpr unsigned kNoGroup = 0xffffffffu;
+#ifndef BH_SEED_LOWWORD
+#define BH_SEED_LOWWORD 1                   // rsqrt seed: low word taken from a dead register pair (see interact)
+#endif
 #ifndef BH_SLEEP_FULL
 #define BH_SLEEP_FULL 1000                  // ns a producer sleeps per poll while its ring is full
 #endif
@@ -61,9 +64,20 @@ __device__ __forceinline__ void interact(double px, double py, double pz, double
                                          double &ax, double &ay, double &az)
 {
     const double dx = s.x - px, dy = s.y - py, dz = s.z - pz;
-    const double r2 = fma(dx, dx, fma(dy, dy, fma(dz, dz, eps2)));
+    const double t2 = fma(dy, dy, fma(dz, dz, eps2));
+    const double r2 = fma(dx, dx, t2);
     double y;
+#if BH_SEED_LOWWORD
+    // the seed's low word is irrelevant (the series below corrects any y within 2^-19 of r2^-1/2): take it
+    // from the dead partial sum, so that MUFU.RSQ64H can write into that register pair without a zero-fill
+    {
+        double y0;
+        asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y0) : "d"(r2));
+        y = __hiloint2double(__double2hiint(y0), __double2loint(t2));
+    }
+#else
     asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(r2));
+#endif
     if (GUARD) y = (r2 > 0.0) ? y : 0.0;      // a pair at zero softened distance adds nothing (R13)
     const double u = y * y;
     const double w = s.w * y;
