@@ -261,3 +261,43 @@ def test_full_size_headline_config():
     net = (w.mass[:, None] * a).sum(axis=0)
     assert np.linalg.norm(net) < 1e-3 * (w.mass * np.linalg.norm(a, axis=1)).sum()
     ctx.close()
+
+
+def test_eval_host_pageable_output_is_staged():
+    """bh_eval_host with ordinary (pageable) host memory takes the staged path; with pinned memory the walk
+    stores straight into the output.  Both must give the same accelerations bit for bit."""
+    w = wl.make("c4", 20000)
+    ctx = bh.Context(w.n, 16)
+    pos_h, mass_h = torch.as_tensor(w.pos), torch.as_tensor(w.mass)
+    out_page = torch.empty((w.n, 3), dtype=torch.float64)
+    out_pin = torch.empty((w.n, 3), dtype=torch.float64).pin_memory()
+    bh.bh_eval_host(ctx.ctx, pos_h, mass_h, w.theta, w.eps, w.G, out_page)
+    bh.bh_eval_host(ctx.ctx, pos_h.pin_memory(), mass_h.pin_memory(), w.theta, w.eps, w.G, out_pin)
+    assert np.array_equal(out_page.numpy(), out_pin.numpy())
+    ref = orc.accel(orc.build(w.pos, w.mass, 16), w.theta, w.eps, w.G)[0]
+    assert relerr(out_pin.numpy(), ref).max() <= TOL
+    ctx.close()
+
+
+def test_full_size_largest_config():
+    """configs[4] at its full size (N = 4 194 304 rotating ball, C = 32, theta = 0.6): tree bit-exact, sampled
+    groups against the oracle's walk, and the config's own check — the direct sum on random targets."""
+    w = wl.make("c5")
+    t = orc.build(w.pos, w.mass, w.leaf_cap)
+    ctx = gpu_build(w.pos, w.mass, w.leaf_cap)
+    assert_tree_equal(ctx, t)
+    a = ctx.accel(w.theta, w.eps, w.G).cpu().numpy()
+    gm, gd = (x.cpu().numpy().view(np.uint32) for x in ctx.counts())
+    ng = t.ngroups
+    for g0 in list(range(0, ng, ng // 12))[:12] + [ng - 2]:
+        ref, nm, nd, _ = orc.accel(t, w.theta, w.eps, w.G, g0, g0 + 2)
+        rows = t.perm[t.gstart[g0]:t.gstart[g0 + 2]]
+        assert np.array_equal(gm[g0:g0 + 2], nm) and np.array_equal(gd[g0:g0 + 2], nd)
+        assert relerr(a[rows], ref[rows]).max() <= TOL
+    tg = np.random.default_rng(5).choice(w.n, size=128, replace=False).astype(np.int32)
+    b = ctx.direct(w.eps, w.G, targets=dev(tg, torch.int32)).cpu().numpy()
+    refd = orc.direct(w.pos, w.mass, w.eps, w.G, targets=tg)
+    assert relerr(b, refd).max() <= TOL
+    # tree against direct on those targets: the size of the Barnes-Hut error at theta = 0.6 (BASELINE.md: median 7.5e-3)
+    assert np.median(relerr(a[tg], refd)) < 3e-2
+    ctx.close()
