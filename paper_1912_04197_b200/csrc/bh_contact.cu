@@ -94,7 +94,7 @@ __global__ void __launch_bounds__(256) node_box_kernel(const DevState *__restric
 }
 
 constexpr int kBpWarps = 4;
-constexpr int kBpStack = 2048;   // node ids per warp
+constexpr int kBpStack = 1024;   // node ids per warp (a local search holds a few dozen)
 constexpr int kBpLeafQ = 96;     // surviving leaves waiting for their body tests
 
 __device__ __forceinline__ double gap(double alo, double ahi, double blo, double bhi)
@@ -304,7 +304,7 @@ int launch_broadphase(const Workspace &w, int64_t n, const double *radius, const
     const int64_t want = (w.node_cap + 255) / 256;
     node_box_kernel<<<(int)(want < 148 * 16 ? want : 148 * 16), 256, 0, s>>>(w.st, w.sbody, w.bsort, w.winfo, w.nparent,
                                                                              w.bp_cnt, w.box_lo, w.box_hi, w.node_cap);
-    broadphase_kernel<<<148 * 8, kBpWarps * 32, 0, s>>>(w.st, w.gstart, w.sbody, w.bsort, w.gbox, w.winfo, w.box_lo,
+    broadphase_kernel<<<148 * 16, kBpWarps * 32, 0, s>>>(w.st, w.gstart, w.sbody, w.bsort, w.gbox, w.winfo, w.box_lo,
                                                         w.box_hi, w.idx[0], reinterpret_cast<int2 *>(pairs),
                                                         (unsigned long long)cap);
     return 3;

@@ -301,3 +301,33 @@ def test_full_size_largest_config():
     # tree against direct on those targets: the size of the Barnes-Hut error at theta = 0.6 (median 7.5e-3)
     assert np.median(relerr(a[tg], refd)) < 3e-2
     ctx.close()
+
+
+def test_headline_config_after_ten_kdk_steps():
+    """configs[3] as BASELINE.json states it: 10 leapfrog steps at N = 1M with a rebuild every step.  Compared
+    per evaluation on bit-identical inputs: the GPU's positions after step 10 go to the
+    oracle; its tree must equal the GPU's last build bit for bit and its accelerations on sampled groups
+    must match the accelerations the GPU's last step used."""
+    w = wl.make("c4")
+    pos, vel, mass = dev(w.pos), dev(w.vel), dev(w.mass)
+    ctx = bh.Context(w.n, w.leaf_cap)
+    bh.bh_bind_state(ctx.ctx, pos, vel, mass, w.theta, w.eps, w.G)
+    for _ in range(w.steps):
+        bh.bh_kdk_step(ctx.ctx, w.dt)
+    bh.bh_synchronize(ctx.ctx)
+    p = pos.cpu().numpy()
+    assert np.isfinite(p).all() and np.abs(p - w.pos).max() > 0
+    t = orc.build(p, w.mass, w.leaf_cap)
+    ctx.n = w.n
+    assert_tree_equal(ctx, t)                      # the tree of the last step's rebuild
+    a = torch.empty((w.n, 3), dtype=torch.float64, device="cuda")
+    bh.bh_copy_state_acc(ctx.ctx, a)
+    a = a.cpu().numpy()
+    ng = t.ngroups
+    for g0 in list(range(0, ng, ng // 8))[:8]:
+        ref = orc.accel(t, w.theta, w.eps, w.G, g0, g0 + 2)[0]
+        rows = t.perm[t.gstart[g0]:t.gstart[g0 + 2]]
+        assert relerr(a[rows], ref[rows]).max() <= TOL
+    # the cloud is in equilibrium: ten steps of dt = 1e-3 move bodies by about |v| * 0.01
+    assert np.abs(p - w.pos).max() < 0.05
+    ctx.close()
