@@ -122,6 +122,7 @@ bh_status do_build(bh_ctx *c, const double *pos, const double *mass, int64_t n, 
     cudaStream_t s = c->stream;
     c->built = false;
     c->walked = false;
+    int sort_launches = 0;
     cudaMemsetAsync(w.zero_begin, 0, w.zero_bytes, s);
     {
         Phase p(c, 0);
@@ -133,7 +134,7 @@ bh_status do_build(bh_ctx *c, const double *pos, const double *mass, int64_t n, 
     }
     {
         Phase p(c, 2);
-        launch_sort(w, n, s);
+        sort_launches = launch_sort(w, n, s);
     }
     {
         Phase p(c, 3);
@@ -152,7 +153,7 @@ bh_status do_build(bh_ctx *c, const double *pos, const double *mass, int64_t n, 
     if (st != BH_OK) return st;
     c->n = n;
     c->built = true;
-    c->launches += 2 + kSortPasses + 1 + 4 + 1;   // cube, keys, sort passes, gather, tree (3) + boxes, monopoles
+    c->launches += 2 + sort_launches + 1 + 4 + 1;   // cube, keys, sort passes, gather, tree (3) + boxes, monopoles
     return BH_OK;
 }
 

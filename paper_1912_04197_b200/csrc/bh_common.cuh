@@ -106,7 +106,7 @@ Workspace carve(char *base, int64_t max_n, int leaf_cap);
 // launchers (each enqueues on `s`)
 void launch_cube(const Workspace &w, const double *pos, int64_t n, cudaStream_t s);
 void launch_keys(const Workspace &w, const double *pos, int64_t n, cudaStream_t s);
-void launch_sort(const Workspace &w, int64_t n, cudaStream_t s);   // result in key[0]/idx[0]
+int launch_sort(const Workspace &w, int64_t n, cudaStream_t s);   // result in key[0]/idx[0]; returns the launches
 void launch_gather(const Workspace &w, const double *pos, const double *mass, int64_t n, cudaStream_t s);
 // (x,y,z,m) in the caller's body order with the identity permutation: input of a direct sum without a tree
 void launch_pack(const Workspace &w, const double *pos, const double *mass, int64_t n, cudaStream_t s);

@@ -44,19 +44,21 @@ __global__ void __launch_bounds__(kCubeThreads) cube_kernel(const double *__rest
     smx[tid] = mx;
     sbad[tid] = bad;
     __syncthreads();
-    if (tid < 3) {
-        for (int k = tid + 3; k < kCubeThreads; k += 3) {
-            mn = fmin(mn, smn[k]);
-            mx = fmax(mx, smx[k]);
+    // tree over strides that are multiples of 3, so that a thread only ever meets its own axis
+#pragma unroll
+    for (int h = kCubeThreads / 2; h >= 3; h >>= 1) {
+        if (tid < h) {
+            smn[tid] = fmin(smn[tid], smn[tid + h]);
+            smx[tid] = fmax(smx[tid], smx[tid + h]);
+            sbad[tid] |= sbad[tid + h];
         }
-        part[blockIdx.x * 8 + tid] = mn;
-        part[blockIdx.x * 8 + 3 + tid] = mx;
+        __syncthreads();
     }
-    if (tid == 0) {
-        int b = 0;
-        for (int k = 0; k < kCubeThreads; ++k) b |= sbad[k];
-        part[blockIdx.x * 8 + 6] = b ? 1.0 : 0.0;
+    if (tid < 3) {
+        part[blockIdx.x * 8 + tid] = smn[tid];
+        part[blockIdx.x * 8 + 3 + tid] = smx[tid];
     }
+    if (tid == 0) part[blockIdx.x * 8 + 6] = (sbad[0] | sbad[1] | sbad[2]) ? 1.0 : 0.0;
     __threadfence();
     __syncthreads();
     if (tid == 0) is_last = (atomicAdd(&st->ticket_bbox, 1u) == gridDim.x - 1);
@@ -77,17 +79,22 @@ __global__ void __launch_bounds__(kCubeThreads) cube_kernel(const double *__rest
     smx[tid] = mx;
     sbad[tid] = bad;
     __syncthreads();
+#pragma unroll
+    for (int h = kCubeThreads / 2; h >= 3; h >>= 1) {
+        if (tid < h) {
+            smn[tid] = fmin(smn[tid], smn[tid + h]);
+            smx[tid] = fmax(smx[tid], smx[tid + h]);
+            sbad[tid] |= sbad[tid + h];
+        }
+        __syncthreads();
+    }
     if (tid == 0) {
         double lo[3], hi[3];
         for (int a = 0; a < 3; ++a) {
             lo[a] = smn[a];
             hi[a] = smx[a];
         }
-        for (int k = 3; k < kCubeThreads; ++k) {
-            lo[k % 3] = fmin(lo[k % 3], smn[k]);
-            hi[k % 3] = fmax(hi[k % 3], smx[k]);
-        }
-        for (int k = 0; k < kCubeThreads; ++k) bad |= sbad[k];
+        bad = sbad[0] | sbad[1] | sbad[2];
         double E = 0.0;
         for (int a = 0; a < 3; ++a) E = fmax(E, __dsub_rn(hi[a], lo[a]));   // one rounding per extent
         if (nonfinite(E)) bad = 1;
@@ -163,7 +170,7 @@ __global__ void __launch_bounds__(256) keys_kernel(const double *__restrict__ po
 void launch_cube(const Workspace &w, const double *pos, int64_t n, cudaStream_t s)
 {
     long long n3 = 3 * (long long)n;
-    int blocks = (int)((n3 + kCubeThreads * 8 - 1) / (kCubeThreads * 8));
+    int blocks = (int)((n3 + kCubeThreads * 4 - 1) / (kCubeThreads * 4));   // four loads per thread, all in flight
     if (blocks > kCubeMaxBlocks) blocks = kCubeMaxBlocks;
     if (blocks < 1) blocks = 1;
     cube_kernel<<<blocks, kCubeThreads, 0, s>>>(pos, n3, w.st, w.bbox_part);
