@@ -37,8 +37,8 @@ UNIT = "body-accelerations/s"
 FLOPS_PER_INTERACTION = 20.0
 FP64_PEAK_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12      # derived: SMs x fp64 FMA lanes x 2 x max SM clock
 # dram__bytes_read.sum + dram__bytes_write.sum of one walk_kernel launch, from the committed ncu --set full
-# capture (profiles/r01_walk_ncu_full.md: 65.30 MB + 15.64 MB); a profiler figure, not measured by this run
-WALK_TRAFFIC_NCU = {"c4": 80.94e6}
+# capture (profiles/r01_walk_ncu_full.md: 65.32 MB + 15.84 MB); a profiler figure, not measured by this run
+WALK_TRAFFIC_NCU = {"c4": 81.15e6}
 
 
 def workload_desc(w):
