@@ -152,3 +152,33 @@ def test_broadphase_then_aggregates(mc):
     assert np.array_equal(label.cpu().numpy(), ref["label"]) and np.array_equal(size.cpu().numpy(), ref["size"])
     assert (comps, aggs) == (ref["components"], ref["aggregates"])
     ctx.close()
+
+
+def test_degenerate_clouds_next_rows():
+    """More coincident bodies than a leaf or a walk group holds (depth cap, R9): the potential counts every
+    coincident neighbour (m/eps each) but never the body itself; the broad phase reports all their pairs."""
+    rng = np.random.default_rng(12)
+    pos = np.concatenate([np.full((70, 3), 0.25), rng.random((50, 3))])
+    mass = rng.random(120) + 0.5
+    radius = np.full(120, 1e-3)
+    ctx = bh.Context(120, 4)
+    ctx.build(dev(pos), dev(mass))
+    t = orc.build(pos, mass, 4)
+    for eps in (1e-2, 0.0):
+        ref = orc.potential(t, 0.5, eps, 1.0)
+        phi = ctx.potential(0.5, eps, 1.0).cpu().numpy()
+        assert np.abs((phi - ref) / ref).max() <= 1e-11
+        refd = orc.direct_potential(pos, mass, eps, 1.0)
+        phid = ctx.direct_potential(eps, 1.0).cpu().numpy()
+        assert np.abs((phid - refd) / refd).max() <= 1e-11
+    ref = orc.broadphase(pos, radius)
+    assert len(ref) >= 70 * 69 // 2
+    cnt = bh.bh_broadphase(ctx.ctx, dev(radius), None, 0.0, None)
+    buf = torch.empty((cnt, 2), dtype=torch.int32, device="cuda")
+    bh.bh_broadphase(ctx.ctx, dev(radius), None, 0.0, buf)
+    assert np.array_equal(sorted_pairs(buf.cpu().numpy()), ref)
+    label = torch.empty(120, dtype=torch.int32, device="cuda")
+    comps, aggs = bh.bh_aggregates(ctx.ctx, 120, buf, None, label)
+    r = orc.aggregates(120, ref)
+    assert (comps, aggs) == (r["components"], r["aggregates"]) and np.array_equal(label.cpu().numpy(), r["label"])
+    ctx.close()
