@@ -198,6 +198,11 @@ def next_rows(ctx, w, pos, vel, mass, dev, hbm_peak):
     inter = bh.bh_get_stats(ctx.ctx)["interactions"]
     out["potential_walk"] = {"ms": ms, "interactions_per_s": inter / (ms * 1e-3),
                              "fp64_instr_per_interaction": 12}
+    acc2 = torch.empty((n, 3), dtype=torch.float64, device=dev)
+    bh.bh_accel_potential(ctx.ctx, w.theta, w.eps, w.G, acc2, phi)
+    ms, _ = timed(lambda: bh.bh_accel_potential(ctx.ctx, w.theta, w.eps, w.G, acc2, phi))
+    out["accel_and_potential_walk"] = {"ms": ms, "interactions_per_s": inter / (ms * 1e-3),
+                                       "fp64_instr_per_interaction": 19}
     ms, d = timed(lambda: bh.bh_diagnostics(ctx.ctx, pos, vel, mass, phi))
     out["diagnostics"] = {"ms": ms, "GB_per_s": 64.0 * n / (ms * 1e-3) / 1e9, "frac_of_hbm_peak": 64.0 * n / (ms * 1e-3) / 1e9 / hbm_peak,
                           "bytes_per_body": 64, "virial_2K_over_W": -2.0 * d["ekin"] / d["epot"]}

@@ -60,6 +60,7 @@ def lib() -> C.CDLL:
             "bh_multirate_step": [vp, dbl, i32],
             "bh_potential": [vp, dbl, dbl, dbl, vp],
             "bh_direct_potential": [vp, dbl, dbl, vp],
+            "bh_accel_potential": [vp, dbl, dbl, dbl, vp, vp],
             "bh_diagnostics": [vp, vp, vp, vp, vp, i64, C.POINTER(dbl)],
             "bh_position_error": [vp, vp, vp, i64, C.POINTER(dbl)],
             "bh_broadphase": [vp, vp, vp, dbl, vp, i64, C.POINTER(i64)],
@@ -95,7 +96,7 @@ EXPORTS = ("bh_workspace_bytes", "bh_create", "bh_destroy", "bh_set_stream", "bh
            "bh_get_phase_ms", "bh_measure_fp64_peak", "bh_last_error", "bh_version",
            "bh_euler_step", "bh_multirate_step", "bh_potential", "bh_direct_potential", "bh_diagnostics",
            "bh_position_error", "bh_gravity_dt", "bh_copy_state_acc", "bh_set_gravity_method",
-           "bh_broadphase", "bh_aggregates", "bh_set_graph")
+           "bh_broadphase", "bh_aggregates", "bh_set_graph", "bh_accel_potential")
 
 
 def _check(ctx, status: int):
@@ -195,6 +196,10 @@ def bh_multirate_step(ctx, dt_c: float, n_sub: int):
 
 def bh_potential(ctx, theta: float, eps: float, G: float, phi: torch.Tensor):
     _check(ctx, lib().bh_potential(ctx, theta, eps, G, _dev(phi, torch.float64, "phi")))
+
+
+def bh_accel_potential(ctx, theta: float, eps: float, G: float, acc: torch.Tensor, phi: torch.Tensor):
+    _check(ctx, lib().bh_accel_potential(ctx, theta, eps, G, _dev(acc, torch.float64, "acc"), _dev(phi, torch.float64, "phi")))
 
 
 def bh_direct_potential(ctx, eps: float, G: float, phi: torch.Tensor):

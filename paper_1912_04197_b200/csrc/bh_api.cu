@@ -157,7 +157,7 @@ bh_status do_build(bh_ctx *c, const double *pos, const double *mass, int64_t n, 
     return BH_OK;
 }
 
-bh_status do_accel(bh_ctx *c, double theta, double eps, double G, double *acc, bool potential = false)
+bh_status do_accel(bh_ctx *c, double theta, double eps, double G, double *acc, int mode = 0, double *phi = nullptr)
 {
     const Workspace &w = c->ws;
     // reset the group queue and the counters of this evaluation
@@ -165,7 +165,7 @@ bh_status do_accel(bh_ctx *c, double theta, double eps, double G, double *acc, b
     cudaMemsetAsync(&w.st->stats[0], 0, 4 * sizeof(unsigned long long), c->stream);
     {
         Phase p(c, 6);
-        launch_walk(w, c->n, theta, eps, G, acc, potential, c->stream);
+        launch_walk(w, c->n, theta, eps, G, acc, mode, phi, c->stream);
     }
     bh_status st = cuda_check(c, cudaGetLastError(), "bh_accel launch");
     if (st == BH_OK) {
@@ -551,7 +551,16 @@ bh_status bh_potential(bh_ctx *c, double theta, double eps, double G, double *ph
     if (!c->built) return fail(c, BH_ERR_STATE, "bh_potential before bh_build");
     if (!phi_dev) return fail(c, BH_ERR_INVALID_ARG, "bh_potential: null pointer");
     if (!(theta >= 0.0) || !(eps >= 0.0)) return fail(c, BH_ERR_INVALID_ARG, "bh_potential: theta or eps negative");
-    return do_accel(c, theta, eps, G, phi_dev, true);
+    return do_accel(c, theta, eps, G, phi_dev, 1);
+}
+
+bh_status bh_accel_potential(bh_ctx *c, double theta, double eps, double G, double *acc_dev, double *phi_dev)
+{
+    if (!c) return BH_ERR_INVALID_ARG;
+    if (!c->built) return fail(c, BH_ERR_STATE, "bh_accel_potential before bh_build");
+    if (!acc_dev || !phi_dev) return fail(c, BH_ERR_INVALID_ARG, "bh_accel_potential: null pointer");
+    if (!(theta >= 0.0) || !(eps >= 0.0)) return fail(c, BH_ERR_INVALID_ARG, "bh_accel_potential: theta or eps negative");
+    return do_accel(c, theta, eps, G, acc_dev, 2, phi_dev);
 }
 
 bh_status bh_direct_potential(bh_ctx *c, double eps, double G, double *phi_dev)

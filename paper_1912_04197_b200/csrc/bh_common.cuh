@@ -112,8 +112,8 @@ void launch_gather(const Workspace &w, const double *pos, const double *mass, in
 void launch_pack(const Workspace &w, const double *pos, const double *mass, int64_t n, cudaStream_t s);
 void launch_tree(const Workspace &w, int64_t n, int leaf_cap, cudaStream_t s);
 void launch_monopoles(const Workspace &w, int64_t n, cudaStream_t s);
-// potential = false: acc [n][3] accelerations; true: acc [n] potential (NEXT-1)
-void launch_walk(const Workspace &w, int64_t n, double theta, double eps, double G, double *acc, bool potential,
+// mode 0: acc [n][3] accelerations; 1: acc [n] potential; 2: acc [n][3] and phi [n] from one walk (NEXT-1)
+void launch_walk(const Workspace &w, int64_t n, double theta, double eps, double G, double *acc, int mode, double *phi,
                  cudaStream_t s);
 int launch_direct(const Workspace &w, int64_t n, const int32_t *tgt, int64_t nt, double eps, double G,
                   double *acc, bool potential, cudaStream_t s);   // returns the number of kernels launched

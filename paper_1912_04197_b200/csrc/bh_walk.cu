@@ -108,11 +108,43 @@ __device__ __forceinline__ void interact_pot(double px, double py, double pz, do
     phi = fma(w, h, phi);
 }
 
-template <bool GUARD, bool POT>
-__device__ __forceinline__ void interact_any(double px, double py, double pz, double eps2, const double4 s,
-                                             double &ax, double &ay, double &az)
+// acceleration and potential of one interaction from one seed: 16 + 3 fp64 instructions
+template <bool GUARD>
+__device__ __forceinline__ void interact_both(double px, double py, double pz, double eps2, const double4 s,
+                                              double &ax, double &ay, double &az, double &phi)
 {
-    if constexpr (POT) interact_pot<GUARD>(px, py, pz, eps2, s, ax);
+    const double dx = s.x - px, dy = s.y - py, dz = s.z - pz;
+    const double t2 = fma(dy, dy, fma(dz, dz, eps2));
+    const double r2 = fma(dx, dx, t2);
+    double y;
+    {
+        double y0;
+        asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y0) : "d"(r2));
+        y = __hiloint2double(__double2hiint(y0), __double2loint(t2));
+    }
+    if (GUARD) y = (r2 > 0.0) ? y : 0.0;
+    const double u = y * y;
+    const double w = s.w * y;
+    const double e = fma(-r2, u, 1.0);
+    const double v = u * w;
+    const double p = fma(1.875, e, 1.5);
+    const double q = fma(0.375, e, 0.5);
+    const double h = fma(p, e, 1.0);
+    const double g = fma(q, e, 1.0);
+    const double f = v * h;
+    phi = fma(w, g, phi);
+    ax = fma(f, dx, ax);
+    ay = fma(f, dy, ay);
+    az = fma(f, dz, az);
+}
+
+// MODE 0: accelerations, 1: potential (accumulated in ax), 2: both
+template <bool GUARD, int MODE>
+__device__ __forceinline__ void interact_any(double px, double py, double pz, double eps2, const double4 s,
+                                             double &ax, double &ay, double &az, double &ph)
+{
+    if constexpr (MODE == 1) interact_pot<GUARD>(px, py, pz, eps2, s, ax);
+    else if constexpr (MODE == 2) interact_both<GUARD>(px, py, pz, eps2, s, ax, ay, az, ph);
     else interact<GUARD>(px, py, pz, eps2, s, ax, ay, az);
 }
 
@@ -460,11 +492,11 @@ __device__ void produce(PairSmem &ps, DevState *st, const unsigned *__restrict__
 // real) and, of every chunk of eight sources, takes sources q and q+4.
 template <int NS>
 struct Bodies {
-    double x[NS], y[NS], z[NS], ax[NS], ay[NS], az[NS];
+    double x[NS], y[NS], z[NS], ax[NS], ay[NS], az[NS], ph[NS];   // ph only lives in MODE 2
 };
 
 // evaluate n8 (a multiple of 8) sources starting at ring position head (a multiple of 8)
-template <bool GUARD, int NS, bool POT>
+template <bool GUARD, int NS, int MODE>
 __device__ __forceinline__ void eval_chunks(const double4 *ring, unsigned head, unsigned n8, unsigned quarter,
                                             double eps2, Bodies<NS> &B)
 {
@@ -473,17 +505,17 @@ __device__ __forceinline__ void eval_chunks(const double4 *ring, unsigned head, 
         const double4 *p = ring + ((head + i) & (kRing - 1)) + quarter;
         const double4 s0 = p[0], s1 = p[4];
 #pragma unroll
-        for (int k = 0; k < NS; ++k) interact_any<GUARD, POT>(B.x[k], B.y[k], B.z[k], eps2, s0, B.ax[k], B.ay[k], B.az[k]);
+        for (int k = 0; k < NS; ++k) interact_any<GUARD, MODE>(B.x[k], B.y[k], B.z[k], eps2, s0, B.ax[k], B.ay[k], B.az[k], B.ph[k]);
 #pragma unroll
-        for (int k = 0; k < NS; ++k) interact_any<GUARD, POT>(B.x[k], B.y[k], B.z[k], eps2, s1, B.ax[k], B.ay[k], B.az[k]);
+        for (int k = 0; k < NS; ++k) interact_any<GUARD, MODE>(B.x[k], B.y[k], B.z[k], eps2, s1, B.ax[k], B.ay[k], B.az[k], B.ph[k]);
     }
 }
 
 // one group: evaluate its sources as the producer publishes them, then write the accelerations
-template <bool GUARD, int NS, bool POT>
+template <bool GUARD, int NS, int MODE>
 __device__ __forceinline__ long long consume_group(PairSmem &ps, unsigned k, unsigned head, long long gb, long long ge,
                                               const double4 *__restrict__ sbody, const unsigned *__restrict__ perm,
-                                              double eps2, double G, double *__restrict__ acc)
+                                              double eps2, double G, double *__restrict__ acc, double *__restrict__ phi)
 {
     const unsigned lane = lane_id(), quarter = lane >> 3, r = lane & 7u;
     Bodies<NS> B;
@@ -492,7 +524,7 @@ __device__ __forceinline__ long long consume_group(PairSmem &ps, unsigned k, uns
         const long long j = gb + r + 8 * s;
         const double4 bd = sbody[j < ge ? j : gb];
         B.x[s] = bd.x; B.y[s] = bd.y; B.z[s] = bd.z;
-        B.ax[s] = B.ay[s] = B.az[s] = 0.0;
+        B.ax[s] = B.ay[s] = B.az[s] = B.ph[s] = 0.0;
     }
     const double4 zero4 = make_double4(0.0, 0.0, 0.0, 0.0);
     long long g_prof_wait = 0;   // cycles spent waiting for the producer (profiling builds only)
@@ -517,7 +549,7 @@ __device__ __forceinline__ long long consume_group(PairSmem &ps, unsigned k, uns
             continue;
         }
         const unsigned n8 = avail > 0 ? ((unsigned)avail & ~7u) : 0u;
-        eval_chunks<GUARD, NS, POT>(ps.ring, head, n8, quarter, eps2, B);
+        eval_chunks<GUARD, NS, MODE>(ps.ring, head, n8, quarter, eps2, B);
         head += n8;
         if (fin) {
             const unsigned rest = (unsigned)(avail > 0 ? avail : 0) & 7u;
@@ -526,9 +558,9 @@ __device__ __forceinline__ long long consume_group(PairSmem &ps, unsigned k, uns
                 const double4 s0 = quarter < rest ? p[0] : zero4;
                 const double4 s1 = quarter + 4 < rest ? p[4] : zero4;
 #pragma unroll
-                for (int s = 0; s < NS; ++s) interact_any<GUARD, POT>(B.x[s], B.y[s], B.z[s], eps2, s0, B.ax[s], B.ay[s], B.az[s]);
+                for (int s = 0; s < NS; ++s) interact_any<GUARD, MODE>(B.x[s], B.y[s], B.z[s], eps2, s0, B.ax[s], B.ay[s], B.az[s], B.ph[s]);
 #pragma unroll
-                for (int s = 0; s < NS; ++s) interact_any<GUARD, POT>(B.x[s], B.y[s], B.z[s], eps2, s1, B.ax[s], B.ay[s], B.az[s]);
+                for (int s = 0; s < NS; ++s) interact_any<GUARD, MODE>(B.x[s], B.y[s], B.z[s], eps2, s1, B.ax[s], B.ay[s], B.az[s], B.ph[s]);
                 head += rest;
             }
             warp_release(&ps.ctrl.head_pub, head, lane);
@@ -536,7 +568,7 @@ __device__ __forceinline__ long long consume_group(PairSmem &ps, unsigned k, uns
         }
         warp_release(&ps.ctrl.head_pub, head, lane);
     }
-    if constexpr (POT) {
+    if constexpr (MODE != 0) {
         // pairs inside the group: quarter q takes the group's bodies gb + q, gb + q + 4, ...; a body skips itself
         for (long long k = gb + quarter; k < ge; k += 4) {
             const double4 sk = sbody[k];
@@ -544,14 +576,20 @@ __device__ __forceinline__ long long consume_group(PairSmem &ps, unsigned k, uns
             for (int s = 0; s < NS; ++s) {
                 double4 src = sk;
                 if (k == gb + r + 8 * s) src.w = 0.0;
-                interact_pot<true>(B.x[s], B.y[s], B.z[s], eps2, src, B.ax[s]);
+                interact_any<true, MODE>(B.x[s], B.y[s], B.z[s], eps2, src, B.ax[s], B.ay[s], B.az[s], B.ph[s]);
             }
         }
     }
     // add the four quarter-warp partial sums; lane 8 q + r then writes body r + 8 q
-    double ox = 0.0, oy = 0.0, oz = 0.0;
+    double ox = 0.0, oy = 0.0, oz = 0.0, op = 0.0;
 #pragma unroll
     for (int s = 0; s < NS; ++s) {
+        if constexpr (MODE == 2) {
+            double tp = B.ph[s];
+            tp += __shfl_xor_sync(0xffffffffu, tp, 8);
+            tp += __shfl_xor_sync(0xffffffffu, tp, 16);
+            if ((int)quarter == s) op = tp;
+        }
         double tx = B.ax[s], ty = B.ay[s], tz = B.az[s];
         tx += __shfl_xor_sync(0xffffffffu, tx, 8);
         ty += __shfl_xor_sync(0xffffffffu, ty, 8);
@@ -564,9 +602,10 @@ __device__ __forceinline__ long long consume_group(PairSmem &ps, unsigned k, uns
     const long long j = gb + lane;
     if (j < ge) {
         const unsigned i = perm[j];
-        if constexpr (POT) {
+        if constexpr (MODE == 1) {
             acc[i] = -G * ox;                       // phi, one value per body
         } else {
+            if constexpr (MODE == 2) phi[i] = -G * op;
             acc[3ll * i + 0] = G * ox;
             acc[3ll * i + 1] = G * oy;
             acc[3ll * i + 2] = G * oz;
@@ -575,9 +614,10 @@ __device__ __forceinline__ long long consume_group(PairSmem &ps, unsigned k, uns
     return g_prof_wait;
 }
 
-template <bool GUARD, bool POT>
+template <bool GUARD, int MODE>
 __device__ void consume(PairSmem &ps, DevState *prof_st, const unsigned *__restrict__ gstart, const double4 *__restrict__ sbody,
-                        const unsigned *__restrict__ perm, double eps2, double G, double *__restrict__ acc)
+                        const unsigned *__restrict__ perm, double eps2, double G, double *__restrict__ acc,
+                        double *__restrict__ phi)
 {
     const unsigned lane = lane_id();
     long long waited = 0;
@@ -598,10 +638,10 @@ __device__ void consume(PairSmem &ps, DevState *prof_st, const unsigned *__restr
         const long long gb = gstart[g];
         const long long ge = gstart[g + 1];
         const int slots = (int)((ge - gb + 7) >> 3);
-        if (slots >= 4) waited += consume_group<GUARD, 4, POT>(ps, k, head, gb, ge, sbody, perm, eps2, G, acc);
-        else if (slots == 3) waited += consume_group<GUARD, 3, POT>(ps, k, head, gb, ge, sbody, perm, eps2, G, acc);
-        else if (slots == 2) waited += consume_group<GUARD, 2, POT>(ps, k, head, gb, ge, sbody, perm, eps2, G, acc);
-        else waited += consume_group<GUARD, 1, POT>(ps, k, head, gb, ge, sbody, perm, eps2, G, acc);
+        if (slots >= 4) waited += consume_group<GUARD, 4, MODE>(ps, k, head, gb, ge, sbody, perm, eps2, G, acc, phi);
+        else if (slots == 3) waited += consume_group<GUARD, 3, MODE>(ps, k, head, gb, ge, sbody, perm, eps2, G, acc, phi);
+        else if (slots == 2) waited += consume_group<GUARD, 2, MODE>(ps, k, head, gb, ge, sbody, perm, eps2, G, acc, phi);
+        else waited += consume_group<GUARD, 1, MODE>(ps, k, head, gb, ge, sbody, perm, eps2, G, acc, phi);
         warp_release(&ps.ctrl.consumed, k + 1, lane);
     }
 #ifdef BH_WALK_PROF
@@ -614,13 +654,13 @@ __device__ void consume(PairSmem &ps, DevState *prof_st, const unsigned *__restr
 #endif
 }
 
-template <bool GUARD, bool POT>
+template <bool GUARD, int MODE>
 __global__ void __launch_bounds__(kWalkThreads, 1)
 walk_kernel(DevState *st, const unsigned *__restrict__ gstart, const double4 *__restrict__ sbody,
             const double *__restrict__ gbox, const unsigned *__restrict__ perm,
             const uint4 *__restrict__ winfo, const double4 *__restrict__ mono, double theta2, double eps2,
             double G, double *__restrict__ acc, unsigned *__restrict__ cnt_mono,
-            unsigned *__restrict__ cnt_direct, unsigned *walk_stack)
+            unsigned *__restrict__ cnt_direct, unsigned *walk_stack, double *__restrict__ phi)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     WalkSmem &sm = *reinterpret_cast<WalkSmem *>(smem_raw);
@@ -638,10 +678,10 @@ walk_kernel(DevState *st, const unsigned *__restrict__ gstart, const double4 *__
     else asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(BH_REG_CONS));
 #endif
     if (producer)
-        produce<POT>(ps, st, gstart, sbody, gbox, winfo, mono, theta2, cnt_mono, cnt_direct,
+        produce<MODE != 0>(ps, st, gstart, sbody, gbox, winfo, mono, theta2, cnt_mono, cnt_direct,
                 reinterpret_cast<uint2 *>(walk_stack) + (size_t)(blockIdx.x * kPairs + pair) * kStackSlab);
     else
-        consume<GUARD, POT>(ps, st, gstart, sbody, perm, eps2, G, acc);
+        consume<GUARD, MODE>(ps, st, gstart, sbody, perm, eps2, G, acc, phi);
 }
 
 // ------------------------------------------------------------------------------------------ a8
@@ -762,31 +802,35 @@ __global__ void __launch_bounds__(256) fp64_peak_kernel(double *sink, int iters,
 }
 
 // ------------------------------------------------------------------------------------------ launchers
-template <bool GUARD, bool POT>
-static void launch_walk_t(const Workspace &w, double theta, double eps2, double G, double *out, cudaStream_t s)
+template <bool GUARD, int MODE>
+static void launch_walk_t(const Workspace &w, double theta, double eps2, double G, double *out, double *phi, cudaStream_t s)
 {
     static bool configured = false;
     if (!configured) {
-        cudaFuncSetAttribute(walk_kernel<GUARD, POT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(WalkSmem));
+        cudaFuncSetAttribute(walk_kernel<GUARD, MODE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(WalkSmem));
         configured = true;
     }
     const int blocks = w.walk_warps / kPairs;   // one persistent block per SM
-    walk_kernel<GUARD, POT><<<blocks, kWalkThreads, sizeof(WalkSmem), s>>>(
+    walk_kernel<GUARD, MODE><<<blocks, kWalkThreads, sizeof(WalkSmem), s>>>(
         w.st, w.gstart, w.sbody, w.gbox, w.idx[0], w.winfo, w.mono, theta * theta, eps2, G, out, w.cnt_mono,
-        w.cnt_direct, w.walk_stack);
+        w.cnt_direct, w.walk_stack, phi);
 }
 
-void launch_walk(const Workspace &w, int64_t n, double theta, double eps, double G, double *acc, bool potential,
+void launch_walk(const Workspace &w, int64_t n, double theta, double eps, double G, double *acc, int mode, double *phi,
                  cudaStream_t s)
 {
     (void)n;
     const double eps2 = eps * eps;
-    if (potential) {
-        if (eps2 > 0.0) launch_walk_t<false, true>(w, theta, eps2, G, acc, s);
-        else launch_walk_t<true, true>(w, theta, eps2, G, acc, s);
+    const bool guard = !(eps2 > 0.0);
+    if (mode == 1) {
+        if (guard) launch_walk_t<true, 1>(w, theta, eps2, G, acc, nullptr, s);
+        else launch_walk_t<false, 1>(w, theta, eps2, G, acc, nullptr, s);
+    } else if (mode == 2) {
+        if (guard) launch_walk_t<true, 2>(w, theta, eps2, G, acc, phi, s);
+        else launch_walk_t<false, 2>(w, theta, eps2, G, acc, phi, s);
     } else {
-        if (eps2 > 0.0) launch_walk_t<false, false>(w, theta, eps2, G, acc, s);
-        else launch_walk_t<true, false>(w, theta, eps2, G, acc, s);
+        if (guard) launch_walk_t<true, 0>(w, theta, eps2, G, acc, nullptr, s);
+        else launch_walk_t<false, 0>(w, theta, eps2, G, acc, nullptr, s);
     }
 }
 

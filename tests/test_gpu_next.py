@@ -256,3 +256,27 @@ def test_cuda_graph_steppers_bit_identical(n, method):
         ctx.close()
     assert np.array_equal(outs[0][0], outs[1][0]) and np.array_equal(outs[0][1], outs[1][1])
     assert outs[0][2] == outs[1][2]             # the launch count is the same claim on both paths
+
+
+@pytest.mark.parametrize("name,n,C", [("c1", 1024, 8), ("c2", 16384, 16), ("c4", 30000, 16), ("c3", 777, 1), ("c3", 5, 16)])
+def test_accel_and_potential_from_one_walk(name, n, C):
+    """bh_accel_potential: both outputs of the fused walk against the oracle's two evaluations (same lists)."""
+    w = wl.make(name, n)
+    t = orc.build(w.pos, w.mass, C)
+    ctx = bh.Context(n, C)
+    ctx.build(dev(w.pos), dev(w.mass))
+    acc = torch.empty((n, 3), dtype=torch.float64, device="cuda")
+    phi = torch.empty(n, dtype=torch.float64, device="cuda")
+    bh.bh_accel_potential(ctx.ctx, w.theta, w.eps, w.G, acc, phi)
+    a_ref, nm, nd, _ = orc.accel(t, w.theta, w.eps, w.G)
+    p_ref = orc.potential(t, w.theta, w.eps, w.G)
+    a = acc.cpu().numpy()
+    nz = np.linalg.norm(a_ref, axis=1) > 0
+    assert (np.linalg.norm(a - a_ref, axis=1)[nz] / np.linalg.norm(a_ref, axis=1)[nz]).max() <= TOL
+    assert np.abs(phi.cpu().numpy() - p_ref).max() <= TOL * np.abs(p_ref).min()
+    gm, gd = ctx.counts()
+    assert np.array_equal(gm.cpu().numpy().view(np.uint32), nm) and np.array_equal(gd.cpu().numpy().view(np.uint32), nd)
+    # and it equals the two separate calls to rounding
+    a2 = ctx.accel(w.theta, w.eps, w.G).cpu().numpy()
+    assert np.abs(a - a2).max() <= 1e-12 * np.abs(a2).max()
+    ctx.close()
