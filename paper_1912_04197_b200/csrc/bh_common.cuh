@@ -16,7 +16,10 @@ constexpr int kRadixBits = 8;
 constexpr int kRadix = 1 << kRadixBits;   // 256 bins
 constexpr int kSortPasses = 8;            // 63 key bits
 constexpr int kSortThreads = 256;
-constexpr int kSortItems = 16;            // keys per thread
+#ifndef BH_SORT_ITEMS
+#define BH_SORT_ITEMS 16
+#endif
+constexpr int kSortItems = BH_SORT_ITEMS;   // keys per thread
 constexpr int kSortTile = kSortThreads * kSortItems;   // 4096 keys per tile
 constexpr int kTreeTile = 1024;           // bodies per block in the tree kernels
 constexpr int kDiagBlocks = 148 * 4;       // diagnostics: most blocks (fixed, so the reduction order is fixed)
