@@ -42,7 +42,9 @@ typedef enum {
 } bh_status;
 
 #define BH_MAX_LEVEL 21    /* 63-bit Morton keys, 3 bits per level (R9) */
+#ifndef BH_GROUP_CELL
 #define BH_GROUP_CELL 512  /* Gc: walk groups never straddle a tree cell holding <= Gc bodies (R6) */
+#endif
 
 /* Bytes of device workspace a context for up to max_n bodies needs.  0 if the arguments are invalid
  * (max_n < 1 or > 2^30, leaf_cap < 1 or > 1024, group_size not 0 or 32). */
