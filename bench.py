@@ -310,6 +310,7 @@ def run_own(args):
     inter_avg = sum(inter) / nph
     achieved = FLOPS_PER_INTERACTION * inter_avg / (walk_avg_ms * 1e-3) / 1e12
     peak_meas = bh.bh_measure_fp64_peak(ctx.ctx)
+    issue = bh.bh_measure_issue_model(ctx.ctx)
     roofline = {"bound": "alu", "kernel": "walk_kernel", "achieved": achieved, "peak": FP64_PEAK_TFLOPS,
                 "unit": "TFLOP/s", "frac": achieved / FP64_PEAK_TFLOPS,
                 "peak_source": "derived 148 SM x 64 fp64 FMA lanes x 2 x 1.965 GHz (DESIGN.md); "
@@ -317,6 +318,8 @@ def run_own(args):
                 "peak_measured_dfma": peak_meas, "frac_of_measured_dfma": achieved / peak_meas,
                 "flops_per_interaction": FLOPS_PER_INTERACTION, "interactions_per_launch": inter_avg,
                 "interactions_per_s": inter_avg / (walk_avg_ms * 1e-3), "kernel_ms": walk_avg_ms,
+                "issue_model_interactions_per_s": issue,
+                "frac_of_eval_loop_alone": inter_avg / (walk_avg_ms * 1e-3) / issue["eval_loop_alone"],
                 "traffic": args.walk_traffic if args.walk_traffic is not None else WALK_TRAFFIC_NCU.get(w.name),
                 "traffic_source": "profiles/r01_walk_ncu_full.md (ncu --set full, bytes per launch)"}
     # build kernels against HBM: algorithmic bytes per body over the build time

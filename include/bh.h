@@ -237,6 +237,14 @@ bh_status bh_get_phase_ms(bh_ctx *ctx, float ms_host[BH_NUM_PHASES]);
  * direct kernels.  Synchronising. */
 bh_status bh_measure_fp64_peak(bh_ctx *ctx, double *tflops_host);
 
+/* Synchronising microbenchmark behind the walk kernel's roofline statement: the walk's own
+ * evaluation loop (two evaluating warps per SM sub-partition, four bodies per lane, sources in shared memory)
+ * in body-source interactions per second  [0] with nothing else on the sub-partition,  [1] beside two warps per
+ * sub-partition running a dependent integer / shared-memory chain at low duty (what the walk's traversal warps
+ * look like),  [2] beside two warps issuing independent integer instructions at full rate.  [0] is the ceiling
+ * of a warp-specialised walk; [0] - [1] is what co-resident traversal warps cost the fp64 warps. */
+bh_status bh_measure_issue_model(bh_ctx *ctx, double out_host[3]);
+
 const char *bh_last_error(const bh_ctx *ctx);
 const char *bh_version(void);
 

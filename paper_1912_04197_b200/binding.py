@@ -79,6 +79,7 @@ def lib() -> C.CDLL:
             "bh_set_timing": [vp, i32],
             "bh_get_phase_ms": [vp, C.POINTER(C.c_float)],
             "bh_measure_fp64_peak": [vp, C.POINTER(dbl)],
+            "bh_measure_issue_model": [vp, C.POINTER(dbl)],
         }
         for name, args in sigs.items():
             f = getattr(L, name)
@@ -96,7 +97,7 @@ EXPORTS = ("bh_workspace_bytes", "bh_create", "bh_destroy", "bh_set_stream", "bh
            "bh_get_phase_ms", "bh_measure_fp64_peak", "bh_last_error", "bh_version",
            "bh_euler_step", "bh_multirate_step", "bh_potential", "bh_direct_potential", "bh_diagnostics",
            "bh_position_error", "bh_gravity_dt", "bh_copy_state_acc", "bh_set_gravity_method",
-           "bh_broadphase", "bh_aggregates", "bh_set_graph", "bh_accel_potential")
+           "bh_broadphase", "bh_aggregates", "bh_set_graph", "bh_accel_potential", "bh_measure_issue_model")
 
 
 def _check(ctx, status: int):
@@ -323,6 +324,12 @@ def bh_measure_fp64_peak(ctx) -> float:
     v = C.c_double()
     _check(ctx, lib().bh_measure_fp64_peak(ctx, C.byref(v)))
     return v.value
+
+
+def bh_measure_issue_model(ctx):
+    v = (C.c_double * 3)()
+    _check(ctx, lib().bh_measure_issue_model(ctx, v))
+    return {"eval_loop_alone": v[0], "beside_low_duty_integer_warps": v[1], "beside_full_rate_integer_warps": v[2]}
 
 
 # ---- convenience owner of a context and its torch-allocated workspace (no arithmetic) ----

@@ -866,4 +866,12 @@ bh_status bh_measure_fp64_peak(bh_ctx *c, double *tflops_host)
     return cuda_check(c, cudaGetLastError(), "bh_measure_fp64_peak");
 }
 
+bh_status bh_measure_issue_model(bh_ctx *c, double out_host[3])
+{
+    if (!c || !out_host) return BH_ERR_INVALID_ARG;
+    run_issue_model(c->ws, out_host, c->stream);
+    c->launches += 6;
+    return cuda_check(c, cudaGetLastError(), "bh_measure_issue_model");
+}
+
 }  // extern "C"

@@ -124,6 +124,7 @@ void launch_kick_drift(double *pos, double *vel, const double *acc, int64_t n, d
 void launch_kick(double *vel, const double *acc, int64_t n, double h, cudaStream_t s);
 void launch_unpack_mask(const Workspace &w, unsigned char *mask_out, int64_t cap, cudaStream_t s);
 double run_fp64_peak(const Workspace &w, cudaStream_t s);
+void run_issue_model(const Workspace &w, double out[3], cudaStream_t s);   // see bh_measure_issue_model
 // rows "next" (bh_diag.cu): results land in w.diag_out
 void launch_diagnostics(const Workspace &w, const double *pos, const double *vel, const double *mass,
                         const double *phi, int64_t n, cudaStream_t s);

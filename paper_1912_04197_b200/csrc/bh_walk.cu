@@ -801,6 +801,74 @@ __global__ void __launch_bounds__(256) fp64_peak_kernel(double *sink, int iters,
     if (s == 123456.789) sink[0] = s;
 }
 
+// ------------------------------------------------------------------------------------------ issue model
+// What the walk's evaluation loop reaches when nothing else runs on its sub-partition, and what it loses to
+// co-resident warps that issue integer / shared-memory instructions (as the walk's producer warps do).  Same
+// block shape as walk_kernel: 16 warps, warps 4-7 and 12-15 evaluate (two per sub-partition, four bodies per
+// lane, sources from a 512-entry shared-memory ring); the other eight warps exit (HOG 0), run a dependent
+// IMAD / LDS chain at low duty (HOG 1) or independent IMADs at full rate (HOG 2) until the evaluators are done.
+template <int HOG>
+__global__ void __launch_bounds__(512, 1) issue_model_kernel(double *sink, int iters, double eps2, int seed)
+{
+    __shared__ double4 ring[512];
+    __shared__ int tab[1024];
+    __shared__ int done;
+    for (int i = threadIdx.x; i < 512; i += blockDim.x) ring[i] = make_double4(1.0 + i * 0.01, 2.0 - i * 0.02, 0.5 + i * 0.003, 1e-3);
+    for (int i = threadIdx.x; i < 1024; i += blockDim.x) tab[i] = (i * 7 + seed) & 1023;
+    if (threadIdx.x == 0) done = 0;
+    __syncthreads();
+    const unsigned warp = threadIdx.x >> 5, lane = threadIdx.x & 31u, quarter = lane >> 3;
+    if (((warp >> 2) & 1u) == 1u) {
+        Bodies<4> B;
+        for (int s = 0; s < 4; ++s) {
+            B.x[s] = 0.1 * lane + s; B.y[s] = 0.2 * s; B.z[s] = 0.05 * lane;
+            B.ax[s] = B.ay[s] = B.az[s] = B.ph[s] = 0.0;
+        }
+        for (int it = 0; it < iters; ++it) eval_chunks<false, 4, 0>(ring, 0u, 512u, quarter, eps2, B);
+        double s = 0.0;
+        for (int q = 0; q < 4; ++q) s += B.ax[q] + B.ay[q] + B.az[q];
+        if (s == 123.456) sink[0] = s;
+        __syncwarp();
+        if (lane == 0) atomicAdd(&done, 1);
+    } else if (HOG != 0) {
+        int a = seed + (int)lane, b = seed * 3 + (int)lane, c = (int)lane;
+        while (*((volatile int *)&done) < 8) {
+            if (HOG == 1) {
+                for (int r = 0; r < 16; ++r) { a = tab[(a * 5 + b) & 1023]; b = b * 3 + a; c ^= a + b; }
+            } else {
+                for (int r = 0; r < 16; ++r) { a = a * 5 + seed; b = b * 3 + seed; c = c * 7 + seed; }
+            }
+        }
+        if (a + b + c == 12345) sink[1] = a;
+    }
+}
+
+template <int HOG>
+static double run_issue_model_one(double *sink, cudaStream_t s)
+{
+    const int iters = 100, blocks = WalkConfig::kSMs;
+    cudaEvent_t a, b;
+    cudaEventCreate(&a);
+    cudaEventCreate(&b);
+    issue_model_kernel<HOG><<<blocks, 512, 0, s>>>(sink, 2, 1e-8, 3);
+    cudaEventRecord(a, s);
+    issue_model_kernel<HOG><<<blocks, 512, 0, s>>>(sink, iters, 1e-8, 3);
+    cudaEventRecord(b, s);
+    cudaEventSynchronize(b);
+    float ms = 0.f;
+    cudaEventElapsedTime(&ms, a, b);
+    cudaEventDestroy(a);
+    cudaEventDestroy(b);
+    return (double)blocks * 8 * 32 * iters * 64.0 * 2.0 * 4 / (ms * 1e-3);   // body-source interactions per second
+}
+
+void run_issue_model(const Workspace &w, double out[3], cudaStream_t s)
+{
+    out[0] = run_issue_model_one<0>(w.peak_sink, s);
+    out[1] = run_issue_model_one<1>(w.peak_sink, s);
+    out[2] = run_issue_model_one<2>(w.peak_sink, s);
+}
+
 // ------------------------------------------------------------------------------------------ launchers
 template <bool GUARD, int MODE>
 static void launch_walk_t(const Workspace &w, double theta, double eps2, double G, double *out, double *phi, cudaStream_t s)
