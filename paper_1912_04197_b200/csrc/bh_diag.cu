@@ -99,15 +99,22 @@ diag_kernel(const double *__restrict__ pos, const double *__restrict__ vel, cons
     __syncthreads();
     if (threadIdx.x == 0) last = atomicAdd(ticket, 1u) == gridDim.x - 1;
     __syncthreads();
-    if (last && threadIdx.x < kDiagQ) {
+    if (last) {
+        // the last block adds the per-block partials in a fixed order: lane j of warp q takes blocks j, j + 32, ...
+        // in increasing order, then the 32 lane sums are added in lane order (warp q = quantity q)
         __threadfence();
-        const int q = threadIdx.x;
+        const int q = threadIdx.x >> 5;
         const volatile double *vp = part;
         dd s = {0.0, 0.0};
-        for (unsigned b = 0; b < gridDim.x; ++b)
+        for (unsigned b = lane; b < gridDim.x; b += 32)
             s = dd_add(s, {vp[((size_t)b * kDiagQ + q) * 2 + 0], vp[((size_t)b * kDiagQ + q) * 2 + 1]});
-        out[q] = s.hi;
-        if (q == 0) *ticket = 0u;
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) {
+            dd other = {__shfl_down_sync(0xffffffffu, s.hi, o), __shfl_down_sync(0xffffffffu, s.lo, o)};
+            s = dd_add(s, other);
+        }
+        if (lane == 0) out[q] = s.hi;
+        if (threadIdx.x == 0) *ticket = 0u;
     }
 }
 
