@@ -690,21 +690,27 @@ walk_kernel(DevState *st, const unsigned *__restrict__ gstart, const double4 *__
 // is split over blockIdx.y so that every SM has work; the partial sums are then added in split order
 // by direct_reduce_kernel (deterministic).
 constexpr int kDirectThreads = 256;
-constexpr int kDirectTargets = 2 * kDirectThreads;
+constexpr int kDirectPer = 4;                            // targets per thread: one shared-memory read feeds four interactions
+constexpr int kDirectTargets = kDirectPer * kDirectThreads;
 
 template <bool GUARD, bool POT>
-__global__ void __launch_bounds__(kDirectThreads)
+__global__ void __launch_bounds__(kDirectThreads, 2)
 direct_kernel(long long n, const double4 *__restrict__ sbody, const unsigned *__restrict__ perm,
               const unsigned *__restrict__ iperm, const int32_t *__restrict__ tgt, long long nt, double eps2,
               double G, double *__restrict__ acc, double *__restrict__ partial, int tiles_per_split)
 {
     __shared__ double4 tile[kDirectThreads];
-    const long long r0 = (long long)blockIdx.x * kDirectTargets + threadIdx.x, r1 = r0 + kDirectThreads;
     // all bodies: row r is sorted body r, written to its original index; sampled: row r is target tgt[r]
-    const long long j0 = r0 < nt ? (tgt ? (long long)iperm[tgt[r0]] : r0) : 0;
-    const long long j1 = r1 < nt ? (tgt ? (long long)iperm[tgt[r1]] : r1) : 0;
-    const double4 p0 = sbody[j0], p1 = sbody[j1];
-    double ax0 = 0.0, ay0 = 0.0, az0 = 0.0, ax1 = 0.0, ay1 = 0.0, az1 = 0.0;
+    long long r[kDirectPer], j[kDirectPer];
+    double px[kDirectPer], py[kDirectPer], pz[kDirectPer], ax[kDirectPer], ay[kDirectPer], az[kDirectPer];
+#pragma unroll
+    for (int t = 0; t < kDirectPer; ++t) {
+        r[t] = (long long)blockIdx.x * kDirectTargets + t * kDirectThreads + threadIdx.x;
+        j[t] = r[t] < nt ? (tgt ? (long long)iperm[tgt[r[t]]] : r[t]) : 0;
+        const double4 p = sbody[j[t]];
+        px[t] = p.x; py[t] = p.y; pz[t] = p.z;
+        ax[t] = ay[t] = az[t] = 0.0;
+    }
     const long long s_begin = (long long)blockIdx.y * tiles_per_split * kDirectThreads;
     long long s_end = s_begin + (long long)tiles_per_split * kDirectThreads;
     if (s_end > n) s_end = n;
@@ -715,41 +721,32 @@ direct_kernel(long long n, const double4 *__restrict__ sbody, const unsigned *__
 #pragma unroll 4
         for (int q = 0; q < kDirectThreads; ++q) {
             const double4 sq = tile[q];
-            if constexpr (POT) {                 // a body skips itself: its own term m/eps is not zero
-                double4 s0 = sq, s1 = sq;
-                if (t0 + q == j0) s0.w = 0.0;
-                if (t0 + q == j1) s1.w = 0.0;
-                interact_pot<GUARD>(p0.x, p0.y, p0.z, eps2, s0, ax0);
-                interact_pot<GUARD>(p1.x, p1.y, p1.z, eps2, s1, ax1);
-            } else {
-                interact<GUARD>(p0.x, p0.y, p0.z, eps2, sq, ax0, ay0, az0);
-                interact<GUARD>(p1.x, p1.y, p1.z, eps2, sq, ax1, ay1, az1);
+#pragma unroll
+            for (int t = 0; t < kDirectPer; ++t) {
+                if constexpr (POT) {             // a body skips itself: its own term m/eps is not zero
+                    double4 st = sq;
+                    if (t0 + q == j[t]) st.w = 0.0;
+                    interact_pot<GUARD>(px[t], py[t], pz[t], eps2, st, ax[t]);
+                } else {
+                    interact<GUARD>(px[t], py[t], pz[t], eps2, sq, ax[t], ay[t], az[t]);
+                }
             }
         }
         __syncthreads();
     }
-    if constexpr (POT) {                     // one value per body: phi = -G sum m / r
-        if (gridDim.y == 1) {
-            if (r0 < nt) acc[tgt ? r0 : (long long)perm[r0]] = -G * ax0;
-            if (r1 < nt) acc[tgt ? r1 : (long long)perm[r1]] = -G * ax1;
+#pragma unroll
+    for (int t = 0; t < kDirectPer; ++t) {
+        if (r[t] >= nt) continue;
+        if constexpr (POT) {                 // one value per body: phi = -G sum m / r
+            if (gridDim.y == 1) acc[tgt ? r[t] : (long long)perm[r[t]]] = -G * ax[t];
+            else partial[(size_t)blockIdx.y * nt + r[t]] = ax[t];
+        } else if (gridDim.y == 1) {
+            const long long o = tgt ? r[t] : (long long)perm[r[t]];
+            acc[3 * o + 0] = G * ax[t]; acc[3 * o + 1] = G * ay[t]; acc[3 * o + 2] = G * az[t];
         } else {
-            double *p = partial + (size_t)blockIdx.y * nt;
-            if (r0 < nt) p[r0] = ax0;
-            if (r1 < nt) p[r1] = ax1;
+            double *p = partial + (size_t)blockIdx.y * nt * 3;
+            p[3 * r[t] + 0] = ax[t]; p[3 * r[t] + 1] = ay[t]; p[3 * r[t] + 2] = az[t];
         }
-    } else if (gridDim.y == 1) {
-        if (r0 < nt) {
-            const long long o = tgt ? r0 : (long long)perm[r0];
-            acc[3 * o + 0] = G * ax0; acc[3 * o + 1] = G * ay0; acc[3 * o + 2] = G * az0;
-        }
-        if (r1 < nt) {
-            const long long o = tgt ? r1 : (long long)perm[r1];
-            acc[3 * o + 0] = G * ax1; acc[3 * o + 1] = G * ay1; acc[3 * o + 2] = G * az1;
-        }
-    } else {
-        double *p = partial + (size_t)blockIdx.y * nt * 3;
-        if (r0 < nt) { p[3 * r0 + 0] = ax0; p[3 * r0 + 1] = ay0; p[3 * r0 + 2] = az0; }
-        if (r1 < nt) { p[3 * r1 + 0] = ax1; p[3 * r1 + 1] = ay1; p[3 * r1 + 2] = az1; }
     }
 }
 
