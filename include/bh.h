@@ -185,9 +185,10 @@ double bh_gravity_dt(double G, double rho);
  * builds, walks, delivers acc_host [n][3] and waits.  Pinned host memory makes the copies asynchronous;
  * pageable memory works too.  The masses travel on a second stream beside the first build kernels (they
  * are first needed after the sort).  If acc_host is pinned (cudaHostAlloc / cudaHostRegister, e.g. a torch
- * pin_memory() tensor) the walk kernel stores the accelerations straight into it over PCIe while it
- * computes and no copy follows; otherwise they are staged in the workspace and copied
- * (environment BH_HOST_DIRECT=0 forces the staged path, for measurements). */
+ * pin_memory() tensor) and the previous evaluation through this call had at least 3400 interactions per
+ * body (so that 24 bytes per body stay below what small PCIe writes sustain), the walk kernel stores the
+ * accelerations straight into it while it computes and no copy follows; otherwise they are staged in the
+ * workspace and copied (environment BH_HOST_DIRECT=0 forces the staged path, for measurements). */
 bh_status bh_eval_host(bh_ctx *ctx, const double *pos_host, const double *mass_host, int64_t n,
                        double theta, double eps, double G, double *acc_host);
 

@@ -46,7 +46,8 @@ struct bh_ctx {
     };
     cudaStream_t copy_stream = nullptr;   // bh_eval_host: mass upload beside the first build kernels
     cudaEvent_t ev_copy[2]{};
-    bool host_direct = true;              // bh_eval_host: store accelerations straight into pinned host memory
+    bool host_direct = true;              // bh_eval_host: store accelerations straight into pinned host memory ...
+    double last_host_ipb = 0.0;           // ... when the previous evaluation had this many interactions per body
     bool use_graph = false;
     cudaGraphExec_t graph_exec = nullptr;
     StepSig graph_sig{}, seen_sig{};
@@ -700,7 +701,11 @@ bh_status bh_eval_host(bh_ctx *c, const double *pos_host, const double *mass_hos
     if ((st = do_build(c, w.stage_pos, w.stage_mass, n, c->ev_copy[1])) != BH_OK) return st;
     // Pinned output: the walk stores the accelerations straight into host memory (24 bytes per body,
     // over PCIe while the kernel computes), so no copy follows it.  Pageable output: staged in the workspace.
-    double *direct_out = c->host_direct ? mapped_alias(acc_host) : nullptr;
+    // It pays only while the stores keep below what small PCIe writes sustain (~6 GB/s measured): 24 bytes
+    // per body against the walk's time per body, i.e. when a body has many interactions (configs[3]: 4100 per
+    // body, 4.9 GB/s, 6.74 -> 6.38 ms; configs[4]: 2100 per body, 9.5 GB/s, 15.7 -> 24.7 ms).  The count of the
+    // previous evaluation through this call decides; the first evaluation is staged.
+    double *direct_out = (c->host_direct && c->last_host_ipb >= 3400.0) ? mapped_alias(acc_host) : nullptr;
     if ((st = do_accel(c, theta, eps, G, direct_out ? direct_out : w.acc)) != BH_OK) return st;
     c->have_acc = false;   // the internal acc buffer no longer belongs to the bound state
     c->acc_filled = false;
@@ -708,7 +713,9 @@ bh_status bh_eval_host(bh_ctx *c, const double *pos_host, const double *mass_hos
         e = cudaMemcpyAsync(acc_host, w.acc, 3 * n * sizeof(double), cudaMemcpyDeviceToHost, c->stream);
         if (e != cudaSuccess) return cuda_check(c, e, "bh_eval_host D2H");
     }
-    return fetch_state(c);
+    st = fetch_state(c);
+    if (st == BH_OK) c->last_host_ipb = (double)c->host_state->stats[2] / (double)n;
+    return st;
 }
 
 bh_status bh_synchronize(bh_ctx *c)

@@ -264,18 +264,28 @@ def test_full_size_headline_config():
 
 
 def test_eval_host_pageable_output_is_staged():
-    """bh_eval_host with ordinary (pageable) host memory takes the staged path; with pinned memory the walk
-    stores straight into the output.  Both must give the same accelerations bit for bit."""
+    """bh_eval_host with ordinary (pageable) host memory takes the staged path; with pinned memory, from the
+    second call on and when a body has enough interactions (>= 3400), the walk stores straight into the output.
+    All paths must give the same accelerations bit for bit."""
     w = wl.make("c4", 20000)
+    theta = 0.2                                      # ~ 6000 interactions per body: the direct-store path is taken
     ctx = bh.Context(w.n, 16)
     pos_h, mass_h = torch.as_tensor(w.pos), torch.as_tensor(w.mass)
     out_page = torch.empty((w.n, 3), dtype=torch.float64)
     out_pin = torch.empty((w.n, 3), dtype=torch.float64).pin_memory()
-    bh.bh_eval_host(ctx.ctx, pos_h, mass_h, w.theta, w.eps, w.G, out_page)
-    bh.bh_eval_host(ctx.ctx, pos_h.pin_memory(), mass_h.pin_memory(), w.theta, w.eps, w.G, out_pin)
-    assert np.array_equal(out_page.numpy(), out_pin.numpy())
-    ref = orc.accel(orc.build(w.pos, w.mass, 16), w.theta, w.eps, w.G)[0]
+    out_pin2 = torch.zeros((w.n, 3), dtype=torch.float64).pin_memory()
+    bh.bh_eval_host(ctx.ctx, pos_h, mass_h, theta, w.eps, w.G, out_page)
+    assert bh.bh_get_stats(ctx.ctx)["interactions"] / w.n >= 3400
+    bh.bh_eval_host(ctx.ctx, pos_h.pin_memory(), mass_h.pin_memory(), theta, w.eps, w.G, out_pin)
+    bh.bh_eval_host(ctx.ctx, pos_h.pin_memory(), mass_h.pin_memory(), theta, w.eps, w.G, out_pin2)
+    assert np.array_equal(out_page.numpy(), out_pin.numpy()) and np.array_equal(out_page.numpy(), out_pin2.numpy())
+    ref = orc.accel(orc.build(w.pos, w.mass, 16), theta, w.eps, w.G)[0]
     assert relerr(out_pin.numpy(), ref).max() <= TOL
+    # few interactions per body (theta = 1): staged again, same contract
+    bh.bh_eval_host(ctx.ctx, pos_h.pin_memory(), mass_h.pin_memory(), 1.0, w.eps, w.G, out_pin)
+    bh.bh_eval_host(ctx.ctx, pos_h.pin_memory(), mass_h.pin_memory(), 1.0, w.eps, w.G, out_pin2)
+    assert np.array_equal(out_pin.numpy(), out_pin2.numpy())
+    assert relerr(out_pin.numpy(), orc.accel(orc.build(w.pos, w.mass, 16), 1.0, w.eps, w.G)[0]).max() <= TOL
     ctx.close()
 
 
