@@ -153,12 +153,18 @@ def group_boxes(sbody, gstart):
     return glo, ghi
 
 
-DEFAULT_GC = 512   # group-cell capacity used by the CUDA path (R6)
+# Reading R6 ("each body is assigned to a thread ... neighbouring threads
+# traverse similar sub-trees"): the method's two grouping parameters and the values the reading fixes
+# when a caller names none.  They are parameters of the METHOD, owned by this oracle: the CUDA path
+# takes them as run-time arguments (bh_create group_size, bh_set_group_cell) and is tested against
+# this file at several (W, Gc), not only at the defaults.
+R6_W = 32      # bodies that walk the tree together
+R6_GC = 512    # group-cell capacity: a group never straddles a tree cell holding <= Gc bodies
 
 
-def build(pos, mass, leaf_cap: int, W: int = 32, Gc: int | None = None, gstart=None) -> Tree:
-    """O1..O7 in order: cube, keys, sort, gather, tree, monopoles, groups.  Gc defaults to
-    max(DEFAULT_GC, W); W = 1 with any Gc is the paper's per-body walk."""
+def build(pos, mass, leaf_cap: int, W: int = R6_W, Gc: int = R6_GC, gstart=None) -> Tree:
+    """O1..O7 in order: cube, keys, sort, gather, tree, monopoles, groups.  W = 1 (any Gc) is the
+    paper's per-body walk."""
     pos = np.ascontiguousarray(pos, dtype=np.float64)
     mass = np.ascontiguousarray(mass, dtype=np.float64)
     n = pos.shape[0]
@@ -169,8 +175,6 @@ def build(pos, mass, leaf_cap: int, W: int = 32, Gc: int | None = None, gstart=N
     lib().orc_gather(_p(pos), _p(mass), _p(perm), C.c_int64(n), _p(sbody))
     M, depth, level, begin, count, first_child, child_mask, parent = tree_from_keys(skey, leaf_cap)
     mono = monopoles(sbody, begin, count, first_child, child_mask)
-    if Gc is None:
-        Gc = max(DEFAULT_GC, W)
     if gstart is None:
         gstart = group_starts(n, W, Gc, begin, count, first_child, parent)
     gstart = np.ascontiguousarray(gstart, dtype=np.uint32)
@@ -243,18 +247,18 @@ class Leapfrog:
     """O11: KDK state machine with the semantics of include/bh.h bh_kdk_step: the first step
     evaluates a(x0) once; each step is kick(dt/2), drift(dt), rebuild + accel, kick(dt/2)."""
 
-    def __init__(self, pos, vel, mass, theta, eps, G, leaf_cap, W=32, use_direct=False):
+    def __init__(self, pos, vel, mass, theta, eps, G, leaf_cap, W=R6_W, use_direct=False, Gc=R6_GC):
         self.pos = np.array(pos, dtype=np.float64, order="C")
         self.vel = np.array(vel, dtype=np.float64, order="C")
         self.mass = np.ascontiguousarray(mass, dtype=np.float64)
-        self.theta, self.eps, self.G, self.C, self.W = theta, eps, G, leaf_cap, W
+        self.theta, self.eps, self.G, self.C, self.W, self.Gc = theta, eps, G, leaf_cap, W, Gc
         self.use_direct = use_direct
         self.acc = None
 
     def _eval(self):
         if self.use_direct:
             return direct(self.pos, self.mass, self.eps, self.G)
-        t = build(self.pos, self.mass, self.C, self.W)
+        t = build(self.pos, self.mass, self.C, self.W, self.Gc)
         return accel(t, self.theta, self.eps, self.G)[0]
 
     def step(self, dt: float):
@@ -327,18 +331,18 @@ class Stepper:
         with contacts out of scope nothing else acts between evaluations).
     """
 
-    def __init__(self, pos, vel, mass, theta, eps, G, leaf_cap, W=32, use_direct=False):
+    def __init__(self, pos, vel, mass, theta, eps, G, leaf_cap, W=R6_W, use_direct=False, Gc=R6_GC):
         self.pos = np.array(pos, dtype=np.float64, order="C")
         self.vel = np.array(vel, dtype=np.float64, order="C")
         self.mass = np.ascontiguousarray(mass, dtype=np.float64)
-        self.theta, self.eps, self.G, self.C, self.W = theta, eps, G, leaf_cap, W
+        self.theta, self.eps, self.G, self.C, self.W, self.Gc = theta, eps, G, leaf_cap, W, Gc
         self.use_direct = use_direct
         self.acc = None
 
     def _eval(self):
         if self.use_direct:
             return direct(self.pos, self.mass, self.eps, self.G)
-        t = build(self.pos, self.mass, self.C, self.W)
+        t = build(self.pos, self.mass, self.C, self.W, self.Gc)
         return accel(t, self.theta, self.eps, self.G)[0]
 
     def euler(self, dt: float):
