@@ -13,7 +13,9 @@ value   = body-accelerations per second = n_gpus * N * K / (sum of the K per-ste
           ranks.  Inputs are resident in HBM.
 e2e     = the same metric through bh_eval_host: pinned host pos/mass in, acc out, copies timed.
 roofline= the walk kernel (dominant): 20 flops per body-source interaction over its
-          CUDA-event duration, against the fp64 FMA peak 148 SM x 64 lanes x 2 x 1.965 GHz.
+          CUDA-event duration, against the fp64 FMA rate MEASURED in the same run (libbh_microbench.so;
+          MEASURED_PEAKS.json has no fp64 entry); the nominal 148 SM x 64 lanes x 2 x 1.965 GHz beside it.
+          traffic and l2_hit_rate are profiler figures read from profiles/r02_roofline.csv (ncu --set full).
 cpu_baseline = the oracle as it stands on the host cores, on a bounded sample of the same workload.
 
 Multi-GPU: the path does not shard (north_star: one GPU, no collectives) -> replicas only; every
@@ -35,15 +37,52 @@ sys.path.insert(0, ROOT)
 METRIC = "BH accel evals/s (build+walk) N=1M theta=0.5 fp64; speedup vs direct N^2"
 UNIT = "body-accelerations/s"
 FLOPS_PER_INTERACTION = 20.0
-FP64_PEAK_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12      # derived: SMs x fp64 FMA lanes x 2 x max SM clock
-# dram__bytes_read.sum + dram__bytes_write.sum of one walk_kernel launch, from the committed ncu --set full
-# capture (profiles/r01_walk_ncu_full.md: 65.32 MB + 15.84 MB); a profiler figure, not measured by this run
-WALK_TRAFFIC_NCU = {"c4": 81.15e6}
+FP64_NOMINAL_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12   # nominal: SMs x fp64 FMA lanes x 2 x max SM clock
+PROFILE_CSV = os.path.join(ROOT, "profiles", "r02_roofline.csv")
 
 
 def workload_desc(w):
     return (f"{w.name}: N={w.n} {w.note}, G={w.G:g}, eps={w.eps:g}, theta={w.theta:g}, leaf cap {w.leaf_cap}, "
             f"W=32, Gc=512, KDK dt={w.dt:g}")
+
+
+def profile_row(kernel: str, config: str):
+    """Profiler figures of one kernel launch (dram bytes, L2 hit rate, ...) from the committed summary of the
+    ncu --set full captures, profiles/r02_roofline.csv (its .md names the commands and the commit)."""
+    import csv
+    try:
+        with open(PROFILE_CSV) as f:
+            for row in csv.DictReader(f):
+                if row["kernel"] == kernel and row["config"] == config:
+                    return row
+    except OSError:
+        pass
+    return None
+
+
+class Microbench:
+    """libbh_microbench.so: measurement-only kernels (fp64 FMA rate, the walk's evaluation loop alone)."""
+
+    def __init__(self):
+        import ctypes as C
+        from paper_1912_04197_b200 import build as pbuild
+        self.C = C
+        self.lib = C.CDLL(pbuild.MICRO_LIB)
+        for name in ("bhmb_fp64_peak", "bhmb_issue_model"):
+            getattr(self.lib, name).restype = C.c_int
+            getattr(self.lib, name).argtypes = [C.c_void_p, C.POINTER(C.c_double)]
+
+    def fp64_peak(self, stream) -> float:
+        v = self.C.c_double()
+        if self.lib.bhmb_fp64_peak(stream.cuda_stream, self.C.byref(v)) != 0:
+            raise RuntimeError("bhmb_fp64_peak failed")
+        return v.value
+
+    def issue_model(self, stream):
+        v = (self.C.c_double * 3)()
+        if self.lib.bhmb_issue_model(stream.cuda_stream, v) != 0:
+            raise RuntimeError("bhmb_issue_model failed")
+        return {"eval_loop_alone": v[0], "beside_low_duty_integer_warps": v[1], "beside_full_rate_integer_warps": v[2]}
 
 
 # ------------------------------------------------------------------------------------------ clocks
@@ -110,7 +149,7 @@ def oracle_sample(w, budget_s: float, seed: int = 0):
     orc.accel(t, w.theta, w.eps, w.G, g0, min(ng, g0 + cal))
     per_group = (time.perf_counter() - t0) / cal
     want = int(max(cal, min(ng, budget_s / max(per_group, 1e-9))))
-    rng = np.random.default_rng(seed)
+    rng = np.random.default_rng(1912041970 + seed)    # fixed: the same chunks in every run with the same budget
     # contiguous chunks of 32 groups at random offsets (the oracle API walks ranges)
     chunks = max(1, want // 32)
     starts = rng.choice(max(1, ng - 32), size=chunks, replace=False) if ng > 64 else np.array([0])
@@ -124,8 +163,57 @@ def oracle_sample(w, budget_s: float, seed: int = 0):
     frac = bodies / w.n
     value = bodies / (t_build * frac + t_walk)
     desc = (f"oracle build of all N={w.n} bodies ({t_build:.2f} s, prorated) + walk of {bodies} bodies in "
-            f"{len(starts)} chunks of 32 groups ({t_walk:.2f} s)")
+            f"{len(starts)} chunks of 32 groups at seeded offsets (seed 1912041970+{seed}; the count follows a "
+            f"{budget_s:g} s budget calibrated on {cal} groups) ({t_walk:.2f} s)")
     return value, desc, cores
+
+
+def oracle_context(w, budget_s: float = 10.0):
+    """The two oracle timings SURVEY.md 8(d) lists for scale beside the headline (PAPER.md:194-197 gives the paper's
+    own CPU/GPU context): (i) the oracle on ONE thread at configs[2] (N = 131072, theta = 0.5), bounded sample;
+    (ii) the oracle's direct sum, Eq. (1), on 4096 targets of this workload, the full N^2 time extrapolated
+    x N/4096 and labelled so."""
+    import ctypes as C
+    import numpy as np
+    from oracle import bh_oracle as orc
+    from paper_1912_04197_b200 import workloads as wl
+    out = {}
+    cores = orc.num_threads()
+    gomp = None
+    try:
+        gomp = C.CDLL("libgomp.so.1")
+        gomp.omp_set_num_threads(1)
+        w3 = wl.make("c3")
+        t0 = time.perf_counter()
+        t3 = orc.build(w3.pos, w3.mass, w3.leaf_cap)
+        tb = time.perf_counter() - t0
+        ng = t3.ngroups
+        step = 4
+        t0 = time.perf_counter()
+        bodies = 0
+        for g0 in range(0, ng, step):                   # every step-th group until the budget is spent
+            orc.accel(t3, 0.5, w3.eps, w3.G, g0, g0 + 1)
+            bodies += int(t3.gstart[g0 + 1] - t3.gstart[g0])
+            if time.perf_counter() - t0 > budget_s:
+                break
+        tw = time.perf_counter() - t0
+        out["single_thread_c3"] = {"value": bodies / (tb * bodies / w3.n + tw), "unit": UNIT, "cores": 1,
+                                   "sample": f"c3 N={w3.n} theta=0.5: full build ({tb:.2f} s, prorated) + walk of {bodies} "
+                                             f"bodies (every {step}-th group, {tw:.2f} s)"}
+    except OSError:
+        out["single_thread_c3"] = None
+    finally:
+        if gomp is not None:
+            gomp.omp_set_num_threads(cores)
+    nt = min(4096, w.n)
+    tg = np.arange(0, w.n, max(1, w.n // nt), dtype=np.int32)[:nt]
+    t0 = time.perf_counter()
+    orc.direct(w.pos, w.mass, w.eps, w.G, targets=tg)
+    td = time.perf_counter() - t0
+    out["direct_sum"] = {"targets": int(nt), "seconds": td, "interactions_per_s": nt * float(w.n) / td, "cores": cores,
+                         "full_n2_seconds_extrapolated": td * w.n / nt, "extrapolated": nt != w.n,
+                         "body_accelerations_per_s": nt / td}
+    return out
 
 
 def run_reference(args):
@@ -309,19 +397,24 @@ def run_own(args):
     walk_avg_ms = sum(walk_ms) / nph
     inter_avg = sum(inter) / nph
     achieved = FLOPS_PER_INTERACTION * inter_avg / (walk_avg_ms * 1e-3) / 1e12
-    peak_meas = bh.bh_measure_fp64_peak(ctx.ctx)
-    issue = bh.bh_measure_issue_model(ctx.ctx)
-    roofline = {"bound": "alu", "kernel": "walk_kernel", "achieved": achieved, "peak": FP64_PEAK_TFLOPS,
-                "unit": "TFLOP/s", "frac": achieved / FP64_PEAK_TFLOPS,
-                "peak_source": "derived 148 SM x 64 fp64 FMA lanes x 2 x 1.965 GHz (DESIGN.md); "
-                               "MEASURED_PEAKS.json has no fp64 entry",
-                "peak_measured_dfma": peak_meas, "frac_of_measured_dfma": achieved / peak_meas,
+    mb = Microbench()
+    peak_meas = mb.fp64_peak(stream)
+    issue = mb.issue_model(stream)
+    prof = profile_row("walk_kernel", w.name)
+    roofline = {"bound": "alu", "kernel": "walk_kernel", "achieved": achieved, "peak": peak_meas,
+                "unit": "TFLOP/s", "frac": achieved / peak_meas,
+                "peak_source": "fp64 FMA rate measured in this run (register-resident DFMA chains on every SM, "
+                               "libbh_microbench.so); MEASURED_PEAKS.json has no fp64 entry",
+                "peak_nominal": FP64_NOMINAL_TFLOPS, "frac_of_nominal": achieved / FP64_NOMINAL_TFLOPS,
                 "flops_per_interaction": FLOPS_PER_INTERACTION, "interactions_per_launch": inter_avg,
                 "interactions_per_s": inter_avg / (walk_avg_ms * 1e-3), "kernel_ms": walk_avg_ms,
                 "issue_model_interactions_per_s": issue,
                 "frac_of_eval_loop_alone": inter_avg / (walk_avg_ms * 1e-3) / issue["eval_loop_alone"],
-                "traffic": args.walk_traffic if args.walk_traffic is not None else WALK_TRAFFIC_NCU.get(w.name),
-                "traffic_source": "profiles/r01_walk_ncu_full.md (ncu --set full, bytes per launch)"}
+                "traffic": float(prof["dram_bytes_per_launch"]) if prof else None,
+                "l2_hit_rate": float(prof["l2_hit_pct"]) / 100.0 if prof else None,
+                "fp64_pipe_active": float(prof["fp64_pipe_pct"]) / 100.0 if prof else None,
+                "profile_source": (f"profiles/r02_roofline.csv (ncu --set full at commit {prof['commit']}; profiler "
+                                   "figures, not measured by this run)") if prof else None}
     # build kernels against HBM: algorithmic bytes per body over the build time
     build_ms = sum(phases[k] for k in ("cube", "keys", "sort", "gather", "tree", "monopoles"))
     build_bytes = 390.0 * w.n
@@ -359,10 +452,15 @@ def run_own(args):
         dms = a.elapsed_time(b)
         direct_full_ms = dms * w.n / tg.numel()
         pairs = float(tg.numel()) * w.n
+        dprof = profile_row("direct_kernel", w.name)
+        dtf = FLOPS_PER_INTERACTION * pairs / (dms * 1e-3) / 1e12
         out["direct"] = {"targets": int(tg.numel()), "ms": dms, "full_n2_ms": direct_full_ms,
                          "extrapolated": tg.numel() != w.n, "interactions_per_s": pairs / (dms * 1e-3),
-                         "tflops": FLOPS_PER_INTERACTION * pairs / (dms * 1e-3) / 1e12,
-                         "frac_of_fp64_peak": FLOPS_PER_INTERACTION * pairs / (dms * 1e-3) / 1e12 / FP64_PEAK_TFLOPS}
+                         "roofline": {"bound": "alu", "kernel": "direct_kernel", "achieved": dtf, "peak": peak_meas,
+                                      "unit": "TFLOP/s", "frac": dtf / peak_meas, "frac_of_nominal": dtf / FP64_NOMINAL_TFLOPS,
+                                      "traffic": float(dprof["dram_bytes_per_launch"]) if dprof else None,
+                                      "l2_hit_rate": float(dprof["l2_hit_pct"]) / 100.0 if dprof else None,
+                                      "fp64_pipe_active": float(dprof["fp64_pipe_pct"]) / 100.0 if dprof else None}}
         out["speedup_vs_direct"] = direct_full_ms / (total_ms / args.steps)
 
         # ---- end to end through the C ABI with host buffers ----
@@ -377,8 +475,8 @@ def run_own(args):
             bh.bh_eval_host(ctx.ctx, ph, mh, w.theta, w.eps, w.G, ah)   # synchronising call
         te = (time.perf_counter() - t0) / ke
         out["e2e"] = {"value": w.n / te, "unit": UNIT, "h2d_bytes_per_step": 32 * w.n, "d2h_bytes_per_step": 24 * w.n,
-                      "ms_per_step": te * 1e3, "call": "bh_eval_host (pinned host pos+mass in, acc out; mass upload beside the first build kernels, "
-                              "accelerations stored by the walk kernel straight into the pinned output)"}
+                      "ms_per_step": te * 1e3, "call": "bh_eval_host (pinned host pos+mass in, acc out; mass upload beside the "
+                              "first build kernels; one code path, no state between calls)"}
 
         # ---- rows "next" of SURVEY.md 8(f), timed beside the headline ----
         if not args.no_next:
@@ -388,6 +486,8 @@ def run_own(args):
         if not args.no_cpu:
             v, desc, cores = oracle_sample(w, args.cpu_budget)
             out["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc}
+            if not args.no_cpu_context:
+                out["cpu_baseline"]["context"] = oracle_context(w)
         print(json.dumps(out), flush=True)
     ctx.close()
     if world > 1:
@@ -407,8 +507,8 @@ def main():
     ap.add_argument("--no-cpu", action="store_true", help="skip the oracle leg")
     ap.add_argument("--no-next", action="store_true", help="skip the timings of the SURVEY 8(f) 'next' rows")
     ap.add_argument("--cpu-budget", type=float, default=15.0, help="seconds of oracle work for cpu_baseline")
-    ap.add_argument("--walk-traffic", type=float, default=None,
-                    help="dram bytes per walk launch from the committed ncu capture (profiles/)")
+    ap.add_argument("--no-cpu-context", action="store_true",
+                    help="skip the two extra oracle timings (single thread at c3, direct sum on 4096 targets)")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)

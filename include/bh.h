@@ -17,8 +17,14 @@
  *     the next synchronising call.  bh_last_error() gives a human-readable message.
  *   - Ownership: the caller owns every buffer it passes, including the workspace; the library
  *     allocates no device memory except a few bytes of pinned host memory at bh_create.
- *   - Preconditions that are not checked: masses finite and > 0 (R15); |coordinate| < 2^1000 and the
- *     largest extent either 0 or >= 2^-900.
+ *   - Range of the input.  Checked on the GPU (sticky BH_ERR_NONFINITE / BH_ERR_INVALID_ARG): every
+ *     coordinate finite; the largest extent E = max over axes of (max - min) either 0 or in
+ *     [2^-300, 2^300] (the squares of cell edges and distances that the opening test compares, Eq. (3)
+ *     PAPER.md:86, then stay normal doubles down to level 21).  Not checked: masses finite and > 0 (R15),
+ *     and such that m x (Eq. (2)) and m / r^3 (Eq. (6)) are representable for the coordinates and
+ *     distances that occur.  A pair whose softened squared
+ *     distance |d|^2 + eps^2 is below the smallest normal double (2.2e-308; eps = 0 with coincident
+ *     bodies is the usual case) contributes nothing (R13).
  */
 #ifndef BH_H_
 #define BH_H_
@@ -42,23 +48,34 @@ typedef enum {
 } bh_status;
 
 #define BH_MAX_LEVEL 21    /* 63-bit Morton keys, 3 bits per level (R9) */
-#ifndef BH_GROUP_CELL
-#define BH_GROUP_CELL 512  /* Gc: walk groups never straddle a tree cell holding <= Gc bodies (R6) */
-#endif
+/* Reading R6: W bodies walk the tree together (bh_create group_size, default 32),
+ * and a group never straddles a tree cell that holds <= Gc bodies (bh_set_group_cell).  Both are parameters
+ * of the method: the oracle takes them as arguments too, and parity is tested at several (W, Gc). */
+#define BH_GROUP_SIZE_DEFAULT 32
+#define BH_GROUP_CELL_DEFAULT 512
+#define BH_NUM_STATS 5
 
 /* Bytes of device workspace a context for up to max_n bodies needs.  0 if the arguments are invalid
- * (max_n < 1 or > 2^30, leaf_cap < 1 or > 1024, group_size not 0 or 32). */
+ * (max_n < 1 or > 2^30, leaf_cap < 1 or > 1024, group_size < 0 or > 32).  Depends on the number of
+ * multiprocessors of the current CUDA device: query it on the device the context will be created on. */
 size_t bh_workspace_bytes(int64_t max_n, int leaf_cap, int group_size);
 
 /* Create a context.  leaf_cap = C: a node is a leaf iff it holds <= C bodies or sits at level 21
  * (PAPER.md:62 subdivides "until each node ... contains zero or one particle" = C 1; R8).
- * group_size = W, the most bodies that walk the tree together (0 or 32; R6).  workspace_dev must hold
+ * group_size = W, the most bodies that walk the tree together: 1..32, 0 = 32 (R6).  W = 1 is the paper's
+ * own per-body walk ("for each body-node pair", 118 "each body is assigned to a thread"): one warp
+ * per body, slow, there to quantify the group reading against it.  workspace_dev must hold
  * bh_workspace_bytes() bytes, be 256-byte aligned and stay valid until bh_destroy.  cuda_stream is a
  * cudaStream_t (NULL = the legacy default stream). */
 bh_status bh_create(bh_ctx **out, int64_t max_n, int leaf_cap, int group_size, void *workspace_dev,
                     size_t workspace_bytes, void *cuda_stream);
 bh_status bh_destroy(bh_ctx *ctx);
 bh_status bh_set_stream(bh_ctx *ctx, void *cuda_stream);
+
+/* Group-cell capacity Gc of reading R6, 1..2048 (default BH_GROUP_CELL_DEFAULT): a group cell is a tree node
+ * holding <= Gc bodies (or a leaf) whose parent holds more; group cells tile the sorted bodies and each is cut
+ * into runs of W.  Takes effect at the next build. */
+bh_status bh_set_group_cell(bh_ctx *ctx, int group_cell);
 
 /* Build the octree of the n bodies ("re-built at each time step"):
  * bounding cube -> 63-bit Morton keys -> stable LSD radix sort -> sorted (x,y,z,m) bodies and group
@@ -182,13 +199,9 @@ bh_status bh_aggregates(bh_ctx *ctx, int64_t n, const int32_t *pairs_dev, int64_
 double bh_gravity_dt(double G, double rho);
 
 /* End-to-end evaluation from HOST buffers: copies pos_host [n][3] and mass_host [n] to the GPU,
- * builds, walks, delivers acc_host [n][3] and waits.  Pinned host memory makes the copies asynchronous;
- * pageable memory works too.  The masses travel on a second stream beside the first build kernels (they
- * are first needed after the sort).  If acc_host is pinned (cudaHostAlloc / cudaHostRegister, e.g. a torch
- * pin_memory() tensor) and the previous evaluation through this call had at least 3400 interactions per
- * body (so that 24 bytes per body stay below what small PCIe writes sustain), the walk kernel stores the
- * accelerations straight into it while it computes and no copy follows; otherwise they are staged in the
- * workspace and copied (environment BH_HOST_DIRECT=0 forces the staged path, for measurements). */
+ * builds, walks, copies the accelerations to acc_host [n][3] and waits.  Pinned host memory makes the
+ * copies asynchronous; pageable memory works too.  The masses travel on a second stream beside the first
+ * build kernels (they are first needed after the sort).  One code path, no state carried between calls. */
 bh_status bh_eval_host(bh_ctx *ctx, const double *pos_host, const double *mass_host, int64_t n,
                        double theta, double eps, double G, double *acc_host);
 
@@ -207,7 +220,7 @@ bh_status bh_get_node_count(bh_ctx *ctx, int64_t *m_host, int32_t *depth_host);
 bh_status bh_get_nodes(bh_ctx *ctx, uint8_t *level_dev, uint32_t *begin_dev, uint32_t *count_dev,
                        int32_t *first_child_dev, uint8_t *child_mask_dev, int32_t *parent_dev,
                        double *mono_dev);
-/* Synchronising. Walk groups (R6): a group cell is a tree node with <= BH_GROUP_CELL bodies (or a
+/* Synchronising. Walk groups (R6): a group cell is a tree node with <= Gc bodies (or a
  * leaf) whose parent has more; each group cell is cut into runs of W consecutive sorted bodies;
  * groups are numbered in sorted-body order.  *ng_host = number of groups Ng; gstart_dev (may be
  * NULL, else room for Ng+1 <= n+1 entries) receives the first sorted body of each group, then n. */
@@ -219,8 +232,9 @@ bh_status bh_get_counts(bh_ctx *ctx, uint32_t *n_mono_per_group_dev, uint32_t *n
 
 /* Synchronising. Totals of the last bh_accel: stats[0] = sum over groups of n_mono, stats[1] = sum
  * of n_direct, stats[2] = body-source interactions evaluated (sum of group bodies x list length),
- * stats[3] = nodes tested by the opening criterion. */
-bh_status bh_get_stats(bh_ctx *ctx, uint64_t stats_host[4]);
+ * stats[3] = nodes tested by the opening criterion, stats[4] = times a traversal stack outgrew shared
+ * memory and spilled 128 entries to the workspace (deep or wide traversals: small theta). */
+bh_status bh_get_stats(bh_ctx *ctx, uint64_t stats_host[BH_NUM_STATS]);
 
 /* Number of CUDA kernels this context has launched since bh_create (memsets and copies excluded). */
 bh_status bh_get_launches(bh_ctx *ctx, uint64_t *count_host);
@@ -232,19 +246,6 @@ bh_status bh_get_launches(bh_ctx *ctx, uint64_t *count_host);
 #define BH_NUM_PHASES 9
 bh_status bh_set_timing(bh_ctx *ctx, int enable);
 bh_status bh_get_phase_ms(bh_ctx *ctx, float ms_host[BH_NUM_PHASES]);
-
-/* fp64 FMA throughput microbenchmark (register-resident DFMA chains on every SM): returns the
- * measured TFLOP/s (2 flops per FMA) in *tflops_host.  The roofline denominator of the walk and
- * direct kernels.  Synchronising. */
-bh_status bh_measure_fp64_peak(bh_ctx *ctx, double *tflops_host);
-
-/* Synchronising microbenchmark behind the walk kernel's roofline statement: the walk's own
- * evaluation loop (two evaluating warps per SM sub-partition, four bodies per lane, sources in shared memory)
- * in body-source interactions per second  [0] with nothing else on the sub-partition,  [1] beside two warps per
- * sub-partition running a dependent integer / shared-memory chain at low duty (what the walk's traversal warps
- * look like),  [2] beside two warps issuing independent integer instructions at full rate.  [0] is the ceiling
- * of a warp-specialised walk; [0] - [1] is what co-resident traversal warps cost the fp64 warps. */
-bh_status bh_measure_issue_model(bh_ctx *ctx, double out_host[3]);
 
 const char *bh_last_error(const bh_ctx *ctx);
 const char *bh_version(void);

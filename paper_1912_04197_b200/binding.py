@@ -78,8 +78,7 @@ def lib() -> C.CDLL:
             "bh_get_launches": [vp, C.POINTER(C.c_uint64)],
             "bh_set_timing": [vp, i32],
             "bh_get_phase_ms": [vp, C.POINTER(C.c_float)],
-            "bh_measure_fp64_peak": [vp, C.POINTER(dbl)],
-            "bh_measure_issue_model": [vp, C.POINTER(dbl)],
+            "bh_set_group_cell": [vp, i32],
         }
         for name, args in sigs.items():
             f = getattr(L, name)
@@ -94,10 +93,10 @@ EXPORTS = ("bh_workspace_bytes", "bh_create", "bh_destroy", "bh_set_stream", "bh
            "bh_eval_host", "bh_synchronize", "bh_get_cube", "bh_get_keys", "bh_get_node_count",
            "bh_get_nodes", "bh_get_groups", "bh_get_bodies", "bh_get_counts", "bh_get_stats", "bh_get_launches",
            "bh_set_timing",
-           "bh_get_phase_ms", "bh_measure_fp64_peak", "bh_last_error", "bh_version",
+           "bh_get_phase_ms", "bh_set_group_cell", "bh_last_error", "bh_version",
            "bh_euler_step", "bh_multirate_step", "bh_potential", "bh_direct_potential", "bh_diagnostics",
            "bh_position_error", "bh_gravity_dt", "bh_copy_state_acc", "bh_set_gravity_method",
-           "bh_broadphase", "bh_aggregates", "bh_set_graph", "bh_accel_potential", "bh_measure_issue_model")
+           "bh_broadphase", "bh_aggregates", "bh_set_graph", "bh_accel_potential")
 
 
 def _check(ctx, status: int):
@@ -144,6 +143,10 @@ def bh_destroy(ctx):
 
 def bh_set_stream(ctx, stream):
     _check(ctx, lib().bh_set_stream(ctx, _stream_ptr(stream)))
+
+
+def bh_set_group_cell(ctx, group_cell: int):
+    _check(ctx, lib().bh_set_group_cell(ctx, group_cell))
 
 
 def bh_build(ctx, pos: torch.Tensor, mass: torch.Tensor):
@@ -299,9 +302,9 @@ def bh_get_counts(ctx, n_mono=None, n_direct=None):
 
 
 def bh_get_stats(ctx):
-    s = (C.c_uint64 * 4)()
+    s = (C.c_uint64 * 5)()
     _check(ctx, lib().bh_get_stats(ctx, s))
-    return {"n_mono": s[0], "n_direct": s[1], "interactions": s[2], "nodes_tested": s[3]}
+    return {"n_mono": s[0], "n_direct": s[1], "interactions": s[2], "nodes_tested": s[3], "stack_spills": s[4]}
 
 
 def bh_get_launches(ctx) -> int:
@@ -320,25 +323,14 @@ def bh_get_phase_ms(ctx):
     return {PHASE_NAMES[i]: ms[i] for i in range(NUM_PHASES)}
 
 
-def bh_measure_fp64_peak(ctx) -> float:
-    v = C.c_double()
-    _check(ctx, lib().bh_measure_fp64_peak(ctx, C.byref(v)))
-    return v.value
-
-
-def bh_measure_issue_model(ctx):
-    v = (C.c_double * 3)()
-    _check(ctx, lib().bh_measure_issue_model(ctx, v))
-    return {"eval_loop_alone": v[0], "beside_low_duty_integer_warps": v[1], "beside_full_rate_integer_warps": v[2]}
-
-
 # ---- convenience owner of a context and its torch-allocated workspace (no arithmetic) ----
 class Context:
-    def __init__(self, max_n: int, leaf_cap: int, group_size: int = 0, device="cuda:0", stream=None):
+    def __init__(self, max_n: int, leaf_cap: int, group_size: int = 0, device="cuda:0", stream=None,
+                 group_cell: int | None = None):
         if not torch.cuda.is_available():
             raise RuntimeError("libbh needs a CUDA device; there is no CPU fallback")
         self.device = torch.device(device)
-        self.max_n, self.leaf_cap, self.W = max_n, leaf_cap, 32
+        self.max_n, self.leaf_cap, self.W = max_n, leaf_cap, group_size or 32
         nbytes = bh_workspace_bytes(max_n, leaf_cap, group_size)
         if nbytes == 0:
             raise BhError(BH_ERR_INVALID_ARG, "max_n, leaf_cap or group_size out of range")
@@ -347,6 +339,8 @@ class Context:
             off = (-self.workspace.data_ptr()) % 256
             self._ws = self.workspace[off:off + nbytes]
             self.ctx = bh_create(max_n, leaf_cap, group_size, self._ws, stream)
+            if group_cell is not None:
+                bh_set_group_cell(self.ctx, group_cell)
         self.n = 0
 
     def close(self):

@@ -8,6 +8,7 @@ import subprocess
 HERE = os.path.dirname(os.path.abspath(__file__))
 ROOT = os.path.dirname(HERE)
 LIB = os.path.join(HERE, "libbh.so")
+MICRO_LIB = os.path.join(HERE, "libbh_microbench.so")   # measurement-only kernels, loaded by bench.py alone
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "--fmad=true", "-Xcompiler", "-fPIC", "-shared", "-cudart", "static"]
 
@@ -16,8 +17,12 @@ def sources():
     return sorted(glob.glob(os.path.join(HERE, "csrc", "*.cu")))
 
 
+def micro_sources():
+    return sorted(glob.glob(os.path.join(HERE, "csrc", "bench", "*.cu")))
+
+
 def _deps():
-    return sources() + glob.glob(os.path.join(HERE, "csrc", "*.cuh")) + \
+    return sources() + micro_sources() + glob.glob(os.path.join(HERE, "csrc", "*.cuh")) + \
         glob.glob(os.path.join(ROOT, "include", "*.h"))
 
 
@@ -25,13 +30,26 @@ def build(force: bool = False, verbose: bool = False) -> str:
     deps = _deps()
     if not sources():
         raise FileNotFoundError('no CUDA sources under csrc/')
-    if not force and os.path.exists(LIB) and all(os.path.getmtime(LIB) >= os.path.getmtime(d) for d in deps):
+    if not force and all(os.path.exists(lib) and all(os.path.getmtime(lib) >= os.path.getmtime(d) for d in deps)
+                         for lib in (LIB, MICRO_LIB)):
         return LIB
     nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
-    extra = os.environ.get("BH_NVCC_EXTRA", "").split()       # e.g. -DBH_WALK_PROF, for experiments
-    cmd = [nvcc] + NVCC_FLAGS + extra + (["-Xptxas", "-v"] if verbose else []) + \
-        ["-I", os.path.join(ROOT, "include"), "-o", LIB] + sources()
-    subprocess.run(cmd, check=True)
+    extra = os.environ.get("BH_NVCC_EXTRA", "").split()       # extra nvcc flags, e.g. -DBH_TRIP_UNROLL=2
+    flags = [f for f in NVCC_FLAGS if f != "-shared"] + extra + (["-Xptxas", "-v"] if verbose else []) + \
+        ["-I", os.path.join(ROOT, "include")]
+    objdir = os.path.join(HERE, "build")
+    os.makedirs(objdir, exist_ok=True)
+    # one nvcc per translation unit, all at once (no relocatable device code: kernels share nothing but headers)
+    jobs = []
+    for src in sources() + micro_sources():
+        obj = os.path.join(objdir, os.path.basename(src)[:-3] + ".o")
+        jobs.append((src, obj, subprocess.Popen([nvcc] + flags + ["-c", "-o", obj, src])))
+    if any(j.wait() != 0 for _, _, j in jobs):
+        raise RuntimeError("nvcc failed")
+    objs = {src: obj for src, obj, _ in jobs}
+    link = [nvcc, "-gencode", "arch=compute_100a,code=sm_100a", "-shared", "-cudart", "static", "-Xcompiler", "-fPIC"]
+    subprocess.run(link + ["-o", LIB] + [objs[x] for x in sources()], check=True)
+    subprocess.run(link + ["-o", MICRO_LIB] + [objs[x] for x in micro_sources()], check=True)
     return LIB
 
 

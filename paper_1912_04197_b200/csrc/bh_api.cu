@@ -12,7 +12,8 @@ using namespace bh;
 struct bh_ctx {
     int64_t max_n = 0;
     int leaf_cap = 0;
-    int group = kGroup;
+    int group = kMaxGroup;   // W
+    int group_cell = BH_GROUP_CELL_DEFAULT;   // Gc
     cudaStream_t stream = nullptr;
     Workspace ws{};
     int64_t n = 0;          // bodies of the last build
@@ -46,8 +47,6 @@ struct bh_ctx {
     };
     cudaStream_t copy_stream = nullptr;   // bh_eval_host: mass upload beside the first build kernels
     cudaEvent_t ev_copy[2]{};
-    bool host_direct = true;              // bh_eval_host: store accelerations straight into pinned host memory ...
-    double last_host_ipb = 0.0;           // ... when the previous evaluation had this many interactions per body
     bool use_graph = false;
     cudaGraphExec_t graph_exec = nullptr;
     StepSig graph_sig{}, seen_sig{};
@@ -111,9 +110,14 @@ bh_status fetch_state(bh_ctx *c)   // synchronising
     if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
     if (e != cudaSuccess) return cuda_check(c, e, "state readback");
     const int s = c->host_state->status;
+    if (s == 0) return BH_OK;
+    // sticky until reported: the device word is cleared now that the caller is being told
+    cudaMemsetAsync(&c->ws.st->status, 0, sizeof(int), c->stream);
     if (s & kStatNonFinite) return fail(c, BH_ERR_NONFINITE, "a body coordinate is NaN or infinite");
+    if (s & kStatRange) return fail(c, BH_ERR_INVALID_ARG, "largest extent of the bodies outside [2^-300, 2^300]");
     if (s & kStatCapacity) return fail(c, BH_ERR_CAPACITY, "node array overflow");
     if (s & kStatStack) return fail(c, BH_ERR_CAPACITY, "walk stack overflow");
+    if (s & kStatBpStack) return fail(c, BH_ERR_CAPACITY, "broad-phase search stack overflow");
     return BH_OK;
 }
 
@@ -124,7 +128,11 @@ bh_status do_build(bh_ctx *c, const double *pos, const double *mass, int64_t n, 
     c->built = false;
     c->walked = false;
     int sort_launches = 0;
-    cudaMemsetAsync(w.zero_begin, 0, w.zero_bytes, s);
+    // cleared per build, sized by n (not by max_n): histograms + tickets + look-back words of this n's tiles,
+    // and the child masks / arrival counters of the nodes n bodies can make
+    const int64_t tiles = (n + kSortTile - 1) / kSortTile;
+    cudaMemsetAsync(w.zero_begin, 0, (size_t)((char *)w.lookback - (char *)w.zero_begin) + (size_t)kSortPasses * tiles * kRadix * sizeof(unsigned), s);
+    cudaMemsetAsync(w.node_meta, 0, (size_t)node_capacity(n, c->leaf_cap) * sizeof(unsigned), s);
     {
         Phase p(c, 0);
         launch_cube(w, pos, n, s);
@@ -163,7 +171,7 @@ bh_status do_accel(bh_ctx *c, double theta, double eps, double G, double *acc, i
     const Workspace &w = c->ws;
     // reset the group queue and the counters of this evaluation
     cudaMemsetAsync(&w.st->walk_queue, 0, sizeof(unsigned), c->stream);
-    cudaMemsetAsync(&w.st->stats[0], 0, 4 * sizeof(unsigned long long), c->stream);
+    cudaMemsetAsync(&w.st->stats[0], 0, kNumStats * sizeof(unsigned long long), c->stream);
     {
         Phase p(c, 6);
         launch_walk(w, c->n, theta, eps, G, acc, mode, phi, c->stream);
@@ -208,7 +216,7 @@ bh_status run_stepper(bh_ctx *c, int kind, double dt, int n_sub, F enqueue)
     sig.kind = kind; sig.n_sub = n_sub; sig.dt = dt; sig.theta = c->theta; sig.eps = c->eps; sig.G = c->G;
     sig.pos = c->pos; sig.vel = c->vel; sig.mass = c->mass; sig.n = c->bound_n; sig.direct = c->use_direct;
     sig.stream = c->stream;
-    if (c->graph_exec && sig == c->graph_sig) {
+    if (c->graph_exec && sig == c->graph_sig) {   // the callers refresh built / walked / n (stepper_done)
         c->launches += c->graph_launches;
         return cuda_check(c, cudaGraphLaunch(c->graph_exec, c->stream), "stepper graph launch");
     }
@@ -247,18 +255,38 @@ bh_status run_stepper(bh_ctx *c, int kind, double dt, int n_sub, F enqueue)
 
 namespace bh {
 
+int sm_count()
+{
+    static int sms = 0;
+    if (sms == 0) {
+        int dev = 0, v = 0;
+        if (cudaGetDevice(&dev) == cudaSuccess &&
+            cudaDeviceGetAttribute(&v, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess && v > 0) {
+            sms = v;
+        } else {
+            cudaGetLastError();
+            return kDefaultSMs;   // no device (yet): not cached
+        }
+    }
+    return sms;
+}
+
 Workspace carve(char *base, int64_t max_n, int leaf_cap)
 {
     Workspace w{};
     Carver cv{base};
     const int64_t n = max_n;
+    w.sms = sm_count();
+    w.leaf_cap = leaf_cap;
+    w.group_w = kMaxGroup;
+    w.group_cell = BH_GROUP_CELL_DEFAULT;
     w.node_cap = node_capacity(n, leaf_cap);
     w.sort_tiles = (n + kSortTile - 1) / kSortTile;
     w.tree_tiles = (n + kTreeTile - 1) / kTreeTile;
-    w.walk_warps = WalkConfig::kSMs * WalkConfig::kPairsPerBlock;
+    w.walk_warps = w.sms * WalkConfig::kPairsPerBlock;
     const int64_t groups = n;   // capacity: a group holds at least one body
     w.st = cv.take<DevState>(1);
-    w.bbox_part = cv.take<double>(148 * 4 * 8);
+    w.bbox_part = cv.take<double>(kMaxBboxBlocks * 8);
     // --- region cleared by one memset at every build ---
     size_t z0 = cv.off;
     w.hist = cv.take<unsigned>(kSortPasses * kRadix);
@@ -292,7 +320,6 @@ Workspace carve(char *base, int64_t max_n, int leaf_cap)
     w.stage_pos = cv.take<double>(3 * n);
     w.stage_doubles = 3 * n;
     w.stage_mass = cv.take<double>(n);
-    w.peak_sink = cv.take<double>(32);
     w.diag_part = cv.take<double>((size_t)kDiagBlocks * 16);
     w.diag_out = cv.take<double>(16);
     w.diag_ticket = base ? &w.st->ticket_diag : nullptr;
@@ -316,7 +343,7 @@ const char *bh_last_error(const bh_ctx *ctx) { return ctx ? ctx->err : g_err; }
 static bool args_ok(int64_t max_n, int leaf_cap, int group_size)
 {
     return max_n >= 1 && max_n <= ((int64_t)1 << 30) && leaf_cap >= 1 && leaf_cap <= 1024 &&
-           (group_size == 0 || group_size == kGroup);
+           group_size >= 0 && group_size <= kMaxGroup;
 }
 
 size_t bh_workspace_bytes(int64_t max_n, int leaf_cap, int group_size)
@@ -341,8 +368,9 @@ bh_status bh_create(bh_ctx **out, int64_t max_n, int leaf_cap, int group_size, v
     c->max_n = max_n;
     c->leaf_cap = leaf_cap;
     c->stream = (cudaStream_t)cuda_stream;
+    c->group = group_size == 0 ? kMaxGroup : group_size;
+    w.group_w = c->group;
     c->ws = w;
-    if (const char *hd = getenv("BH_HOST_DIRECT")) c->host_direct = hd[0] != '0';   // A/B switch for measurements
     const size_t hs = (sizeof(DevState) + 63) & ~(size_t)63;
     cudaError_t e = cudaMallocHost((void **)&c->host_state, hs + 16 * sizeof(double));
     if (e == cudaSuccess) c->host_diag = reinterpret_cast<double *>(reinterpret_cast<char *>(c->host_state) + hs);
@@ -457,6 +485,20 @@ bh_status bh_bind_state(bh_ctx *c, double *pos_dev, double *vel_dev, const doubl
     return BH_OK;
 }
 
+bh_status bh_set_group_cell(bh_ctx *c, int group_cell)
+{
+    if (!c) return BH_ERR_INVALID_ARG;
+    if (group_cell < 1 || group_cell > kMaxGroupCell) return fail(c, BH_ERR_INVALID_ARG, "bh_set_group_cell: Gc out of range");
+    c->group_cell = group_cell;
+    c->ws.group_cell = group_cell;
+    c->seen_sig = bh_ctx::StepSig{};   // a captured stepper graph holds the old Gc as a kernel argument
+    if (c->graph_exec) {
+        cudaGraphExecDestroy(c->graph_exec);
+        c->graph_exec = nullptr;
+    }
+    return BH_OK;
+}
+
 bh_status bh_set_graph(bh_ctx *c, int enable)
 {
     if (!c) return BH_ERR_INVALID_ARG;
@@ -471,12 +513,26 @@ bh_status bh_set_graph(bh_ctx *c, int enable)
 
 static bh_status kdk_enqueue(bh_ctx *c, double dt);
 
+// Host-side view of the context after a stepper call, whichever way it ran (plain, captured or replayed
+// graph): a replay does on the device what a plain call does, so the flags must say the same.  Tree
+// method: the context holds the tree and the walk of the bound state's n bodies.  Direct method: the
+// sorted-body arrays were overwritten by the identity packing, so it holds no tree.
+static void stepper_done(bh_ctx *c, bool acc_is_current)
+{
+    c->have_acc = acc_is_current;
+    c->acc_filled = true;
+    c->n = c->bound_n;
+    c->built = c->walked = !c->use_direct;
+}
+
 bh_status bh_kdk_step(bh_ctx *c, double dt)
 {
     if (!c) return BH_ERR_INVALID_ARG;
     if (!c->bound) return fail(c, BH_ERR_STATE, "bh_kdk_step before bh_bind_state");
-    if (!c->have_acc) return kdk_enqueue(c, dt);   // the first step also evaluates a(x0): not the repeating pattern
-    return run_stepper(c, 0, dt, 0, [=]() { return kdk_enqueue(c, dt); });
+    // the first step also evaluates a(x0): not the repeating pattern
+    const bh_status st = !c->have_acc ? kdk_enqueue(c, dt) : run_stepper(c, 0, dt, 0, [=]() { return kdk_enqueue(c, dt); });
+    if (st == BH_OK) stepper_done(c, true);
+    return st;
 }
 
 static bh_status kdk_enqueue(bh_ctx *c, double dt)
@@ -507,10 +563,8 @@ static bh_status euler_like(bh_ctx *c, double dt, int n_sub, const char *who)
     if (!c) return BH_ERR_INVALID_ARG;
     if (!c->bound) return fail(c, BH_ERR_STATE, "stepper called before bh_bind_state");
     if (n_sub < 1) return fail(c, BH_ERR_INVALID_ARG, "n_sub < 1");
-    bh_status st = run_stepper(c, 1, dt, n_sub, [=]() { return euler_enqueue(c, dt, n_sub, who); });
-    c->have_acc = false;   // whatever path ran: acc is a(x_k)
-    c->acc_filled = true;
-    if (!c->use_direct) { c->built = true; c->walked = true; c->n = c->bound_n; }
+    const bh_status st = run_stepper(c, 1, dt, n_sub, [=]() { return euler_enqueue(c, dt, n_sub, who); });
+    if (st == BH_OK) stepper_done(c, false);   // acc is a(x_k), not a(x_k+1): a later bh_kdk_step re-evaluates
     return st;
 }
 
@@ -667,17 +721,6 @@ bh_status bh_copy_state_acc(bh_ctx *c, double *acc_dev)
                                          c->stream), "bh_copy_state_acc");
 }
 
-// device alias of a pinned (page-locked, mapped) host buffer, or nullptr for pageable memory
-static double *mapped_alias(const void *host)
-{
-    cudaPointerAttributes a{};
-    if (cudaPointerGetAttributes(&a, host) != cudaSuccess) {
-        cudaGetLastError();
-        return nullptr;
-    }
-    return a.type == cudaMemoryTypeHost ? static_cast<double *>(a.devicePointer) : nullptr;
-}
-
 bh_status bh_eval_host(bh_ctx *c, const double *pos_host, const double *mass_host, int64_t n, double theta,
                        double eps, double G, double *acc_host)
 {
@@ -687,9 +730,8 @@ bh_status bh_eval_host(bh_ctx *c, const double *pos_host, const double *mass_hos
     if (!(theta >= 0.0) || !(eps >= 0.0)) return fail(c, BH_ERR_INVALID_ARG, "bh_eval_host: theta or eps negative");
     const Workspace &w = c->ws;
     // The masses are first needed by the gather (after the sort): their copy runs on a second stream,
-    // beside cube / keys / sort.  It may start once the previous user of the staging buffer is done.
-    // It starts after the positions have arrived (one transfer at a time gets the whole link) and after
-    // the previous user of the staging buffer (stream order of the main stream up to the event).
+    // beside cube / keys / sort.  It starts after the positions have arrived (one transfer at a time gets
+    // the whole link) and after the previous user of the staging buffer (stream order up to the event).
     cudaError_t e = cudaMemcpyAsync(w.stage_pos, pos_host, 3 * n * sizeof(double), cudaMemcpyHostToDevice, c->stream);
     if (e == cudaSuccess) e = cudaEventRecord(c->ev_copy[0], c->stream);
     if (e == cudaSuccess) e = cudaStreamWaitEvent(c->copy_stream, c->ev_copy[0], 0);
@@ -699,23 +741,12 @@ bh_status bh_eval_host(bh_ctx *c, const double *pos_host, const double *mass_hos
     if (e != cudaSuccess) return cuda_check(c, e, "bh_eval_host H2D");
     bh_status st;
     if ((st = do_build(c, w.stage_pos, w.stage_mass, n, c->ev_copy[1])) != BH_OK) return st;
-    // Pinned output: the walk stores the accelerations straight into host memory (24 bytes per body,
-    // over PCIe while the kernel computes), so no copy follows it.  Pageable output: staged in the workspace.
-    // It pays only while the stores keep below what small PCIe writes sustain (~6 GB/s measured): 24 bytes
-    // per body against the walk's time per body, i.e. when a body has many interactions (configs[3]: 4100 per
-    // body, 4.9 GB/s, 6.74 -> 6.38 ms; configs[4]: 2100 per body, 9.5 GB/s, 15.7 -> 24.7 ms).  The count of the
-    // previous evaluation through this call decides; the first evaluation is staged.
-    double *direct_out = (c->host_direct && c->last_host_ipb >= 3400.0) ? mapped_alias(acc_host) : nullptr;
-    if ((st = do_accel(c, theta, eps, G, direct_out ? direct_out : w.acc)) != BH_OK) return st;
+    if ((st = do_accel(c, theta, eps, G, w.acc)) != BH_OK) return st;
     c->have_acc = false;   // the internal acc buffer no longer belongs to the bound state
     c->acc_filled = false;
-    if (!direct_out) {
-        e = cudaMemcpyAsync(acc_host, w.acc, 3 * n * sizeof(double), cudaMemcpyDeviceToHost, c->stream);
-        if (e != cudaSuccess) return cuda_check(c, e, "bh_eval_host D2H");
-    }
-    st = fetch_state(c);
-    if (st == BH_OK) c->last_host_ipb = (double)c->host_state->stats[2] / (double)n;
-    return st;
+    e = cudaMemcpyAsync(acc_host, w.acc, 3 * n * sizeof(double), cudaMemcpyDeviceToHost, c->stream);
+    if (e != cudaSuccess) return cuda_check(c, e, "bh_eval_host D2H");
+    return fetch_state(c);
 }
 
 bh_status bh_synchronize(bh_ctx *c)
@@ -829,13 +860,13 @@ bh_status bh_get_counts(bh_ctx *c, uint32_t *n_mono_dev, uint32_t *n_direct_dev)
     return cuda_check(c, e, "bh_get_counts");
 }
 
-bh_status bh_get_stats(bh_ctx *c, uint64_t stats_host[4])
+bh_status bh_get_stats(bh_ctx *c, uint64_t stats_host[BH_NUM_STATS])
 {
     if (!c || !stats_host) return BH_ERR_INVALID_ARG;
     if (!c->walked) return fail(c, BH_ERR_STATE, "no bh_accel since the last build");
     bh_status st = fetch_state(c);
     if (st != BH_OK) return st;
-    for (int k = 0; k < 4; ++k) stats_host[k] = c->host_state->stats[k];
+    for (int k = 0; k < kNumStats; ++k) stats_host[k] = c->host_state->stats[k];
     return BH_OK;
 }
 
@@ -864,21 +895,6 @@ bh_status bh_get_phase_ms(bh_ctx *c, float ms_host[BH_NUM_PHASES])
         if (c->ev_set[p]) cudaEventElapsedTime(&ms_host[p], c->ev[p][0], c->ev[p][1]);
     }
     return BH_OK;
-}
-
-bh_status bh_measure_fp64_peak(bh_ctx *c, double *tflops_host)
-{
-    if (!c || !tflops_host) return BH_ERR_INVALID_ARG;
-    *tflops_host = run_fp64_peak(c->ws, c->stream);
-    return cuda_check(c, cudaGetLastError(), "bh_measure_fp64_peak");
-}
-
-bh_status bh_measure_issue_model(bh_ctx *c, double out_host[3])
-{
-    if (!c || !out_host) return BH_ERR_INVALID_ARG;
-    run_issue_model(c->ws, out_host, c->stream);
-    c->launches += 6;
-    return cuda_check(c, cudaGetLastError(), "bh_measure_issue_model");
 }
 
 }  // extern "C"

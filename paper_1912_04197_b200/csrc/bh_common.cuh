@@ -10,8 +10,10 @@ namespace bh {
 
 constexpr int kMaxLevel = BH_MAX_LEVEL;   // 21
 constexpr int kLevels = kMaxLevel + 1;    // levels 0..21
-constexpr int kGroup = 32;                // W: bodies per walk group = one warp
-constexpr int kGroupCell = BH_GROUP_CELL;           // Gc: groups never straddle a tree cell that holds <= Gc bodies
+constexpr int kMaxGroup = 32;             // W <= 32: a walk group is evaluated by one warp (run-time, bh_create)
+constexpr int kMaxGroupCell = 2048;       // Gc <= 2048 (run-time, bh_set_group_cell): bounds the window scratch of the tree kernels
+constexpr int kMaxBboxBlocks = 1024;       // rows of the bounding-box partials
+constexpr int kDefaultSMs = 148;          // B200; the real count is queried once (sm_count())
 constexpr int kRadixBits = 8;
 constexpr int kRadix = 1 << kRadixBits;   // 256 bins
 constexpr int kSortPasses = 8;            // 63 key bits
@@ -22,10 +24,12 @@ constexpr int kSortThreads = 256;
 constexpr int kSortItems = BH_SORT_ITEMS;   // keys per thread
 constexpr int kSortTile = kSortThreads * kSortItems;   // 4096 keys per tile
 constexpr int kTreeTile = 1024;           // bodies per block in the tree kernels
-constexpr int kDiagBlocks = 148 * 4;       // diagnostics: most blocks (fixed, so the reduction order is fixed)
+constexpr int kDiagBlocks = 592;          // diagnostics: a FIXED number of partial sums, whatever the device, so that the reduction order is fixed
 constexpr int kStackSlab = 22 * 256;      // walk: spill entries (8 bytes each) per producer warp: <= 32 x 7 ranges per level; overflow sets kStatStack
 
-enum StatusBits : int { kStatNonFinite = 1, kStatCapacity = 2, kStatStack = 4 };
+enum StatusBits : int { kStatNonFinite = 1, kStatCapacity = 2, kStatStack = 4, kStatRange = 8, kStatBpStack = 16 };
+constexpr int kMaxExtentExp = 300;        // largest extent must lie in [2^-300, 2^300] (or be 0): bh.h preconditions
+constexpr int kNumStats = BH_NUM_STATS;
 
 // Device-resident state of one build; written by kernels, read by later kernels (no host round trip).
 struct DevState {
@@ -33,7 +37,7 @@ struct DevState {
     double side;           // L = 2^e
     double scale;          // 2^(21-e)
     int e;                 // exponent of L
-    int status;            // StatusBits, sticky until the next bh_build
+    int status;            // StatusBits, OR-ed by kernels, cleared by the host once it has reported them
     int n_nodes;           // M
     int depth;             // deepest level
     unsigned n_groups;     // Ng walk groups
@@ -43,7 +47,7 @@ struct DevState {
     unsigned ticket_diag;  // last-block election of the diagnostics reduction (resets itself)
     unsigned long long pair_count;     // broad phase: candidate pairs found (may exceed the caller's capacity)
     unsigned long long agg_counts[3];  // aggregates: connected components, aggregates (size > 1), bad pairs
-    unsigned long long stats[4];       // n_mono, n_direct, interactions, nodes tested
+    unsigned long long stats[kNumStats];   // n_mono, n_direct, interactions, nodes tested, stack spills
 };
 
 // Pointers into the caller's workspace.
@@ -79,7 +83,6 @@ struct Workspace {
     double *stage_pos;            // [n][3] host-call staging; also the direct kernel's partial sums
     int64_t stage_doubles;        // capacity of stage_pos in doubles
     double *stage_mass;           // [n]
-    double *peak_sink;            // fp64 microbenchmark sink
     double *diag_part;            // [kDiagBlocks][8][2] double-double partial sums of the diagnostics
     double *diag_out;             // [8] conserved quantities, [8] bits of the Eq. (7) maximum
     unsigned *diag_ticket;        // = &st->ticket_diag
@@ -93,13 +96,20 @@ struct Workspace {
     int64_t sort_tiles;
     int64_t tree_tiles;
     int walk_warps;               // producer warps of the walk = SMs x pairs per block
+    int sms;                      // multiprocessors of the device (grid sizing)
+    int leaf_cap;                 // C
+    int group_w;                  // W, bodies per walk group (1..32)
+    int group_cell;               // Gc
     size_t total_bytes;
 };
 
 struct WalkConfig {
     static constexpr int kPairsPerBlock = 8;   // producer/consumer warp pairs in the one block of an SM
-    static constexpr int kSMs = 148;
 };
+
+// multiprocessors of the current device, queried once; kDefaultSMs when there is no device (host-only
+// argument checks and size queries still work)
+int sm_count();
 
 inline int64_t node_capacity(int64_t n, int leaf_cap) { return n + 21 * (n / (leaf_cap + 1)) + 1; }
 
@@ -123,8 +133,6 @@ int launch_direct(const Workspace &w, int64_t n, const int32_t *tgt, int64_t nt,
 void launch_kick_drift(double *pos, double *vel, const double *acc, int64_t n, double dt, cudaStream_t s);
 void launch_kick(double *vel, const double *acc, int64_t n, double h, cudaStream_t s);
 void launch_unpack_mask(const Workspace &w, unsigned char *mask_out, int64_t cap, cudaStream_t s);
-double run_fp64_peak(const Workspace &w, cudaStream_t s);
-void run_issue_model(const Workspace &w, double out[3], cudaStream_t s);   // see bh_measure_issue_model
 // rows "next" (bh_diag.cu): results land in w.diag_out
 void launch_diagnostics(const Workspace &w, const double *pos, const double *vel, const double *mass,
                         const double *phi, int64_t n, cudaStream_t s);

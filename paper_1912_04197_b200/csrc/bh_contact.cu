@@ -95,6 +95,7 @@ __global__ void __launch_bounds__(256) node_box_kernel(const DevState *__restric
 
 constexpr int kBpWarps = 4;
 constexpr int kBpStack = 1024;   // node ids per warp (a local search holds a few dozen)
+constexpr int kBpRoom = kBpStack - 7 * kMaxLevel - 1;   // wide pops keep the stack below this (see the pop rule)
 constexpr int kBpLeafQ = 96;     // surviving leaves waiting for their body tests
 
 __device__ __forceinline__ double gap(double alo, double ahi, double blo, double bhi)
@@ -166,7 +167,14 @@ broadphase_kernel(DevState *st, const unsigned *__restrict__ gstart, const doubl
             }
             if (top == 0) break;
             // ---- pop up to 32 nodes, one per lane ----
-            const unsigned take = top < 32u ? top : 32u;
+            // A pop of k nodes pushes at most 8k children, so k <= (kBpRoom - top) / 7 keeps the stack below
+            // kBpRoom; when that allows fewer than two, the walk goes node by node (depth first), which adds at
+            // most 7 entries per level below the popped node: <= 7 * 21 = 147 more.  The stack cannot overflow.
+            unsigned take = top < 32u ? top : 32u;
+            {
+                const unsigned room = (unsigned)kBpRoom > top ? ((unsigned)kBpRoom - top) / 7u : 0u;
+                if (take > room) take = room > 1u ? room : 1u;
+            }
             top -= take;
             const bool have = lane < take;
             const unsigned t = have ? stack[top + lane] : 0u;
@@ -200,8 +208,8 @@ broadphase_kernel(DevState *st, const unsigned *__restrict__ gstart, const doubl
                     if (lane >= (unsigned)o) inc += u;
                 }
                 const unsigned total = __shfl_sync(0xffffffffu, inc, 31);
-                if (top + total > (unsigned)kBpStack) {      // cannot happen for a local search; stay memory-safe
-                    if (lane == 0) atomicOr(&st->status, (int)kStatStack);
+                if (top + total > (unsigned)kBpStack) {      // excluded by the pop rule above; stay memory-safe
+                    if (lane == 0) atomicOr(&st->status, (int)kStatBpStack);
                 } else {
                     for (unsigned u = 0; u < c; ++u) stack[top + inc - c + u] = first + u;
                     top += total;
@@ -298,13 +306,13 @@ __global__ void uf_count_kernel(const int *__restrict__ label, const int *__rest
 int launch_broadphase(const Workspace &w, int64_t n, const double *radius, const double *vel, double dt,
                       int32_t *pairs, int64_t cap, cudaStream_t s)
 {
-    cudaMemsetAsync(w.bp_cnt, 0, (size_t)w.node_cap * sizeof(unsigned), s);
+    cudaMemsetAsync(w.bp_cnt, 0, (size_t)node_capacity(n, w.leaf_cap) * sizeof(unsigned), s);
     cudaMemsetAsync(&w.st->pair_count, 0, sizeof(unsigned long long), s);
     bound_radius_kernel<<<(int)((n + 255) / 256), 256, 0, s>>>(radius, vel, w.idx[0], n, dt, w.bsort);
-    const int64_t want = (w.node_cap + 255) / 256;
-    node_box_kernel<<<(int)(want < 148 * 16 ? want : 148 * 16), 256, 0, s>>>(w.st, w.sbody, w.bsort, w.winfo, w.nparent,
+    const int64_t want = (node_capacity(n, w.leaf_cap) + 255) / 256;
+    node_box_kernel<<<(int)(want < w.sms * 16 ? want : w.sms * 16), 256, 0, s>>>(w.st, w.sbody, w.bsort, w.winfo, w.nparent,
                                                                              w.bp_cnt, w.box_lo, w.box_hi, w.node_cap);
-    broadphase_kernel<<<148 * 16, kBpWarps * 32, 0, s>>>(w.st, w.gstart, w.sbody, w.bsort, w.gbox, w.winfo, w.box_lo,
+    broadphase_kernel<<<w.sms * 16, kBpWarps * 32, 0, s>>>(w.st, w.gstart, w.sbody, w.bsort, w.gbox, w.winfo, w.box_lo,
                                                         w.box_hi, w.idx[0], reinterpret_cast<int2 *>(pairs),
                                                         (unsigned long long)cap);
     return 3;
@@ -315,11 +323,11 @@ int launch_aggregates(const Workspace &w, int64_t n, const int32_t *pairs, int64
 {
     cudaMemsetAsync(w.st->agg_counts, 0, 3 * sizeof(unsigned long long), s);
     if (!size) size = w.agg_size;
-    const int nb = (int)((n + 255) / 256 < 148 * 8 ? (n + 255) / 256 : 148 * 8);
+    const int nb = (int)((n + 255) / 256 < w.sms * 8 ? (n + 255) / 256 : w.sms * 8);
     uf_init_kernel<<<nb, 256, 0, s>>>(label, size, mass, n);
     int launches = 3;
     if (n_pairs > 0) {
-        const int pb = (int)((n_pairs + 255) / 256 < 148 * 16 ? (n_pairs + 255) / 256 : 148 * 16);
+        const int pb = (int)((n_pairs + 255) / 256 < w.sms * 16 ? (n_pairs + 255) / 256 : w.sms * 16);
         uf_union_kernel<<<pb, 256, 0, s>>>(label, reinterpret_cast<const int2 *>(pairs), n_pairs, n, w.st);
         ++launches;
     }

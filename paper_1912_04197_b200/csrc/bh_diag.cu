@@ -174,7 +174,7 @@ void launch_position_error(const Workspace &w, const double *pos, const double *
 {
     cudaMemsetAsync(w.diag_out + kDiagQ, 0, sizeof(double), s);
     int blocks = (int)((n + 255) / 256);
-    if (blocks > 148 * 8) blocks = 148 * 8;
+    if (blocks > w.sms * 8) blocks = w.sms * 8;
     poserr_kernel<<<blocks, 256, 0, s>>>(pos, ref, n, reinterpret_cast<unsigned long long *>(w.diag_out + kDiagQ));
 }
 
@@ -182,7 +182,7 @@ void launch_euler_sub(double *pos, double *vel, const double *acc, int64_t n, do
 {
     const long long n3 = 3ll * n;
     int blocks = (int)((n3 + 1023) / 1024);
-    if (blocks > 148 * 8) blocks = 148 * 8;
+    if (blocks > sm_count() * 8) blocks = sm_count() * 8;
     euler_sub_kernel<<<blocks, 256, 0, s>>>(pos, vel, acc, n3, dt, n_sub);
 }
 

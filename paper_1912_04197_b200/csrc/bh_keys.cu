@@ -5,7 +5,6 @@
 namespace bh {
 
 constexpr int kCubeThreads = 192;   // multiple of 3: a thread always sees the same axis
-constexpr int kCubeMaxBlocks = 148 * 4;
 
 __device__ __forceinline__ bool nonfinite(double x)
 {
@@ -110,13 +109,16 @@ __global__ void __launch_bounds__(kCubeThreads) cube_kernel(const double *__rest
         st->e = e;
         st->side = ldexp(1.0, e);
         st->scale = ldexp(1.0, 21 - e);
-        st->status = bad ? kStatNonFinite : 0;
+        // sticky error bits: OR-ed in, cleared by the host once it has reported them (bh.h)
+        int flags = bad ? (int)kStatNonFinite : 0;
+        if (!bad && E != 0.0 && (e < -kMaxExtentExp + 1 || e > kMaxExtentExp + 1)) flags |= (int)kStatRange;
+        if (flags) atomicOr(&st->status, flags);
         st->n_nodes = 0;
         st->n_groups = 0;
         st->depth = 0;
         st->ticket_bbox = 0;
         st->walk_queue = 0;
-        st->stats[0] = st->stats[1] = st->stats[2] = st->stats[3] = 0ull;
+        for (int k = 0; k < kNumStats; ++k) st->stats[k] = 0ull;
     }
 }
 
@@ -171,7 +173,8 @@ void launch_cube(const Workspace &w, const double *pos, int64_t n, cudaStream_t 
 {
     long long n3 = 3 * (long long)n;
     int blocks = (int)((n3 + kCubeThreads * 4 - 1) / (kCubeThreads * 4));   // four loads per thread, all in flight
-    if (blocks > kCubeMaxBlocks) blocks = kCubeMaxBlocks;
+    if (blocks > w.sms * 4) blocks = w.sms * 4;   // bbox_part holds kMaxBboxBlocks rows
+    if (blocks > kMaxBboxBlocks) blocks = kMaxBboxBlocks;
     if (blocks < 1) blocks = 1;
     cube_kernel<<<blocks, kCubeThreads, 0, s>>>(pos, n3, w.st, w.bbox_part);
 }
@@ -179,7 +182,7 @@ void launch_cube(const Workspace &w, const double *pos, int64_t n, cudaStream_t 
 void launch_keys(const Workspace &w, const double *pos, int64_t n, cudaStream_t s)
 {
     int blocks = (int)((n + 256 * 4 - 1) / (256 * 4));
-    if (blocks > 148 * 8) blocks = 148 * 8;
+    if (blocks > w.sms * 8) blocks = w.sms * 8;
     if (blocks < 1) blocks = 1;
     keys_kernel<<<blocks, 256, 0, s>>>(pos, n, w.st, w.key[0], w.hist);
 }

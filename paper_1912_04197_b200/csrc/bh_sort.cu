@@ -245,7 +245,7 @@ int launch_sort(const Workspace &w, int64_t n, cudaStream_t s)
     }
     for (int p = 0; p < kSortPasses; ++p) {
         const int a = p & 1, b = a ^ 1;
-        unsigned *lb = w.lookback + (size_t)p * w.sort_tiles * kRadix;
+        unsigned *lb = w.lookback + (size_t)p * tiles * kRadix;   // [pass][tiles of this n][256]: cleared per build
         if (p == 0)
             sort_pass_kernel<true><<<tiles, kSortThreads, 0, s>>>(w.key[a], w.idx[a], w.key[b], w.idx[b], n,
                                                                  p * kRadixBits, w.hist + p * kRadix, lb,

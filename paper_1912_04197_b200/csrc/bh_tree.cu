@@ -134,7 +134,7 @@ __device__ __forceinline__ unsigned range_begin(const unsigned long long *__rest
 // Kernel A: per body (d+1, leaf, group-start flag) and per-tile counts of nodes per level and of
 // group starts.
 __global__ void __launch_bounds__(256) tree_levels_kernel(const unsigned long long *__restrict__ skey,
-                                                          long long n, int C, int Gc, uchar4 *__restrict__ dlev,
+                                                          long long n, int C, int Gc, int W, uchar4 *__restrict__ dlev,
                                                           unsigned *__restrict__ tile_lvl, int ntiles)
 {
     extern __shared__ signed char sw[];   // [kTreeTile + C] leaf windows, then [kTreeTile + Gc] group windows
@@ -168,7 +168,7 @@ __global__ void __launch_bounds__(256) tree_levels_kernel(const unsigned long lo
         const int glev = min(leaf, mg + 1);
         const int d = (j == 0) ? -1 : common_levels(skey[j - 1], skey[j]);
         const unsigned cb = range_begin(skey, (unsigned)j, glev);
-        const bool gs = (((unsigned)j - cb) % kGroup) == 0u;
+        const bool gs = (((unsigned)j - cb) % (unsigned)W) == 0u;
         dlev[j] = make_uchar4((unsigned char)(d + 1), (unsigned char)leaf, gs ? 1 : 0, (unsigned char)glev);
         for (int l = d + 1; l <= leaf; ++l) atomicAdd(&shist[l], 1u);
         if (gs) atomicAdd(&shist[kLevels], 1u);
@@ -423,26 +423,25 @@ void launch_pack(const Workspace &w, const double *pos, const double *mass, int6
 void launch_tree(const Workspace &w, int64_t n, int leaf_cap, cudaStream_t s)
 {
     const int ntiles = (int)((n + kTreeTile - 1) / kTreeTile);
-    size_t smem = (size_t)(2 * kTreeTile + leaf_cap + kGroupCell);
-    tree_levels_kernel<<<ntiles, 256, smem, s>>>(w.key[0], n, leaf_cap, kGroupCell, w.dlev, w.tile_lvl, ntiles);
+    size_t smem = (size_t)(2 * kTreeTile + leaf_cap + w.group_cell);
+    tree_levels_kernel<<<ntiles, 256, smem, s>>>(w.key[0], n, leaf_cap, w.group_cell, w.group_w, w.dlev, w.tile_lvl, ntiles);
     tree_scan_kernel<<<1, (kLevels + 1) * 32, 0, s>>>(w.tile_lvl, ntiles, w.st, w.node_cap, w.gstart, (unsigned)n);
     tree_emit_kernel<<<ntiles, 256, 0, s>>>(w.key[0], n, w.dlev, w.tile_lvl, ntiles, w.st, w.node_cap, w.nlevel,
                                             w.nbegin, w.ncount, w.nfirst, w.nparent, w.node_meta, w.gstart);
-    group_box_kernel<<<148 * 4, 256, 0, s>>>(w.st, w.gstart, w.sbody, w.gbox);
+    group_box_kernel<<<w.sms * 4, 256, 0, s>>>(w.st, w.gstart, w.sbody, w.gbox);
 }
 
 void launch_monopoles(const Workspace &w, int64_t n, cudaStream_t s)
 {
-    int64_t want = (w.node_cap + 255) / 256;
-    int blocks = (int)(want < 148 * 16 ? want : 148 * 16);
-    (void)n;
+    const int64_t want = (node_capacity(n, w.leaf_cap) + 255) / 256;
+    int blocks = (int)(want < w.sms * 16 ? want : w.sms * 16);
     monopole_kernel<<<blocks, 256, 0, s>>>(w.st, w.sbody, w.nbegin, w.ncount, w.nfirst, w.nparent, w.node_meta,
                                            w.mono, w.node_cap, w.nlevel, w.winfo);
 }
 
 void launch_unpack_mask(const Workspace &w, unsigned char *mask_out, int64_t cap, cudaStream_t s)
 {
-    unpack_mask_kernel<<<148 * 4, 256, 0, s>>>(w.node_meta, w.st, mask_out, cap);
+    unpack_mask_kernel<<<w.sms * 4, 256, 0, s>>>(w.node_meta, w.st, mask_out, cap);
 }
 
 }  // namespace bh

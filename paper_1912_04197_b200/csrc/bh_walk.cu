@@ -23,130 +23,31 @@
 // sub-partition is fed by its two consumers while its two producers wait on L2.
 // The test arithmetic is the canonical one (each operation rounded once, fma where stated) so that
 // every accept/open decision equals the oracle's; traversal and accumulation order are free (R23).
-#include "bh_common.cuh"
+#include "bh_eval.cuh"
 
 namespace bh {
 
 constexpr int kPairs = WalkConfig::kPairsPerBlock;       // producer/consumer pairs per block
 constexpr int kWalkThreads = kPairs * 64;
-constexpr int kRing = 512;                  // sources per pair (power of two, multiple of 8)
 constexpr int kStack = 512;                 // sibling ranges per producer in shared memory (ring)
 constexpr int kSpill = 128;                 // spill / refill unit
 constexpr int kDesc = 4;                    // group descriptors in flight per pair
 constexpr unsigned kNoGroup = 0xffffffffu;
-#ifndef BH_SEED_LOWWORD
-#define BH_SEED_LOWWORD 1                   // rsqrt seed: low word taken from a dead register pair (see interact)
-#endif
 #ifndef BH_SLEEP_FULL
 #define BH_SLEEP_FULL 1000                  // ns a producer sleeps per poll while its ring is full
 #endif
 #ifndef BH_TRIP_UNROLL
 #define BH_TRIP_UNROLL 1
 #endif
-#ifndef BH_EVAL_UNROLL
-#define BH_EVAL_UNROLL 4
-#endif
 #ifndef BH_REG_PROD
 #define BH_REG_PROD 96                      // registers per thread of the producer warpgroups ...
 #define BH_REG_CONS 160                     // ... and of the consumer warpgroups (launch: 128)
 #endif
 constexpr int kTripUnroll = BH_TRIP_UNROLL;   // producer: trips of a pop unrolled
-constexpr int kEvalUnroll = BH_EVAL_UNROLL;   // consumer: chunks of eight sources unrolled
 #ifndef BH_PUB_MIN
 #define BH_PUB_MIN 0                        // a trip publishes only if at least this many entries are pending
 #endif
 
-// m / r^3 from r2 = |d|^2 + eps^2: MUFU.RSQ64H seed y (about 20 good bits), e = 1 - r2 y^2 and the
-// series (1-e)^(-3/2) = 1 + e (3/2 + 15/8 e) + O(e^3).  Every fp64 instruction except the three
-// accumulations reads at most two distinct register operands (a third costs the pipe a cycle on sm_100).
-template <bool GUARD>
-__device__ __forceinline__ void interact(double px, double py, double pz, double eps2, const double4 s,
-                                         double &ax, double &ay, double &az)
-{
-    const double dx = s.x - px, dy = s.y - py, dz = s.z - pz;
-    const double t2 = fma(dy, dy, fma(dz, dz, eps2));
-    const double r2 = fma(dx, dx, t2);
-    double y;
-#if BH_SEED_LOWWORD
-    // the seed's low word is irrelevant (the series below corrects any y within 2^-19 of r2^-1/2): take it
-    // from the dead partial sum, so that MUFU.RSQ64H can write into that register pair without a zero-fill
-    {
-        double y0;
-        asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y0) : "d"(r2));
-        y = __hiloint2double(__double2hiint(y0), __double2loint(t2));
-    }
-#else
-    asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(r2));
-#endif
-    if (GUARD) y = (r2 > 0.0) ? y : 0.0;      // a pair at zero softened distance adds nothing (R13)
-    const double u = y * y;
-    const double w = s.w * y;
-    const double e = fma(-r2, u, 1.0);
-    const double v = u * w;
-    const double p = fma(1.875, e, 1.5);
-    const double h = fma(p, e, 1.0);
-    const double f = v * h;
-    ax = fma(f, dx, ax);
-    ay = fma(f, dy, ay);
-    az = fma(f, dz, az);
-}
-
-// m / r from the same seed (NEXT-1, potential of the softened force, R24): (1-e)^(-1/2) = 1 + e (1/2 + 3/8 e) + O(e^3)
-template <bool GUARD>
-__device__ __forceinline__ void interact_pot(double px, double py, double pz, double eps2, const double4 s, double &phi)
-{
-    const double dx = s.x - px, dy = s.y - py, dz = s.z - pz;
-    const double r2 = fma(dx, dx, fma(dy, dy, fma(dz, dz, eps2)));
-    double y;
-    asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(r2));
-    if (GUARD) y = (r2 > 0.0) ? y : 0.0;
-    const double u = y * y;
-    const double w = s.w * y;
-    const double e = fma(-r2, u, 1.0);
-    const double p = fma(0.375, e, 0.5);
-    const double h = fma(p, e, 1.0);
-    phi = fma(w, h, phi);
-}
-
-// acceleration and potential of one interaction from one seed: 16 + 3 fp64 instructions
-template <bool GUARD>
-__device__ __forceinline__ void interact_both(double px, double py, double pz, double eps2, const double4 s,
-                                              double &ax, double &ay, double &az, double &phi)
-{
-    const double dx = s.x - px, dy = s.y - py, dz = s.z - pz;
-    const double t2 = fma(dy, dy, fma(dz, dz, eps2));
-    const double r2 = fma(dx, dx, t2);
-    double y;
-    {
-        double y0;
-        asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y0) : "d"(r2));
-        y = __hiloint2double(__double2hiint(y0), __double2loint(t2));
-    }
-    if (GUARD) y = (r2 > 0.0) ? y : 0.0;
-    const double u = y * y;
-    const double w = s.w * y;
-    const double e = fma(-r2, u, 1.0);
-    const double v = u * w;
-    const double p = fma(1.875, e, 1.5);
-    const double q = fma(0.375, e, 0.5);
-    const double h = fma(p, e, 1.0);
-    const double g = fma(q, e, 1.0);
-    const double f = v * h;
-    phi = fma(w, g, phi);
-    ax = fma(f, dx, ax);
-    ay = fma(f, dy, ay);
-    az = fma(f, dz, az);
-}
-
-// MODE 0: accelerations, 1: potential (accumulated in ax), 2: both
-template <bool GUARD, int MODE>
-__device__ __forceinline__ void interact_any(double px, double py, double pz, double eps2, const double4 s,
-                                             double &ax, double &ay, double &az, double &ph)
-{
-    if constexpr (MODE == 1) interact_pot<GUARD>(px, py, pz, eps2, s, ax);
-    else if constexpr (MODE == 2) interact_both<GUARD>(px, py, pz, eps2, s, ax, ay, az, ph);
-    else interact<GUARD>(px, py, pz, eps2, s, ax, ay, az);
-}
 
 struct PairCtrl {                            // all words are written by one role and read by the other
     unsigned tail_pub;                       // producer: ring entries below this are complete
@@ -211,10 +112,6 @@ struct Producer {
     unsigned tail;        // ring entries written (absolute)
     unsigned head_seen;   // last value read from ctrl.head_pub
     unsigned pub;         // last value stored to ctrl.tail_pub
-#ifdef BH_WALK_PROF
-    long long wait_cycles = 0;
-    unsigned long long iterations = 0;
-#endif
 
     __device__ __forceinline__ void publish(unsigned v)
     {
@@ -228,9 +125,6 @@ struct Producer {
     // is free again, so that the producer works in bursts and does not burn issue slots polling
     __device__ __forceinline__ void reserve_slow(unsigned n)
     {
-#ifdef BH_WALK_PROF
-        const long long t0 = clock64();
-#endif
         cp_async_commit();
         cp_async_wait_all();
         publish(tail);
@@ -240,9 +134,6 @@ struct Producer {
             head_seen = warp_acquire(&ps.ctrl.head_pub, lane);
             if (tail + want - head_seen <= (unsigned)kRing) break;
         }
-#ifdef BH_WALK_PROF
-        wait_cycles += clock64() - t0;
-#endif
     }
     __device__ __forceinline__ void reserve(unsigned n)
     {
@@ -298,12 +189,10 @@ __device__ void produce(PairSmem &ps, DevState *st, const unsigned *__restrict__
     const unsigned lane = lane_id();
     const unsigned lt = (1u << lane) - 1u;
     const unsigned ngroups = st->n_groups;
-    const int s2_base = (2 * st->e + 1023) << 20;   // high word of L^2; a level down is 2^-2: subtract 2 << 20
+    const int s2_base = (2 * st->e + 1023) << 20;   // high word of L^2; a level down is 2^-2: subtract 2 << 20 (|e| <= 301 is checked by cube_kernel, so the exponent field stays in range)
     unsigned long long tot_mono = 0, tot_direct = 0, tot_inter = 0, tot_tested = 0;
+    unsigned tot_spills = 0;   // times the shared stack overflowed into the global slab (stats[4])
     Producer P{ps, lane, 0u, 0u, 0u};
-#ifdef BH_WALK_PROF
-    const long long prof_t0 = clock64();
-#endif
     uint2 *stack = ps.stack;
     unsigned k = 0;   // groups started by this pair
 
@@ -355,9 +244,6 @@ __device__ void produce(PairSmem &ps, DevState *st, const unsigned *__restrict__
                 const bool have = q < nsib;
                 const NodeRec cur = nxt;
                 if (q + 1 < nsib) nxt = load_rec(winfo, mono, first + q + 1);
-#ifdef BH_WALK_PROF
-                ++P.iterations;
-#endif
                 // ---- opening test (canonical arithmetic, R22) ----
                 const unsigned nb = cur.info.x, nc = cur.info.y;
                 const bool internal = (int)cur.info.z >= 0;
@@ -392,6 +278,7 @@ __device__ void produce(PairSmem &ps, DevState *st, const unsigned *__restrict__
                                 for (unsigned u = lane; u < (unsigned)kSpill; u += 32) slab[gsp + u] = stack[(bot + u) & (kStack - 1)];
                                 gsp += kSpill;
                                 bot += kSpill;
+                                ++tot_spills;
                             }
                         }
                         if (open_int) stack[(top + __popc(m & lt)) & (kStack - 1)] = make_uint2(cur.info.z, (cur.info.w >> 8) & 0xffu);
@@ -469,13 +356,6 @@ __device__ void produce(PairSmem &ps, DevState *st, const unsigned *__restrict__
         tot_inter += (unsigned long long)(n_mono + n_direct) * (unsigned long long)(ge - gb);
         tot_tested += my_tested;               // per lane; summed over the warp by the atomics below
     }
-#ifdef BH_WALK_PROF
-    (void)tot_mono; (void)tot_direct; (void)tot_inter; (void)tot_tested;
-    if (lane == 0) {
-        atomicAdd(&st->stats[2], (unsigned long long)P.wait_cycles);
-        atomicAdd(&st->stats[3], P.iterations);
-    }
-#else
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) tot_tested += __shfl_xor_sync(0xffffffffu, tot_tested, o);
     if (lane == 0) {
@@ -483,37 +363,14 @@ __device__ void produce(PairSmem &ps, DevState *st, const unsigned *__restrict__
         atomicAdd(&st->stats[1], tot_direct);
         atomicAdd(&st->stats[2], tot_inter);
         atomicAdd(&st->stats[3], tot_tested);
+        if (tot_spills) atomicAdd(&st->stats[4], (unsigned long long)tot_spills);
     }
-#endif
 }
 
 // ------------------------------------------------------------------------------------------ consumer
-// Lane l = 8 q + r holds bodies r, r+8, r+16, r+24 of the group (NS = ceil(bodies / 8) of them are
-// real) and, of every chunk of eight sources, takes sources q and q+4.
-template <int NS>
-struct Bodies {
-    double x[NS], y[NS], z[NS], ax[NS], ay[NS], az[NS], ph[NS];   // ph only lives in MODE 2
-};
-
-// evaluate n8 (a multiple of 8) sources starting at ring position head (a multiple of 8)
-template <bool GUARD, int NS, int MODE>
-__device__ __forceinline__ void eval_chunks(const double4 *ring, unsigned head, unsigned n8, unsigned quarter,
-                                            double eps2, Bodies<NS> &B)
-{
-#pragma unroll kEvalUnroll
-    for (unsigned i = 0; i < n8; i += 8) {
-        const double4 *p = ring + ((head + i) & (kRing - 1)) + quarter;
-        const double4 s0 = p[0], s1 = p[4];
-#pragma unroll
-        for (int k = 0; k < NS; ++k) interact_any<GUARD, MODE>(B.x[k], B.y[k], B.z[k], eps2, s0, B.ax[k], B.ay[k], B.az[k], B.ph[k]);
-#pragma unroll
-        for (int k = 0; k < NS; ++k) interact_any<GUARD, MODE>(B.x[k], B.y[k], B.z[k], eps2, s1, B.ax[k], B.ay[k], B.az[k], B.ph[k]);
-    }
-}
-
 // one group: evaluate its sources as the producer publishes them, then write the accelerations
 template <bool GUARD, int NS, int MODE>
-__device__ __forceinline__ long long consume_group(PairSmem &ps, unsigned k, unsigned head, long long gb, long long ge,
+__device__ __forceinline__ void consume_group(PairSmem &ps, unsigned k, unsigned head, long long gb, long long ge,
                                               const double4 *__restrict__ sbody, const unsigned *__restrict__ perm,
                                               double eps2, double G, double *__restrict__ acc, double *__restrict__ phi)
 {
@@ -527,25 +384,22 @@ __device__ __forceinline__ long long consume_group(PairSmem &ps, unsigned k, uns
         B.ax[s] = B.ay[s] = B.az[s] = B.ph[s] = 0.0;
     }
     const double4 zero4 = make_double4(0.0, 0.0, 0.0, 0.0);
-    long long g_prof_wait = 0;   // cycles spent waiting for the producer (profiling builds only)
     while (true) {
         unsigned lim = 0;
         bool fin = false;
         if (lane == 0) {
+            // tail_pub FIRST, then finished: if the group is not finished at the second load, the earlier
+            // tail_pub cannot yet include entries of a later group (the producer publishes those only after
+            // it has finished this one)
+            const unsigned tp = ld_acquire(&ps.ctrl.tail_pub);
             fin = (int)(ld_acquire(&ps.ctrl.finished) - k) > 0;
-            lim = fin ? ps.ctrl.desc_end[k % kDesc] : ld_acquire(&ps.ctrl.tail_pub);
+            lim = fin ? ps.ctrl.desc_end[k % kDesc] : tp;
         }
         fin = __shfl_sync(0xffffffffu, (int)fin, 0) != 0;
         lim = __shfl_sync(0xffffffffu, lim, 0);
         const int avail = (int)(lim - head);       // negative while tail_pub still belongs to the last group
         if (!fin && avail < 32) {
-#ifdef BH_WALK_PROF
-            const long long t0 = clock64();
             __nanosleep(32);
-            g_prof_wait += clock64() - t0;
-#else
-            __nanosleep(32);
-#endif
             continue;
         }
         const unsigned n8 = avail > 0 ? ((unsigned)avail & ~7u) : 0u;
@@ -611,47 +465,28 @@ __device__ __forceinline__ long long consume_group(PairSmem &ps, unsigned k, uns
             acc[3ll * i + 2] = G * oz;
         }
     }
-    return g_prof_wait;
 }
 
 template <bool GUARD, int MODE>
-__device__ void consume(PairSmem &ps, DevState *prof_st, const unsigned *__restrict__ gstart, const double4 *__restrict__ sbody,
+__device__ void consume(PairSmem &ps, const unsigned *__restrict__ gstart, const double4 *__restrict__ sbody,
                         const unsigned *__restrict__ perm, double eps2, double G, double *__restrict__ acc,
                         double *__restrict__ phi)
 {
     const unsigned lane = lane_id();
-    long long waited = 0;
-#ifdef BH_WALK_PROF
-    const long long prof_t0 = clock64();
-#endif
     for (unsigned k = 0;; ++k) {
-#ifdef BH_WALK_PROF
-        const long long w0 = clock64();
-#endif
         while ((int)(warp_acquire(&ps.ctrl.started, lane) - k) <= 0) __nanosleep(64);
-#ifdef BH_WALK_PROF
-        waited += clock64() - w0;
-#endif
         const unsigned g = ps.ctrl.desc_g[k % kDesc];
         if (g == kNoGroup) break;
         const unsigned head = ps.ctrl.desc_begin[k % kDesc];
         const long long gb = gstart[g];
         const long long ge = gstart[g + 1];
         const int slots = (int)((ge - gb + 7) >> 3);
-        if (slots >= 4) waited += consume_group<GUARD, 4, MODE>(ps, k, head, gb, ge, sbody, perm, eps2, G, acc, phi);
-        else if (slots == 3) waited += consume_group<GUARD, 3, MODE>(ps, k, head, gb, ge, sbody, perm, eps2, G, acc, phi);
-        else if (slots == 2) waited += consume_group<GUARD, 2, MODE>(ps, k, head, gb, ge, sbody, perm, eps2, G, acc, phi);
-        else waited += consume_group<GUARD, 1, MODE>(ps, k, head, gb, ge, sbody, perm, eps2, G, acc, phi);
+        if (slots >= 4) consume_group<GUARD, 4, MODE>(ps, k, head, gb, ge, sbody, perm, eps2, G, acc, phi);
+        else if (slots == 3) consume_group<GUARD, 3, MODE>(ps, k, head, gb, ge, sbody, perm, eps2, G, acc, phi);
+        else if (slots == 2) consume_group<GUARD, 2, MODE>(ps, k, head, gb, ge, sbody, perm, eps2, G, acc, phi);
+        else consume_group<GUARD, 1, MODE>(ps, k, head, gb, ge, sbody, perm, eps2, G, acc, phi);
         warp_release(&ps.ctrl.consumed, k + 1, lane);
     }
-#ifdef BH_WALK_PROF
-    if (lane == 0) {
-        atomicAdd(&prof_st->stats[0], (unsigned long long)waited);
-        atomicAdd(&prof_st->stats[1], (unsigned long long)(clock64() - prof_t0));
-    }
-#else
-    (void)waited;
-#endif
 }
 
 template <bool GUARD, int MODE>
@@ -681,7 +516,7 @@ walk_kernel(DevState *st, const unsigned *__restrict__ gstart, const double4 *__
         produce<MODE != 0>(ps, st, gstart, sbody, gbox, winfo, mono, theta2, cnt_mono, cnt_direct,
                 reinterpret_cast<uint2 *>(walk_stack) + (size_t)(blockIdx.x * kPairs + pair) * kStackSlab);
     else
-        consume<GUARD, MODE>(ps, st, gstart, sbody, perm, eps2, G, acc, phi);
+        consume<GUARD, MODE>(ps, gstart, sbody, perm, eps2, G, acc, phi);
 }
 
 // ------------------------------------------------------------------------------------------ a8
@@ -785,88 +620,6 @@ __global__ void kick_kernel(double *__restrict__ vel, const double *__restrict__
         vel[k] = __fma_rn(acc[k], h, vel[k]);
 }
 
-// ------------------------------------------------------------------------------------------ fp64 peak
-__global__ void __launch_bounds__(256) fp64_peak_kernel(double *sink, int iters, double seed)
-{
-    double a0 = seed + threadIdx.x, a1 = a0 + 1, a2 = a0 + 2, a3 = a0 + 3, a4 = a0 + 4, a5 = a0 + 5, a6 = a0 + 6,
-           a7 = a0 + 7;
-    const double m = 0.999999, c = 1e-9;
-    for (int i = 0; i < iters; ++i) {
-        a0 = fma(a0, m, c); a1 = fma(a1, m, c); a2 = fma(a2, m, c); a3 = fma(a3, m, c);
-        a4 = fma(a4, m, c); a5 = fma(a5, m, c); a6 = fma(a6, m, c); a7 = fma(a7, m, c);
-    }
-    double s = a0 + a1 + a2 + a3 + a4 + a5 + a6 + a7;
-    if (s == 123456.789) sink[0] = s;
-}
-
-// ------------------------------------------------------------------------------------------ issue model
-// What the walk's evaluation loop reaches when nothing else runs on its sub-partition, and what it loses to
-// co-resident warps that issue integer / shared-memory instructions (as the walk's producer warps do).  Same
-// block shape as walk_kernel: 16 warps, warps 4-7 and 12-15 evaluate (two per sub-partition, four bodies per
-// lane, sources from a 512-entry shared-memory ring); the other eight warps exit (HOG 0), run a dependent
-// IMAD / LDS chain at low duty (HOG 1) or independent IMADs at full rate (HOG 2) until the evaluators are done.
-template <int HOG>
-__global__ void __launch_bounds__(512, 1) issue_model_kernel(double *sink, int iters, double eps2, int seed)
-{
-    __shared__ double4 ring[512];
-    __shared__ int tab[1024];
-    __shared__ int done;
-    for (int i = threadIdx.x; i < 512; i += blockDim.x) ring[i] = make_double4(1.0 + i * 0.01, 2.0 - i * 0.02, 0.5 + i * 0.003, 1e-3);
-    for (int i = threadIdx.x; i < 1024; i += blockDim.x) tab[i] = (i * 7 + seed) & 1023;
-    if (threadIdx.x == 0) done = 0;
-    __syncthreads();
-    const unsigned warp = threadIdx.x >> 5, lane = threadIdx.x & 31u, quarter = lane >> 3;
-    if (((warp >> 2) & 1u) == 1u) {
-        Bodies<4> B;
-        for (int s = 0; s < 4; ++s) {
-            B.x[s] = 0.1 * lane + s; B.y[s] = 0.2 * s; B.z[s] = 0.05 * lane;
-            B.ax[s] = B.ay[s] = B.az[s] = B.ph[s] = 0.0;
-        }
-        for (int it = 0; it < iters; ++it) eval_chunks<false, 4, 0>(ring, 0u, 512u, quarter, eps2, B);
-        double s = 0.0;
-        for (int q = 0; q < 4; ++q) s += B.ax[q] + B.ay[q] + B.az[q];
-        if (s == 123.456) sink[0] = s;
-        __syncwarp();
-        if (lane == 0) atomicAdd(&done, 1);
-    } else if (HOG != 0) {
-        int a = seed + (int)lane, b = seed * 3 + (int)lane, c = (int)lane;
-        while (*((volatile int *)&done) < 8) {
-            if (HOG == 1) {
-                for (int r = 0; r < 16; ++r) { a = tab[(a * 5 + b) & 1023]; b = b * 3 + a; c ^= a + b; }
-            } else {
-                for (int r = 0; r < 16; ++r) { a = a * 5 + seed; b = b * 3 + seed; c = c * 7 + seed; }
-            }
-        }
-        if (a + b + c == 12345) sink[1] = a;
-    }
-}
-
-template <int HOG>
-static double run_issue_model_one(double *sink, cudaStream_t s)
-{
-    const int iters = 100, blocks = WalkConfig::kSMs;
-    cudaEvent_t a, b;
-    cudaEventCreate(&a);
-    cudaEventCreate(&b);
-    issue_model_kernel<HOG><<<blocks, 512, 0, s>>>(sink, 2, 1e-8, 3);
-    cudaEventRecord(a, s);
-    issue_model_kernel<HOG><<<blocks, 512, 0, s>>>(sink, iters, 1e-8, 3);
-    cudaEventRecord(b, s);
-    cudaEventSynchronize(b);
-    float ms = 0.f;
-    cudaEventElapsedTime(&ms, a, b);
-    cudaEventDestroy(a);
-    cudaEventDestroy(b);
-    return (double)blocks * 8 * 32 * iters * 64.0 * 2.0 * 4 / (ms * 1e-3);   // body-source interactions per second
-}
-
-void run_issue_model(const Workspace &w, double out[3], cudaStream_t s)
-{
-    out[0] = run_issue_model_one<0>(w.peak_sink, s);
-    out[1] = run_issue_model_one<1>(w.peak_sink, s);
-    out[2] = run_issue_model_one<2>(w.peak_sink, s);
-}
-
 // ------------------------------------------------------------------------------------------ launchers
 template <bool GUARD, int MODE>
 static void launch_walk_t(const Workspace &w, double theta, double eps2, double G, double *out, double *phi, cudaStream_t s)
@@ -887,7 +640,7 @@ void launch_walk(const Workspace &w, int64_t n, double theta, double eps, double
 {
     (void)n;
     const double eps2 = eps * eps;
-    const bool guard = !(eps2 > 0.0);
+    const bool guard = !(eps2 >= kTinyR2);
     if (mode == 1) {
         if (guard) launch_walk_t<true, 1>(w, theta, eps2, G, acc, nullptr, s);
         else launch_walk_t<false, 1>(w, theta, eps2, G, acc, nullptr, s);
@@ -908,7 +661,7 @@ int launch_direct(const Workspace &w, int64_t n, const int32_t *tgt, int64_t nt,
     const int tblocks = (int)((rows + per * kDirectThreads - 1) / (per * kDirectThreads));
     const int tiles = (int)((n + kDirectThreads - 1) / kDirectThreads);
     // enough blocks for ~8 per SM; the partial sums live in the host-staging area (3 * max_n doubles)
-    int splits = (148 * 8 + tblocks - 1) / tblocks;
+    int splits = (w.sms * 8 + tblocks - 1) / tblocks;
     if (splits > tiles) splits = tiles;
     const int64_t room = w.stage_doubles / (3 * rows);
     if (splits > room) splits = (int)room;
@@ -927,15 +680,15 @@ int launch_direct(const Workspace &w, int64_t n, const int32_t *tgt, int64_t nt,
                                                                          eps2, G, acc, w.stage_pos, tps);              \
     } while (0)
     if (potential) {
-        if (eps2 > 0.0) BH_DIRECT(false, true);
+        if (eps2 >= kTinyR2) BH_DIRECT(false, true);
         else BH_DIRECT(true, true);
     } else {
-        if (eps2 > 0.0) BH_DIRECT(false, false);
+        if (eps2 >= kTinyR2) BH_DIRECT(false, false);
         else BH_DIRECT(true, false);
     }
 #undef BH_DIRECT
     if (splits > 1)
-        direct_reduce_kernel<<<148 * 2, 256, 0, s>>>(w.stage_pos, rows, splits, potential ? -G : G,
+        direct_reduce_kernel<<<w.sms * 2, 256, 0, s>>>(w.stage_pos, rows, splits, potential ? -G : G,
                                                      potential ? 1 : 3, w.idx[0], tgt != nullptr, acc);
     return splits > 1 ? 2 : 1;
 }
@@ -944,7 +697,7 @@ void launch_kick_drift(double *pos, double *vel, const double *acc, int64_t n, d
 {
     const long long n3 = 3ll * n;
     int blocks = (int)((n3 + 1023) / 1024);
-    if (blocks > 148 * 8) blocks = 148 * 8;
+    if (blocks > sm_count() * 8) blocks = sm_count() * 8;
     kick_drift_kernel<<<blocks, 256, 0, s>>>(pos, vel, acc, n3, dt * 0.5, dt);
 }
 
@@ -952,31 +705,8 @@ void launch_kick(double *vel, const double *acc, int64_t n, double h, cudaStream
 {
     const long long n3 = 3ll * n;
     int blocks = (int)((n3 + 1023) / 1024);
-    if (blocks > 148 * 8) blocks = 148 * 8;
+    if (blocks > sm_count() * 8) blocks = sm_count() * 8;
     kick_kernel<<<blocks, 256, 0, s>>>(vel, acc, n3, h);
-}
-
-double run_fp64_peak(const Workspace &w, cudaStream_t s)
-{
-    const int iters = 1 << 16, blocks = 148 * 8, threads = 256;
-    cudaEvent_t a, b;
-    cudaEventCreate(&a);
-    cudaEventCreate(&b);
-    fp64_peak_kernel<<<blocks, threads, 0, s>>>(w.peak_sink, 1 << 10, 1.0);   // warm-up
-    float best = 1e30f;
-    for (int rep = 0; rep < 3; ++rep) {
-        cudaEventRecord(a, s);
-        fp64_peak_kernel<<<blocks, threads, 0, s>>>(w.peak_sink, iters, 1.0);
-        cudaEventRecord(b, s);
-        cudaEventSynchronize(b);
-        float ms = 0.f;
-        cudaEventElapsedTime(&ms, a, b);
-        if (ms < best) best = ms;
-    }
-    cudaEventDestroy(a);
-    cudaEventDestroy(b);
-    const double flops = 2.0 * 8.0 * (double)iters * (double)blocks * (double)threads;
-    return flops / (best * 1e-3) / 1e12;
 }
 
 }  // namespace bh

@@ -29,12 +29,13 @@ def test_library_exports_every_declared_symbol():
 
 def test_workspace_bytes_host_logic():
     wb = binding.bh_workspace_bytes
-    assert wb(0, 16) == 0 and wb(1024, 0) == 0 and wb(1024, 16, 7) == 0 and wb((1 << 30) + 1, 16) == 0
+    assert wb(0, 16) == 0 and wb(1024, 0) == 0 and wb(1024, 16, 33) == 0 and wb(1024, 16, -1) == 0 and wb((1 << 30) + 1, 16) == 0
     a, b, c = wb(1024, 8), wb(1 << 20, 16), wb(1 << 22, 32)
     assert 0 < a < b < c
     assert b < 1 << 30                      # N=1M fits in well under 1 GiB
     assert c < 4 << 30
     assert wb(1 << 20, 16, 32) == b         # group_size 0 means 32
+    assert wb(1 << 20, 16, 1) == b          # any W in 1..32 (the group arrays are sized for one body per group)
     assert wb(1 << 20, 1) > b               # smaller leaves -> larger node bound
 
 
@@ -47,6 +48,7 @@ def test_create_rejects_bad_arguments_without_gpu():
     assert L.bh_create(C.byref(ctx), 1024, 8, 0, 256, 16, None) == binding.BH_ERR_CAPACITY               # too small
     assert ctx.value is None
     assert L.bh_build(None, None, None, 5) == binding.BH_ERR_INVALID_ARG
+    assert L.bh_set_group_cell(None, 64) == binding.BH_ERR_INVALID_ARG
     assert b"workspace" in L.bh_last_error(None)
 
 

@@ -106,11 +106,13 @@ def test_state_acc_pointer_and_sorted_bodies():
 
 
 def test_roofline_microbenchmarks_are_sane():
-    ctx = bh.Context(1024, 8)
-    peak = bh.bh_measure_fp64_peak(ctx.ctx)
+    """The measurement-only library behind bench.py's roofline denominator (not part of libbh)."""
+    import bench
+    mb = bench.Microbench()
+    stream = torch.cuda.current_stream()
+    peak = mb.fp64_peak(stream)
     assert 20.0 < peak < 45.0                         # B200: 148 SM x 64 lanes x 2 x <= 1.965 GHz = 37.2 TFLOP/s
-    m = bh.bh_measure_issue_model(ctx.ctx)
+    m = mb.issue_model(stream)
     bound = 148 * 4 * 1.965e9                         # one interaction per cycle per sub-partition
     assert 0.6 * bound < m["beside_low_duty_integer_warps"] < m["eval_loop_alone"] <= 1.02 * bound
     assert m["beside_full_rate_integer_warps"] < m["eval_loop_alone"]
-    ctx.close()

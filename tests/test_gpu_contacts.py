@@ -182,3 +182,16 @@ def test_degenerate_clouds_next_rows():
     r = orc.aggregates(120, ref)
     assert (comps, aggs) == (r["components"], r["aggregates"]) and np.array_equal(label.cpu().numpy(), r["label"])
     ctx.close()
+
+
+@pytest.mark.parametrize("n,C,speed,dt", [(2500, 1, 0.0, 0.0), (4000, 2, 3.0, 0.1), (3000, 16, 0.0, 0.0)])
+def test_broadphase_non_local_search(n, C, speed, dt):
+    """Bounding volumes that span a large part of the cloud (big radii, or fast bodies over a long step): the search
+    is not local, most of a deep tree is near every group, and the node stack is held inside its bound by the pop
+    rule (no overflow, no error), still the exact pair set."""
+    w = wl.spheres(n, mean_contacts=2.0, speed=speed)
+    radius = w.extra["radius"] * (1.0 if speed else 6.0)
+    ref = orc.broadphase(w.pos, orc.bound_radius(w.vel if speed else None, radius, dt))
+    got = gpu_pairs(w.pos, w.mass, radius, w.vel if speed else None, dt, C)
+    assert len(ref) > 20 * n
+    assert np.array_equal(sorted_pairs(got), ref)

@@ -258,6 +258,43 @@ def test_cuda_graph_steppers_bit_identical(n, method):
     assert outs[0][2] == outs[1][2]             # the launch count is the same claim on both paths
 
 
+def test_graph_replay_keeps_the_host_view_of_the_context():
+    """A replayed stepper graph rebuilds the tree of the BOUND state on the device; the host-side view (n, built,
+    walked) must say so even if the caller built another, smaller, set of bodies in between: a following bh_accel
+    writes all bound_n rows and the getters describe the bound state's tree."""
+    w, w2 = wl.make("c4", 1000), wl.make("c1", 500)
+    pos, vel, mass = dev(w.pos), dev(w.vel), dev(w.mass)
+    ctx = bh.Context(w.n, 16)
+    bh.bh_bind_state(ctx.ctx, pos, vel, mass, w.theta, w.eps, w.G)
+    bh.bh_set_graph(ctx.ctx, True)
+    for _ in range(4):                                   # plain (a(x0) too), plain, capture, replay
+        bh.bh_kdk_step(ctx.ctx, 1e-3)
+    ctx.build(dev(w2.pos), dev(w2.mass))                 # another body set, n = 500
+    assert bh.bh_get_groups(ctx.ctx) == len(orc.build(w2.pos, w2.mass, 16).gstart) - 1
+    bh.bh_kdk_step(ctx.ctx, 1e-3)                        # replay: the device now holds the 1000-body tree again
+    bh.bh_synchronize(ctx.ctx)
+    p = pos.cpu().numpy()
+    t = orc.build(p, w.mass, 16)
+    assert bh.bh_get_node_count(ctx.ctx) == (t.M, t.depth)
+    ctx.n = w.n
+    guard = torch.full((w.n + 64, 3), 7.0, dtype=torch.float64, device="cuda")
+    bh.bh_accel(ctx.ctx, w.theta, w.eps, w.G, guard[:w.n])
+    a = guard.cpu().numpy()
+    assert (a[w.n:] == 7.0).all()
+    ref = orc.accel(t, w.theta, w.eps, w.G)[0]
+    assert (np.linalg.norm(a[:w.n] - ref, axis=1) / np.linalg.norm(ref, axis=1)).max() <= 1e-11
+    # direct method: after a (replayed) step the context holds no tree, whatever was built before
+    bh.bh_set_gravity_method(ctx.ctx, 1)
+    for _ in range(4):
+        bh.bh_kdk_step(ctx.ctx, 1e-3)
+    ctx.build(dev(w2.pos), dev(w2.mass))
+    bh.bh_kdk_step(ctx.ctx, 1e-3)
+    with pytest.raises(bh.BhError) as e:
+        bh.bh_accel(ctx.ctx, w.theta, w.eps, w.G, guard[:w.n])
+    assert e.value.status == bh.BH_ERR_STATE
+    ctx.close()
+
+
 @pytest.mark.parametrize("name,n,C", [("c1", 1024, 8), ("c2", 16384, 16), ("c4", 30000, 16), ("c3", 777, 1), ("c3", 5, 16)])
 def test_accel_and_potential_from_one_walk(name, n, C):
     """bh_accel_potential: both outputs of the fused walk against the oracle's two evaluations (same lists)."""

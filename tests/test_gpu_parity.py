@@ -263,29 +263,22 @@ def test_full_size_headline_config():
     ctx.close()
 
 
-def test_eval_host_pageable_output_is_staged():
-    """bh_eval_host with ordinary (pageable) host memory takes the staged path; with pinned memory, from the
-    second call on and when a body has enough interactions (>= 3400), the walk stores straight into the output.
-    All paths must give the same accelerations bit for bit."""
+def test_eval_host_pageable_and_pinned_agree():
+    """bh_eval_host has one code path: pageable and pinned host buffers, first and later calls, many and few
+    interactions per body all give the same accelerations bit for bit (no state is carried between calls)."""
     w = wl.make("c4", 20000)
-    theta = 0.2                                      # ~ 6000 interactions per body: the direct-store path is taken
     ctx = bh.Context(w.n, 16)
     pos_h, mass_h = torch.as_tensor(w.pos), torch.as_tensor(w.mass)
-    out_page = torch.empty((w.n, 3), dtype=torch.float64)
-    out_pin = torch.empty((w.n, 3), dtype=torch.float64).pin_memory()
-    out_pin2 = torch.zeros((w.n, 3), dtype=torch.float64).pin_memory()
-    bh.bh_eval_host(ctx.ctx, pos_h, mass_h, theta, w.eps, w.G, out_page)
-    assert bh.bh_get_stats(ctx.ctx)["interactions"] / w.n >= 3400
-    bh.bh_eval_host(ctx.ctx, pos_h.pin_memory(), mass_h.pin_memory(), theta, w.eps, w.G, out_pin)
-    bh.bh_eval_host(ctx.ctx, pos_h.pin_memory(), mass_h.pin_memory(), theta, w.eps, w.G, out_pin2)
-    assert np.array_equal(out_page.numpy(), out_pin.numpy()) and np.array_equal(out_page.numpy(), out_pin2.numpy())
-    ref = orc.accel(orc.build(w.pos, w.mass, 16), theta, w.eps, w.G)[0]
-    assert relerr(out_pin.numpy(), ref).max() <= TOL
-    # few interactions per body (theta = 1): staged again, same contract
-    bh.bh_eval_host(ctx.ctx, pos_h.pin_memory(), mass_h.pin_memory(), 1.0, w.eps, w.G, out_pin)
-    bh.bh_eval_host(ctx.ctx, pos_h.pin_memory(), mass_h.pin_memory(), 1.0, w.eps, w.G, out_pin2)
-    assert np.array_equal(out_pin.numpy(), out_pin2.numpy())
-    assert relerr(out_pin.numpy(), orc.accel(orc.build(w.pos, w.mass, 16), 1.0, w.eps, w.G)[0]).max() <= TOL
+    for theta in (0.2, 1.0):
+        out_page = torch.empty((w.n, 3), dtype=torch.float64)
+        out_pin = torch.empty((w.n, 3), dtype=torch.float64).pin_memory()
+        out_pin2 = torch.zeros((w.n, 3), dtype=torch.float64).pin_memory()
+        bh.bh_eval_host(ctx.ctx, pos_h, mass_h, theta, w.eps, w.G, out_page)
+        bh.bh_eval_host(ctx.ctx, pos_h.pin_memory(), mass_h.pin_memory(), theta, w.eps, w.G, out_pin)
+        bh.bh_eval_host(ctx.ctx, pos_h.pin_memory(), mass_h.pin_memory(), theta, w.eps, w.G, out_pin2)
+        assert np.array_equal(out_page.numpy(), out_pin.numpy()) and np.array_equal(out_page.numpy(), out_pin2.numpy())
+        ref = orc.accel(orc.build(w.pos, w.mass, 16), theta, w.eps, w.G)[0]
+        assert relerr(out_pin.numpy(), ref).max() <= TOL
     ctx.close()
 
 
@@ -340,4 +333,239 @@ def test_headline_config_after_ten_kdk_steps():
         assert relerr(a[rows], ref[rows]).max() <= TOL
     # the cloud is in equilibrium: ten steps of dt = 1e-3 move bodies by about |v| * 0.01
     assert np.abs(p - w.pos).max() < 0.05
+    ctx.close()
+
+
+# ---------------------------------------------------------------------------------------------------------
+# configs[2] and configs[4] at their stated sizes
+def test_c3_full_size_theta_sweep():
+    """configs[2]: N = 131072 uniform ball, C = 16, theta in {0, 0.3, 0.5, 0.7, 1.0}.  Tree bit for bit; for
+    theta >= 0.3 the list lengths of ALL groups and the accelerations of ALL bodies against the oracle; for
+    theta = 0 (the oracle's walk is N^2 in long double) the lists of all groups by the property that fixes them
+    (theta = 0 is the direct sum: no node is accepted, every body is a source) and the accelerations
+    of 64 groups spread over the cloud, against the oracle's walk and against its direct sum (Eq. (1))."""
+    w = wl.make("c3")
+    assert w.n == 131072 and w.leaf_cap == 16
+    t = orc.build(w.pos, w.mass, w.leaf_cap)
+    ctx = gpu_build(w.pos, w.mass, w.leaf_cap)
+    assert_tree_equal(ctx, t)
+    sizes = np.diff(t.gstart.astype(np.int64))
+    inter_prev = None
+    for theta in (0.3, 0.5, 0.7, 1.0):
+        ref, nm, nd, kappa = orc.accel(t, theta, w.eps, w.G, want_kappa=True)
+        a = ctx.accel(theta, w.eps, w.G).cpu().numpy()
+        gm, gd = (x.cpu().numpy().view(np.uint32) for x in ctx.counts())
+        assert np.array_equal(gm, nm) and np.array_equal(gd, nd)
+        e = relerr(a, ref)
+        worst = int(np.argmax(e))
+        assert e.max() <= TOL, f"theta={theta}: max rel err {e.max():.3e} at body {worst} (kappa {kappa[worst]:.3g})"
+        st = bh.bh_get_stats(ctx.ctx)
+        inter = int(((nm.astype(np.int64) + nd) * sizes).sum())
+        assert st["interactions"] == inter
+        assert inter_prev is None or inter < inter_prev          # fewer interactions as theta grows (PAPER.md:211)
+        inter_prev = inter
+    # theta = 0
+    a0 = ctx.accel(0.0, w.eps, w.G).cpu().numpy()
+    gm, gd = (x.cpu().numpy().view(np.uint32) for x in ctx.counts())
+    assert not gm.any() and (gd == w.n).all()
+    st = bh.bh_get_stats(ctx.ctx)
+    assert st["interactions"] == w.n * w.n and st["n_mono"] == 0
+    ng = t.ngroups
+    picks = np.unique(np.linspace(0, ng - 1, 64).astype(np.int64))
+    rows_all = []
+    for g0 in picks:
+        ref, nm, nd, _ = orc.accel(t, 0.0, w.eps, w.G, int(g0), int(g0) + 1)
+        rows = t.perm[t.gstart[g0]:t.gstart[g0 + 1]]
+        assert nm[0] == 0 and nd[0] == w.n
+        assert relerr(a0[rows], ref[rows]).max() <= TOL
+        rows_all.append(rows)
+    rows_all = np.concatenate(rows_all).astype(np.int32)
+    refd = orc.direct(w.pos, w.mass, w.eps, w.G, targets=rows_all)
+    assert relerr(a0[rows_all], refd).max() <= 1e-13             # "equivalent to direct" (PAPER.md:211): same terms, other order
+    # the direct kernel on the same targets
+    b = ctx.direct(w.eps, w.G, targets=dev(rows_all, torch.int32)).cpu().numpy()
+    assert relerr(b, refd).max() <= TOL
+    ctx.close()
+
+
+def test_c5_after_fifty_kdk_steps():
+    """configs[4] as BASELINE.json states it: 50 leapfrog steps at N = 4 194 304, tree rebuilt every step
+    (PAPER.md:62).  Per evaluation on bit-identical inputs: the GPU's positions after step 50 go
+    to the oracle; its tree must equal the GPU's last build bit for bit, and its accelerations and list lengths
+    on sampled groups must match those of the GPU's last evaluation."""
+    w = wl.make("c5")
+    assert w.n == 4194304 and w.steps == 50
+    pos, vel, mass = dev(w.pos), dev(w.vel), dev(w.mass)
+    ctx = bh.Context(w.n, w.leaf_cap)
+    bh.bh_bind_state(ctx.ctx, pos, vel, mass, w.theta, w.eps, w.G)
+    for _ in range(w.steps):
+        bh.bh_kdk_step(ctx.ctx, w.dt)
+    bh.bh_synchronize(ctx.ctx)
+    p = pos.cpu().numpy()
+    assert np.isfinite(p).all() and np.abs(p - w.pos).max() > 0
+    t = orc.build(p, w.mass, w.leaf_cap)
+    ctx.n = w.n
+    assert_tree_equal(ctx, t)
+    a = torch.empty((w.n, 3), dtype=torch.float64, device="cuda")
+    bh.bh_copy_state_acc(ctx.ctx, a)
+    a = a.cpu().numpy()
+    gm, gd = (x.cpu().numpy().view(np.uint32) for x in ctx.counts())
+    ng = t.ngroups
+    for g0 in list(range(0, ng, ng // 12))[:12] + [ng - 2]:
+        ref, nm, nd, _ = orc.accel(t, w.theta, w.eps, w.G, g0, g0 + 2)
+        rows = t.perm[t.gstart[g0]:t.gstart[g0 + 2]]
+        assert np.array_equal(gm[g0:g0 + 2], nm) and np.array_equal(gd[g0:g0 + 2], nd)
+        assert relerr(a[rows], ref[rows]).max() <= TOL
+    ctx.close()
+
+
+@pytest.mark.parametrize("name,n,C,theta,sampled", [("c4", 30000, 1, 0.1, False), ("c3", 131072, 4, 0.0, True),
+                                                     ("c4", 100000, 1, 0.0, True)])
+def test_stack_spill_path(name, n, C, theta, sampled):
+    """Traversals whose LIFO stack of sibling ranges outgrows the 512 entries held in shared memory spill 128
+    entries at a time to the workspace and refill from it (deep trees, small theta: everything is opened).  The
+    spill counter of bh_get_stats proves the path ran; lists and accelerations must still equal the oracle's."""
+    w = wl.make(name, n)
+    t = orc.build(w.pos, w.mass, C)
+    ctx = gpu_build(w.pos, w.mass, C)
+    assert_tree_equal(ctx, t)
+    a = ctx.accel(theta, w.eps, w.G).cpu().numpy()
+    st = bh.bh_get_stats(ctx.ctx)
+    assert st["stack_spills"] > 0, "the walk's stack-spill path was not reached"
+    gm, gd = (x.cpu().numpy().view(np.uint32) for x in ctx.counts())
+    if theta == 0.0:
+        assert not gm.any() and (gd == n).all() and st["interactions"] == n * n
+    ng = t.ngroups
+    groups = np.unique(np.linspace(0, ng - 1, 48).astype(np.int64)) if sampled else [None]
+    for g0 in groups:
+        if g0 is None:
+            ref, nm, nd, _ = orc.accel(t, theta, w.eps, w.G)
+            assert np.array_equal(gm, nm) and np.array_equal(gd, nd)
+            assert relerr(a, ref).max() <= TOL
+        else:
+            g0 = int(g0)
+            ref, nm, nd, _ = orc.accel(t, theta, w.eps, w.G, g0, g0 + 1)
+            rows = t.perm[t.gstart[g0]:t.gstart[g0 + 1]]
+            assert gm[g0] == nm[0] and gd[g0] == nd[0]
+            assert relerr(a[rows], ref[rows]).max() <= TOL
+    ctx.close()
+
+
+# ---------------------------------------------------------------------------------------------------------
+# the grouping parameters of reading R6 are the oracle's: the CUDA path follows them at other values too
+@pytest.mark.parametrize("name,n,C,W,Gc", [("c4", 20000, 16, 32, 64), ("c3", 9000, 16, 8, 512), ("c1", 3000, 8, 1, 512),
+                                           ("c4", 5000, 4, 5, 20), ("c5", 12000, 32, 32, 2048), ("c2", 4000, 1, 1, 1)])
+def test_group_parameters_follow_the_oracle(name, n, C, W, Gc):
+    w = wl.make(name, n)
+    t = orc.build(w.pos, w.mass, C, W=W, Gc=Gc)
+    ctx = bh.Context(n, C, group_size=W, group_cell=Gc)
+    ctx.build(dev(w.pos), dev(w.mass))
+    assert_tree_equal(ctx, t)
+    for theta in (0.5, 0.9):
+        ref, nm, nd, _ = orc.accel(t, theta, w.eps, w.G)
+        a = ctx.accel(theta, w.eps, w.G).cpu().numpy()
+        gm, gd = (x.cpu().numpy().view(np.uint32) for x in ctx.counts())
+        assert np.array_equal(gm, nm) and np.array_equal(gd, nd)
+        assert relerr(a, ref).max() <= TOL
+    ctx.close()
+
+
+def test_per_body_walk_is_the_papers_and_group_walk_opens_a_superset():
+    """W = 1, C = 1 on the GPU is the paper's own tree and walk.  The group reading R6
+    (W = 32) accepts a node only if every member's own test accepts it, so per body it evaluates at least the
+    interactions of the per-body walk, and is at least as close to the direct sum on average."""
+    w = wl.make("c1", 2000)
+    pos, mass = dev(w.pos), dev(w.mass)
+    one = bh.Context(w.n, 1, group_size=1)
+    one.build(pos, mass)
+    t1 = orc.build(w.pos, w.mass, 1, W=1)
+    assert_tree_equal(one, t1)
+    a1 = one.accel(0.5, w.eps, w.G).cpu().numpy()
+    ref1, nm1, nd1, _ = orc.accel(t1, 0.5, w.eps, w.G)
+    g1m, g1d = (x.cpu().numpy().view(np.uint32) for x in one.counts())
+    assert np.array_equal(g1m, nm1) and np.array_equal(g1d, nd1)
+    assert relerr(a1, ref1).max() <= TOL
+    grp = bh.Context(w.n, 1)
+    grp.build(pos, mass)
+    a32 = grp.accel(0.5, w.eps, w.G).cpu().numpy()
+    i1 = bh.bh_get_stats(one.ctx)["interactions"]
+    i32 = bh.bh_get_stats(grp.ctx)["interactions"]
+    assert i32 >= i1
+    d = orc.direct(w.pos, w.mass, w.eps, w.G)
+    assert np.median(relerr(a32, d)) <= np.median(relerr(a1, d))
+    one.close()
+    grp.close()
+
+
+# ---------------------------------------------------------------------------------------------------------
+# the documented range of the input (include/bh.h)
+@pytest.mark.parametrize("k", [-300, -150, 150, 299])
+def test_extreme_scales(k):
+    """Positions and masses scaled by 2^k (accelerations then scale by 2^-k; m x and m / r^3 stay far from the ends
+    of the exponent range, as bh.h asks): the keys, the tree and the list lengths do not change (power-of-two
+    scalings are exact), the monopoles scale exactly, and the accelerations match the oracle at the scaled
+    inputs.  k = -300 and 299 are the edges of the documented extent range."""
+    w = wl.make("c3", 6000)
+    t0 = orc.build(w.pos, w.mass, 16)
+    sc = float(np.ldexp(1.0, k))
+    pos, mass, eps = w.pos * sc, w.mass * sc, w.eps * sc
+    t = orc.build(pos, mass, 16)
+    assert np.array_equal(t.skey, t0.skey) and np.array_equal(t.gstart, t0.gstart) and t.M == t0.M
+    assert np.array_equal(t.mono, t0.mono * sc)
+    ctx = gpu_build(pos, mass, 16)
+    assert_tree_equal(ctx, t)
+    for theta in (0.0, 0.5, 1.0):
+        ref, nm, nd, _ = orc.accel(t, theta, eps, w.G)
+        a = ctx.accel(theta, eps, w.G).cpu().numpy()
+        gm, gd = (x.cpu().numpy().view(np.uint32) for x in ctx.counts())
+        assert np.array_equal(gm, nm) and np.array_equal(gd, nd)
+        assert np.isfinite(a).all() and relerr(a, ref).max() <= TOL
+    ctx.close()
+
+
+def test_extent_outside_documented_range_is_reported():
+    w = wl.make("c1", 500)
+    ctx = bh.Context(w.n, 8)
+    for k in (-320, 320):
+        ctx.build(dev(w.pos * float(np.ldexp(1.0, k))), dev(w.mass))
+        with pytest.raises(bh.BhError) as e:
+            bh.bh_synchronize(ctx.ctx)
+        assert e.value.status == bh.BH_ERR_INVALID_ARG and "extent" in str(e.value)
+    ctx.build(dev(w.pos), dev(w.mass))
+    bh.bh_synchronize(ctx.ctx)
+    ctx.close()
+
+
+def test_tiny_softening_is_treated_as_none():
+    """0 < eps^2 < smallest normal double: the self term and coincident pairs have a subnormal softened distance;
+    they must contribute nothing (bh.h), exactly as with eps = 0 — not infinity times zero."""
+    rng = np.random.default_rng(11)
+    pos = np.concatenate([rng.random((300, 3)), np.full((5, 3), 0.5)])
+    mass = np.full(len(pos), 1.0 / len(pos))
+    ctx = gpu_build(pos, mass, 4)
+    a0 = ctx.accel(0.5, 0.0, 1.0).cpu().numpy()
+    a1 = ctx.accel(0.5, 1e-160, 1.0).cpu().numpy()
+    d0 = ctx.direct(0.0, 1.0).cpu().numpy()
+    d1 = ctx.direct(1e-160, 1.0).cpu().numpy()
+    assert np.isfinite(a1).all() and np.array_equal(a0, a1) and np.array_equal(d0, d1)
+    ref = orc.accel(orc.build(pos, mass, 4), 0.5, 1e-160, 1.0)[0]
+    assert relerr(a1, ref).max() <= TOL
+    ctx.close()
+
+
+def test_device_errors_are_sticky_until_reported():
+    """A non-finite coordinate seen by one build is reported by the next synchronising call even if another,
+    clean, build ran in between; once reported it is cleared (bh.h)."""
+    w = wl.make("c1", 1024)
+    bad = w.pos.copy()
+    bad[5, 0] = np.inf
+    ctx = bh.Context(w.n, 8)
+    ctx.build(dev(bad), dev(w.mass))
+    ctx.build(dev(w.pos), dev(w.mass))
+    with pytest.raises(bh.BhError) as e:
+        bh.bh_synchronize(ctx.ctx)
+    assert e.value.status == bh.BH_ERR_NONFINITE
+    bh.bh_synchronize(ctx.ctx)
+    ctx.build(dev(w.pos), dev(w.mass))
+    assert_tree_equal(ctx, orc.build(w.pos, w.mass, 8))
     ctx.close()
