@@ -127,6 +127,19 @@ bh_status do_build(bh_ctx *c, const double *pos, const double *mass, int64_t n, 
     cudaStream_t s = c->stream;
     c->built = false;
     c->walked = false;
+    if (n <= kSortTile) {   // one block does the whole build (and its own clearing): one launch
+        if (mass_ready) cudaStreamWaitEvent(s, mass_ready, 0);   // masses copied on another stream
+        {
+            Phase p(c, 4);
+            launch_build_small(w, pos, mass, n, s);
+        }
+        bh_status st1 = cuda_check(c, cudaGetLastError(), "bh_build launch");
+        if (st1 != BH_OK) return st1;
+        c->n = n;
+        c->built = true;
+        c->launches += 1;
+        return BH_OK;
+    }
     int sort_launches = 0;
     // cleared per build, sized by n (not by max_n): histograms + tickets + look-back words of this n's tiles,
     // and the child masks / arrival counters of the nodes n bodies can make
@@ -169,9 +182,9 @@ bh_status do_build(bh_ctx *c, const double *pos, const double *mass, int64_t n, 
 bh_status do_accel(bh_ctx *c, double theta, double eps, double G, double *acc, int mode = 0, double *phi = nullptr)
 {
     const Workspace &w = c->ws;
-    // reset the group queue and the counters of this evaluation
-    cudaMemsetAsync(&w.st->walk_queue, 0, sizeof(unsigned), c->stream);
-    cudaMemsetAsync(&w.st->stats[0], 0, kNumStats * sizeof(unsigned long long), c->stream);
+    // The counters of this evaluation: the build zeroes them, so only a second walk of the same build clears
+    // them here.  The group queue is reset by the walk kernel itself when its last producer warp leaves.
+    if (c->walked) cudaMemsetAsync(&w.st->stats[0], 0, kNumStats * sizeof(unsigned long long), c->stream);
     {
         Phase p(c, 6);
         launch_walk(w, c->n, theta, eps, G, acc, mode, phi, c->stream);

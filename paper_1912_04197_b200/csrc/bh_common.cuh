@@ -43,7 +43,8 @@ struct DevState {
     unsigned n_groups;     // Ng walk groups
     unsigned lvl_start[kLevels + 1];   // first node id of each level (lvl_start[kLevels] = M)
     unsigned ticket_bbox;  // last-block election
-    unsigned walk_queue;   // dynamic group counter of the walk
+    unsigned walk_queue;   // dynamic group counter of the walk (reset by the walk's last producer warp)
+    unsigned walk_done;    // producer warps that have left the walk
     unsigned ticket_diag;  // last-block election of the diagnostics reduction (resets itself)
     unsigned long long pair_count;     // broad phase: candidate pairs found (may exceed the caller's capacity)
     unsigned long long agg_counts[3];  // aggregates: connected components, aggregates (size > 1), bad pairs
@@ -120,6 +121,8 @@ Workspace carve(char *base, int64_t max_n, int leaf_cap);
 void launch_cube(const Workspace &w, const double *pos, int64_t n, cudaStream_t s);
 void launch_keys(const Workspace &w, const double *pos, int64_t n, cudaStream_t s);
 int launch_sort(const Workspace &w, int64_t n, cudaStream_t s);   // result in key[0]/idx[0]; returns the launches
+// steps a1-a6 in one kernel of one block, n <= kSortTile (bh_small.cu); needs no prior clearing
+void launch_build_small(const Workspace &w, const double *pos, const double *mass, int64_t n, cudaStream_t s);
 void launch_gather(const Workspace &w, const double *pos, const double *mass, int64_t n, cudaStream_t s);
 // (x,y,z,m) in the caller's body order with the identity permutation: input of a direct sum without a tree
 void launch_pack(const Workspace &w, const double *pos, const double *mass, int64_t n, cudaStream_t s);

@@ -1,15 +1,10 @@
 // bh_keys.cu — step a1 (canonical bounding cube) and step a2 (63-bit Morton keys over
 // that cube, plus the digit histograms of all eight radix passes).  HBM-streaming kernels.
-#include "bh_common.cuh"
+#include "bh_keys.cuh"
 
 namespace bh {
 
 constexpr int kCubeThreads = 192;   // multiple of 3: a thread always sees the same axis
-
-__device__ __forceinline__ bool nonfinite(double x)
-{
-    return (__double2hiint(x) & 0x7ff00000) == 0x7ff00000;
-}
 
 // One pass over the flat [3n] coordinate array; per-block partial (min, max, bad) to part[blk][8];
 // the last block to finish reduces the partials and derives the cube (R11): corner = per-axis
@@ -93,54 +88,8 @@ __global__ void __launch_bounds__(kCubeThreads) cube_kernel(const double *__rest
             lo[a] = smn[a];
             hi[a] = smx[a];
         }
-        bad = sbad[0] | sbad[1] | sbad[2];
-        double E = 0.0;
-        for (int a = 0; a < 3; ++a) E = fmax(E, __dsub_rn(hi[a], lo[a]));   // one rounding per extent
-        if (nonfinite(E)) bad = 1;
-        int e = 0;
-        if (bad) {   // keep every later kernel memory-safe; the error is reported by the host
-            lo[0] = lo[1] = lo[2] = 0.0;
-        } else if (E != 0.0) {
-            (void)frexp(E, &e);   // E = f 2^e, 1/2 <= f < 1  =>  2^(e-1) <= E < 2^e
-        }
-        st->lo[0] = lo[0];
-        st->lo[1] = lo[1];
-        st->lo[2] = lo[2];
-        st->e = e;
-        st->side = ldexp(1.0, e);
-        st->scale = ldexp(1.0, 21 - e);
-        // sticky error bits: OR-ed in, cleared by the host once it has reported them (bh.h)
-        int flags = bad ? (int)kStatNonFinite : 0;
-        if (!bad && E != 0.0 && (e < -kMaxExtentExp + 1 || e > kMaxExtentExp + 1)) flags |= (int)kStatRange;
-        if (flags) atomicOr(&st->status, flags);
-        st->n_nodes = 0;
-        st->n_groups = 0;
-        st->depth = 0;
-        st->ticket_bbox = 0;
-        st->walk_queue = 0;
-        for (int k = 0; k < kNumStats; ++k) st->stats[k] = 0ull;
+        finish_cube(lo, hi, sbad[0] | sbad[1] | sbad[2], st);
     }
-}
-
-// spread the low 21 bits of v so that bit k lands on bit 3k
-__device__ __forceinline__ unsigned long long spread3(unsigned v)
-{
-    unsigned long long x = v & 0x1fffffu;
-    x = (x | (x << 32)) & 0x001f00000000ffffull;
-    x = (x | (x << 16)) & 0x001f0000ff0000ffull;
-    x = (x | (x << 8)) & 0x100f00f00f00f00full;
-    x = (x | (x << 4)) & 0x10c30c30c30c30c3ull;
-    x = (x | (x << 2)) & 0x1249249249249249ull;
-    return x;
-}
-
-__device__ __forceinline__ unsigned quantise(double x, double lo, double scale)
-{
-    // one rounded subtraction, exact power-of-two scaling, truncation (R11/R12); the clamp is a
-    // no-op for finite input (x - lo <= extent < L) and keeps non-finite input memory-safe
-    double d = __dmul_rn(__dsub_rn(x, lo), scale);
-    d = fmin(fmax(d, 0.0), 2097151.0);
-    return (unsigned)__double2uint_rz(d);
 }
 
 // keys + the 8 x 256 digit histograms (shared-memory atomics, flushed once per block)
@@ -155,10 +104,7 @@ __global__ void __launch_bounds__(256) keys_kernel(const double *__restrict__ po
     const double lx = st->lo[0], ly = st->lo[1], lz = st->lo[2], sc = st->scale;
     for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n;
          i += (long long)gridDim.x * blockDim.x) {
-        unsigned qx = quantise(__ldg(pos + 3 * i + 0), lx, sc);
-        unsigned qy = quantise(__ldg(pos + 3 * i + 1), ly, sc);
-        unsigned qz = quantise(__ldg(pos + 3 * i + 2), lz, sc);
-        unsigned long long k = spread3(qx) | (spread3(qy) << 1) | (spread3(qz) << 2);
+        const unsigned long long k = morton_key(__ldg(pos + 3 * i + 0), __ldg(pos + 3 * i + 1), __ldg(pos + 3 * i + 2), lx, ly, lz, sc);
         key[i] = k;
 #pragma unroll
         for (int p = 0; p < kSortPasses; ++p)

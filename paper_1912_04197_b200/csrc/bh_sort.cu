@@ -4,7 +4,7 @@
 // the tile's global digit offsets with a decoupled look-back over the tiles before it, and scatters
 // through shared memory so that the global writes are runs of consecutive addresses per digit.
 // The global digit histograms of all passes were accumulated by keys_kernel.
-#include "bh_common.cuh"
+#include "bh_sort.cuh"
 
 namespace bh {
 
@@ -21,26 +21,6 @@ __device__ __forceinline__ unsigned ld_relaxed(const unsigned *p)
 __device__ __forceinline__ void st_relaxed(unsigned *p, unsigned v)
 {
     asm volatile("st.relaxed.gpu.global.u32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
-}
-
-// exclusive scan of one value per thread over a 256-thread block; tmp is 8 words of shared memory
-__device__ __forceinline__ unsigned block_excl_scan_256(unsigned v, unsigned *tmp)
-{
-    const unsigned lane = threadIdx.x & 31u, warp = threadIdx.x >> 5;
-    unsigned inc = v;
-#pragma unroll
-    for (int o = 1; o < 32; o <<= 1) {
-        unsigned t = __shfl_up_sync(0xffffffffu, inc, o);
-        if (lane >= (unsigned)o) inc += t;
-    }
-    if (lane == 31) tmp[warp] = inc;
-    __syncthreads();
-    unsigned base = 0;
-#pragma unroll
-    for (int k = 0; k < 8; ++k)
-        if ((unsigned)k < warp) base += tmp[k];
-    __syncthreads();
-    return base + inc - v;
 }
 
 #ifndef BH_SORT_MINBLOCKS
@@ -160,89 +140,9 @@ sort_pass_kernel(const unsigned long long *__restrict__ kin, const unsigned *__r
     }
 }
 
-// n <= one tile: all eight digit passes inside one block, keys and values staying in registers and
-// shared memory between passes (a step over a few thousand bodies is bound by the latency of its
-// dependent launches, "for a low number of bodies the computational time is dominated by
-// the octree creation": eight launches become one).  Same per-warp match.any ranking, same stable order.
-__global__ void __launch_bounds__(kSortThreads)
-sort_small_kernel(const unsigned long long *kin, unsigned long long *kout, unsigned *__restrict__ vout, int n)
-{
-    __shared__ unsigned long long skey[kSortTile];          // 32 KB, reused for the values
-    __shared__ unsigned whist[kSortThreads / 32][kRadix];
-    __shared__ unsigned stoff[kRadix];
-    __shared__ unsigned stmp[8];
-    const unsigned tid = threadIdx.x, lane = tid & 31u, warp = tid >> 5;
-    const unsigned lt = (1u << lane) - 1u;
-    unsigned long long k[kSortItems];
-    unsigned v[kSortItems];
-    unsigned pos[kSortItems];
-#pragma unroll
-    for (int i = 0; i < kSortItems; ++i) {
-        const int idx = warp * (32 * kSortItems) + i * 32 + lane;
-        k[i] = idx < n ? kin[idx] : ~0ull;      // padding sorts last in every pass (all digits 255, after the real 255s: stable)
-        v[i] = (unsigned)idx;
-    }
-#pragma unroll 1
-    for (int p = 0; p < kSortPasses; ++p) {
-        const int shift = p * kRadixBits;
-#pragma unroll
-        for (int w = 0; w < kSortThreads / 32; ++w) whist[w][tid] = 0u;
-        __syncthreads();
-#pragma unroll
-        for (int i = 0; i < kSortItems; ++i) {
-            const unsigned d = (unsigned)(k[i] >> shift) & (kRadix - 1);
-            const unsigned peers = __match_any_sync(0xffffffffu, d);
-            const unsigned pre = whist[warp][d];
-            __syncwarp();
-            if ((peers & lt) == 0u) whist[warp][d] = pre + __popc(peers);
-            __syncwarp();
-            pos[i] = pre + __popc(peers & lt);
-        }
-        __syncthreads();
-        unsigned tot = 0;
-#pragma unroll
-        for (int w = 0; w < kSortThreads / 32; ++w) {
-            const unsigned c = whist[w][tid];
-            whist[w][tid] = tot;
-            tot += c;
-        }
-        stoff[tid] = block_excl_scan_256(tot, stmp);
-        __syncthreads();
-#pragma unroll
-        for (int i = 0; i < kSortItems; ++i) {
-            const unsigned d = (unsigned)(k[i] >> shift) & (kRadix - 1);
-            pos[i] += stoff[d] + whist[warp][d];
-            skey[pos[i]] = k[i];
-        }
-        __syncthreads();
-#pragma unroll
-        for (int i = 0; i < kSortItems; ++i) k[i] = skey[warp * (32 * kSortItems) + i * 32 + lane];
-        __syncthreads();
-        unsigned *sval = reinterpret_cast<unsigned *>(skey);
-#pragma unroll
-        for (int i = 0; i < kSortItems; ++i) sval[pos[i]] = v[i];
-        __syncthreads();
-#pragma unroll
-        for (int i = 0; i < kSortItems; ++i) v[i] = sval[warp * (32 * kSortItems) + i * 32 + lane];
-        __syncthreads();
-    }
-#pragma unroll
-    for (int i = 0; i < kSortItems; ++i) {
-        const int idx = warp * (32 * kSortItems) + i * 32 + lane;
-        if (idx < n) {
-            kout[idx] = k[i];
-            vout[idx] = v[i];
-        }
-    }
-}
-
 int launch_sort(const Workspace &w, int64_t n, cudaStream_t s)
 {
-    const int tiles = (int)((n + kSortTile - 1) / kSortTile);
-    if (tiles == 1) {   // result in key[0] / idx[0], as after the eight passes below
-        sort_small_kernel<<<1, kSortThreads, 0, s>>>(w.key[0], w.key[0], w.idx[0], (int)n);
-        return 1;
-    }
+    const int tiles = (int)((n + kSortTile - 1) / kSortTile);   // one tile: the whole build is one block (bh_small.cu)
     for (int p = 0; p < kSortPasses; ++p) {
         const int a = p & 1, b = a ^ 1;
         unsigned *lb = w.lookback + (size_t)p * tiles * kRadix;   // [pass][tiles of this n][256]: cleared per build

@@ -19,7 +19,7 @@
 //     glev_j = min(leaf_j, 1 + max_{s in [j-Gc, j]} (digits shared by keys s and s+Gc))
 // and body j starts a group iff its distance to the first body of its group cell is a multiple of
 // W.  Group starts are counted and ranked like one more "level" (row kLevels of the histograms).
-#include "bh_common.cuh"
+#include "bh_tree.cuh"
 
 namespace bh {
 
@@ -52,85 +52,15 @@ __global__ void __launch_bounds__(256) pack_kernel(const double *__restrict__ po
     iperm[i] = (unsigned)i;
 }
 
-// exact bounding box of every walk group (one warp per group, lanes stride over its bodies)
 __global__ void __launch_bounds__(256) group_box_kernel(const DevState *__restrict__ st,
                                                         const unsigned *__restrict__ gstart,
                                                         const double4 *__restrict__ sbody,
                                                         double *__restrict__ gbox)
 {
-    const unsigned ng = st->n_groups;
-    const unsigned lane = lane_id();
-    const double inf = __longlong_as_double(0x7ff0000000000000ll);
-    for (unsigned g = (blockIdx.x * blockDim.x + threadIdx.x) >> 5; g < ng; g += (gridDim.x * blockDim.x) >> 5) {
-        const unsigned b = gstart[g], e = gstart[g + 1];
-        double lx = inf, ly = inf, lz = inf, hx = -inf, hy = -inf, hz = -inf;
-        for (unsigned j = b + lane; j < e; j += 32) {
-            const double4 p = sbody[j];
-            lx = fmin(lx, p.x); ly = fmin(ly, p.y); lz = fmin(lz, p.z);
-            hx = fmax(hx, p.x); hy = fmax(hy, p.y); hz = fmax(hz, p.z);
-        }
-#pragma unroll
-        for (int o = 16; o > 0; o >>= 1) {
-            lx = fmin(lx, __shfl_xor_sync(0xffffffffu, lx, o));
-            ly = fmin(ly, __shfl_xor_sync(0xffffffffu, ly, o));
-            lz = fmin(lz, __shfl_xor_sync(0xffffffffu, lz, o));
-            hx = fmax(hx, __shfl_xor_sync(0xffffffffu, hx, o));
-            hy = fmax(hy, __shfl_xor_sync(0xffffffffu, hy, o));
-            hz = fmax(hz, __shfl_xor_sync(0xffffffffu, hz, o));
-        }
-        if (lane == 0) {
-            double *q = gbox + 6ull * g;
-            q[0] = lx; q[1] = ly; q[2] = lz; q[3] = hx; q[4] = hy; q[5] = hz;
-        }
-    }
+    group_boxes(st->n_groups, (blockIdx.x * blockDim.x + threadIdx.x) >> 5, (gridDim.x * blockDim.x) >> 5, gstart, sbody, gbox);
 }
 
 // ------------------------------------------------------------------------------------------ a5
-// sliding maximum over windows of k consecutive entries of a[0..len): after the call a[i] holds
-// max(a[i .. i+2^p-1]) with p = floor(log2 k); the caller combines a[i] and a[i + k - 2^p].
-__device__ __forceinline__ int window_doubling(signed char *a, int len, int k)
-{
-    int p = 0;
-    while ((2 << p) <= k) ++p;
-    for (int r = 0; r < p; ++r) {
-        const int h = 1 << r;
-        signed char v[12];   // len <= kTreeTile + 1024 + 1, 256 threads
-        int c = 0;
-        for (int i = threadIdx.x; i < len; i += blockDim.x, ++c) {
-            signed char x = a[i];
-            if (i + h < len) x = max(x, a[i + h]);
-            v[c] = x;
-        }
-        __syncthreads();
-        c = 0;
-        for (int i = threadIdx.x; i < len; i += blockDim.x, ++c) a[i] = v[c];
-        __syncthreads();
-    }
-    return 1 << p;
-}
-
-// first index <= j whose key shares its leading `lvl` digits with key j (galloping search)
-__device__ __forceinline__ unsigned range_begin(const unsigned long long *__restrict__ skey, unsigned j, int lvl)
-{
-    if (lvl == 0) return 0u;
-    const int sh = 63 - 3 * lvl;
-    const unsigned long long pre = skey[j] >> sh;
-    unsigned hi = j, step = 1, lo;          // invariant: key[hi] has the prefix
-    while (true) {
-        if (hi < step) { lo = 0u; if ((skey[0] >> sh) == pre) return 0u; break; }
-        lo = hi - step;
-        if ((skey[lo] >> sh) != pre) break;
-        hi = lo;
-        step <<= 1;
-    }
-    // key[lo] lacks the prefix, key[hi] has it: answer in (lo, hi]
-    while (hi - lo > 1) {
-        unsigned mid = lo + ((hi - lo) >> 1);
-        if ((skey[mid] >> sh) == pre) hi = mid; else lo = mid;
-    }
-    return hi;
-}
-
 // Kernel A: per body (d+1, leaf, group-start flag) and per-tile counts of nodes per level and of
 // group starts.
 __global__ void __launch_bounds__(256) tree_levels_kernel(const unsigned long long *__restrict__ skey,
@@ -139,112 +69,19 @@ __global__ void __launch_bounds__(256) tree_levels_kernel(const unsigned long lo
 {
     extern __shared__ signed char sw[];   // [kTreeTile + C] leaf windows, then [kTreeTile + Gc] group windows
     __shared__ unsigned shist[kLevels + 1];
-    signed char *swc = sw;
-    signed char *swg = sw + kTreeTile + C;
-    const long long t0 = (long long)blockIdx.x * kTreeTile;
-    if (threadIdx.x <= kLevels) shist[threadIdx.x] = 0u;
-    for (int k = threadIdx.x; k < kTreeTile + C; k += blockDim.x) {
-        long long s = t0 - C + k;
-        int wv = -1;
-        if (s >= 0 && s + C < n) wv = common_levels(skey[s], skey[s + C]);
-        swc[k] = (signed char)wv;
-    }
-    for (int k = threadIdx.x; k < kTreeTile + Gc; k += blockDim.x) {
-        long long s = t0 - Gc + k;
-        int wv = -1;
-        if (s >= 0 && s + Gc < n) wv = common_levels(skey[s], skey[s + Gc]);
-        swg[k] = (signed char)wv;
-    }
-    __syncthreads();
-    const int pc = window_doubling(swc, kTreeTile + C, C + 1);
-    const int pg = window_doubling(swg, kTreeTile + Gc, Gc + 1);
-    for (int k = threadIdx.x; k < kTreeTile; k += blockDim.x) {
-        long long j = t0 + k;
-        if (j >= n) break;
-        // windows of C+1 (Gc+1) bodies that start at j-C .. j  (j-Gc .. j)
-        const int mw = max((int)swc[k], (int)swc[k + C + 1 - pc]);
-        const int mg = max((int)swg[k], (int)swg[k + Gc + 1 - pg]);
-        const int leaf = min(kMaxLevel, mw + 1);
-        const int glev = min(leaf, mg + 1);
-        const int d = (j == 0) ? -1 : common_levels(skey[j - 1], skey[j]);
-        const unsigned cb = range_begin(skey, (unsigned)j, glev);
-        const bool gs = (((unsigned)j - cb) % (unsigned)W) == 0u;
-        dlev[j] = make_uchar4((unsigned char)(d + 1), (unsigned char)leaf, gs ? 1 : 0, (unsigned char)glev);
-        for (int l = d + 1; l <= leaf; ++l) atomicAdd(&shist[l], 1u);
-        if (gs) atomicAdd(&shist[kLevels], 1u);
-    }
-    __syncthreads();
-    if (threadIdx.x <= kLevels) tile_lvl[(size_t)threadIdx.x * ntiles + blockIdx.x] = shist[threadIdx.x];
+    tree_levels_tile(skey, n, C, Gc, W, dlev, tile_lvl, ntiles, blockIdx.x, sw, shist);
 }
 
-// Kernel B (one block, one warp per level): exclusive scan of the tile counts of each level, level
-// starts, node count, depth.
+// Kernel B (one block): exclusive scan of the tile counts of each level, level starts, node count, depth.
 __global__ void __launch_bounds__((kLevels + 1) * 32) tree_scan_kernel(unsigned *tile_lvl, int ntiles, DevState *st,
                                                                        long long node_cap, unsigned *gstart,
                                                                        unsigned n)
 {
     __shared__ unsigned stot[kLevels + 1];
-    const int l = threadIdx.x >> 5;
-    const unsigned lane = lane_id();
-    unsigned *row = tile_lvl + (size_t)l * ntiles;
-    unsigned run = 0;
-    for (int b = 0; b < ntiles; b += 32) {
-        int t = b + lane;
-        unsigned v = t < ntiles ? row[t] : 0u;
-        unsigned inc = v;
-#pragma unroll
-        for (int o = 1; o < 32; o <<= 1) {
-            unsigned u = __shfl_up_sync(0xffffffffu, inc, o);
-            if (lane >= (unsigned)o) inc += u;
-        }
-        if (t < ntiles) row[t] = run + inc - v;
-        run += __shfl_sync(0xffffffffu, inc, 31);
-    }
-    if (lane == 0) stot[l] = run;
-    __syncthreads();
-    if (threadIdx.x == 0) {
-        unsigned acc = 0;
-        int depth = 0;
-        for (int k = 0; k < kLevels; ++k) {
-            st->lvl_start[k] = acc;
-            acc += stot[k];
-            if (stot[k]) depth = k;
-        }
-        st->lvl_start[kLevels] = acc;
-        st->n_nodes = (int)acc;
-        st->depth = depth;
-        st->n_groups = stot[kLevels];
-        gstart[stot[kLevels]] = n;
-        if ((long long)acc > node_cap) st->status |= kStatCapacity;
-    }
+    tree_scan_block(tile_lvl, ntiles, st, node_cap, gstart, n, stot);
 }
 
-// first index > j (<= n) whose key differs from key j in its leading `lvl` digits (galloping search)
-__device__ __forceinline__ unsigned range_end(const unsigned long long *__restrict__ skey, unsigned n,
-                                              unsigned j, int lvl)
-{
-    if (lvl == 0) return n;
-    const int sh = 63 - 3 * lvl;
-    const unsigned long long pre = skey[j] >> sh;
-    unsigned lo = j, step = 1;               // invariant: key[lo] has the prefix
-    unsigned hi;
-    while (true) {
-        hi = lo + step;
-        if (hi >= n) { hi = n; break; }
-        if ((skey[hi] >> sh) != pre) break;
-        lo = hi;
-        step <<= 1;
-    }
-    // answer in (lo, hi]
-    while (hi - lo > 1) {
-        unsigned mid = lo + ((hi - lo) >> 1);
-        if ((skey[mid] >> sh) == pre) lo = mid; else hi = mid;
-    }
-    return hi;
-}
-
-// Kernel C: emit the nodes.  One warp handles 32 consecutive bodies at a time; for each level a
-// ballot gives the rank of the bodies that start a node there.
+// Kernel C: emit the nodes.
 __global__ void __launch_bounds__(256) tree_emit_kernel(const unsigned long long *__restrict__ skey, long long n,
                                                         const uchar4 *__restrict__ dlev,
                                                         const unsigned *__restrict__ tile_lvl, int ntiles,
@@ -254,90 +91,13 @@ __global__ void __launch_bounds__(256) tree_emit_kernel(const unsigned long long
                                                         int *__restrict__ nfirst, int *__restrict__ nparent,
                                                         unsigned *node_meta, unsigned *__restrict__ gstart)
 {
-    constexpr int kChunks = kTreeTile / 32;          // 32 chunks of 32 bodies
-    __shared__ unsigned scnt[kChunks][kLevels + 1];  // per chunk, per level (+ group starts): counts -> bases
+    __shared__ unsigned scnt[kTreeTile / 32][kLevels + 1];  // per chunk, per level (+ group starts): counts -> bases
     __shared__ unsigned sstart[kLevels + 1];
-    const unsigned lane = lane_id(), warp = threadIdx.x >> 5;
-    const long long t0 = (long long)blockIdx.x * kTreeTile;
-    if (threadIdx.x <= kLevels) sstart[threadIdx.x] = st->lvl_start[threadIdx.x];
-    if ((long long)st->n_nodes > node_cap) return;   // flagged by the scan kernel; stay in bounds
-    // phase 1: per chunk level counts
-    for (int c = warp; c < kChunks; c += 8) {
-        long long j = t0 + c * 32 + lane;
-        uchar4 dl = j < n ? dlev[j] : make_uchar4(255, 0, 0, 0);
-#pragma unroll
-        for (int l = 0; l < kLevels; ++l) {
-            unsigned b = __ballot_sync(0xffffffffu, (int)dl.x <= l && l <= (int)dl.y);
-            if (lane == 0) scnt[c][l] = __popc(b);
-        }
-        unsigned bg = __ballot_sync(0xffffffffu, dl.z != 0);
-        if (lane == 0) scnt[c][kLevels] = __popc(bg);
-    }
-    __syncthreads();
-    if (threadIdx.x <= kLevels) {
-        unsigned run = tile_lvl[(size_t)threadIdx.x * ntiles + blockIdx.x];
-        for (int c = 0; c < kChunks; ++c) {
-            unsigned v = scnt[c][threadIdx.x];
-            scnt[c][threadIdx.x] = run;
-            run += v;
-        }
-    }
-    __syncthreads();
-    // phase 2: ids and emission
-    const unsigned le = (lane == 31) ? 0xffffffffu : ((2u << lane) - 1u);
-    for (int c = warp; c < kChunks; c += 8) {
-        long long j = t0 + c * 32 + lane;
-        uchar4 dl = j < n ? dlev[j] : make_uchar4(255, 0, 0, 0);
-        const int first = dl.x, leaf = dl.y;
-        {   // group starts, numbered in sorted-body order
-            const unsigned bg = __ballot_sync(0xffffffffu, dl.z != 0);
-            if (dl.z) gstart[scnt[c][kLevels] + __popc(bg & le) - 1u] = (unsigned)j;
-        }
-        // inclusive per-level counts at this body: prev (l-1), cur (l), next (l+1)
-        unsigned pprev = 0, pcur, pnext;
-        {
-            unsigned b = __ballot_sync(0xffffffffu, first <= 0 && 0 <= leaf);
-            pcur = scnt[c][0] + __popc(b & le);
-        }
-#pragma unroll 1
-        for (int l = 0; l < kLevels; ++l) {
-            pnext = 0;
-            if (l + 1 < kLevels) {
-                unsigned b = __ballot_sync(0xffffffffu, first <= l + 1 && l + 1 <= leaf);
-                pnext = scnt[c][l + 1] + __popc(b & le);
-            }
-            if (first <= l && l <= leaf) {
-                const unsigned id = sstart[l] + pcur - 1u;
-                const int par = l ? (int)(sstart[l - 1] + pprev - 1u) : -1;
-                const bool internal = l < leaf;
-                nlevel[id] = (unsigned char)l;
-                nbegin[id] = (unsigned)j;
-                ncount[id] = range_end(skey, (unsigned)n, (unsigned)j, l) - (unsigned)j;
-                nfirst[id] = internal ? (int)(sstart[l + 1] + pnext - 1u) : -1;
-                nparent[id] = par;
-                if (l) {   // record my octant in the parent's child mask
-                    unsigned oct = (unsigned)(skey[j] >> (63 - 3 * l)) & 7u;
-                    atomicOr(&node_meta[par], 1u << oct);
-                }
-            }
-            pprev = pcur;
-            pcur = pnext;
-        }
-    }
+    tree_emit_tile(skey, n, dlev, tile_lvl, ntiles, blockIdx.x, st, node_cap, nlevel, nbegin, ncount, nfirst, nparent,
+                   node_meta, gstart, scnt, sstart);
 }
 
 // ------------------------------------------------------------------------------------------ a6
-// Monopoles by arrival counters: a thread computes each leaf from its bodies, then climbs; the last
-// child to arrive at a parent (counter in node_meta bits 8..) computes it from ALL children in
-// ascending id, so the arithmetic order is fixed (bit-reproducible): masses added left to right,
-// weighted sums by fma from 0, one IEEE division.
-__device__ __forceinline__ double4 ldcg4(const double4 *p)
-{
-    const double2 *q = reinterpret_cast<const double2 *>(p);
-    double2 a = __ldcg(q), b = __ldcg(q + 1);
-    return make_double4(a.x, a.y, b.x, b.y);
-}
-
 __global__ void __launch_bounds__(256) monopole_kernel(const DevState *__restrict__ st,
                                                        const double4 *__restrict__ sbody,
                                                        const unsigned *__restrict__ nbegin,
@@ -350,53 +110,8 @@ __global__ void __launch_bounds__(256) monopole_kernel(const DevState *__restric
 {
     const int M = st->n_nodes;
     if ((long long)M > node_cap) return;
-    for (int t = blockIdx.x * blockDim.x + threadIdx.x; t < M; t += gridDim.x * blockDim.x) {
-        // the walk's packed record of this node (the child mask is complete: bits 0-7 are only
-        // written by tree_emit_kernel)
-        const int first = nfirst[t];
-        const unsigned kids = (unsigned)__popc(__ldcg(node_meta + t) & 0xffu);
-        winfo[t] = make_uint4(nbegin[t], ncount[t], (unsigned)first, (unsigned)nlevel[t] | (kids << 8));
-        if (first >= 0) continue;   // internal nodes are computed by their last child
-        const unsigned b = nbegin[t], c = ncount[t];
-        double4 r;
-        if (c == 1) {
-            r = sbody[b];
-        } else {
-            double4 s = sbody[b];
-            double m = s.w;
-            double wx = __fma_rn(s.w, s.x, 0.0), wy = __fma_rn(s.w, s.y, 0.0), wz = __fma_rn(s.w, s.z, 0.0);
-            for (unsigned j = b + 1; j < b + c; ++j) {
-                s = sbody[j];
-                m = __dadd_rn(m, s.w);
-                wx = __fma_rn(s.w, s.x, wx);
-                wy = __fma_rn(s.w, s.y, wy);
-                wz = __fma_rn(s.w, s.z, wz);
-            }
-            r = make_double4(__ddiv_rn(wx, m), __ddiv_rn(wy, m), __ddiv_rn(wz, m), m);
-        }
-        mono[t] = r;
-        int p = nparent[t];
-        while (p >= 0) {
-            __threadfence();
-            const unsigned old = atomicAdd(&node_meta[p], 256u);
-            const int nch = __popc(old & 0xffu);
-            if ((int)(old >> 8) != nch - 1) break;   // siblings still pending
-            __threadfence();
-            const int f = nfirst[p];
-            double4 s = ldcg4(mono + f);
-            double m = s.w;
-            double wx = __fma_rn(s.w, s.x, 0.0), wy = __fma_rn(s.w, s.y, 0.0), wz = __fma_rn(s.w, s.z, 0.0);
-            for (int u = f + 1; u < f + nch; ++u) {
-                s = ldcg4(mono + u);
-                m = __dadd_rn(m, s.w);
-                wx = __fma_rn(s.w, s.x, wx);
-                wy = __fma_rn(s.w, s.y, wy);
-                wz = __fma_rn(s.w, s.z, wz);
-            }
-            mono[p] = make_double4(__ddiv_rn(wx, m), __ddiv_rn(wy, m), __ddiv_rn(wz, m), m);
-            p = nparent[p];
-        }
-    }
+    monopoles_and_records(M, blockIdx.x * blockDim.x + threadIdx.x, gridDim.x * blockDim.x, sbody, nbegin, ncount, nfirst,
+                          nparent, node_meta, mono, nlevel, winfo);
 }
 
 __global__ void unpack_mask_kernel(const unsigned *__restrict__ node_meta, const DevState *__restrict__ st,

@@ -208,7 +208,14 @@ __device__ void produce(PairSmem &ps, DevState *st, const unsigned *__restrict__
             ps.ctrl.desc_begin[k % kDesc] = P.tail;
         }
         warp_release(&ps.ctrl.started, k + 1, lane);
-        if (g == kNoGroup) break;
+        if (g == kNoGroup) {
+            // the last producer warp of the grid to run out of groups leaves the queue ready for the next walk
+            if (lane == 0 && atomicAdd(&st->walk_done, 1u) == gridDim.x * (unsigned)kPairs - 1u) {
+                st->walk_queue = 0u;
+                st->walk_done = 0u;
+            }
+            break;
+        }
 
         const unsigned gb = gstart[g], ge = gstart[g + 1];
         const double glx = gbox[6 * g + 0], gly = gbox[6 * g + 1], glz = gbox[6 * g + 2];

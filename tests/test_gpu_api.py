@@ -71,12 +71,12 @@ def test_phase_timing_and_launch_count():
     bh.bh_kdk_step(ctx.ctx, 1e-3)
     assert bh.bh_get_launches(ctx.ctx) - l0 == 2 * 19 + 17
     assert bh.bh_get_phase_ms(ctx.ctx)["kick_drift"] > 0.0
-    # one sort tile: a single launch instead of eight passes
+    # one sort tile (n <= 4096): the whole build is one launch of one block
     small = bh.Context(2000, 16)
     w2 = wl.make("c1", 2000)
     l0 = bh.bh_get_launches(small.ctx)
     small.build(dev(w2.pos), dev(w2.mass))
-    assert bh.bh_get_launches(small.ctx) - l0 == 2 + 1 + 1 + 4 + 1
+    assert bh.bh_get_launches(small.ctx) - l0 == 1
     small.close()
     ctx.close()
 
