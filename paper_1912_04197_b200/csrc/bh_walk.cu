@@ -49,14 +49,16 @@ constexpr int kTripUnroll = BH_TRIP_UNROLL;   // producer: trips of a pop unroll
 #endif
 
 
+constexpr int kMaxSplit = 4;                 // most consumer warps that share one producer's ring (see walk_kernel)
+
 struct PairCtrl {                            // all words are written by one role and read by the other
     unsigned tail_pub;                       // producer: ring entries below this are complete
-    unsigned head_pub;                       // consumer: ring entries below this are free again
     unsigned started;                        // producer: groups whose descriptor is valid
     unsigned finished;                       // producer: groups whose list is complete (desc_end valid)
-    unsigned consumed;                       // consumer: groups it is done with
+    unsigned head_pub[kMaxSplit];            // consumer s: ring entries below this are free again
+    unsigned consumed[kMaxSplit];            // consumer s: groups it is done with
     unsigned desc_g[kDesc], desc_begin[kDesc], desc_end[kDesc];
-    unsigned pad[3];
+    unsigned pad;
 };
 
 struct PairSmem {
@@ -98,6 +100,13 @@ __device__ __forceinline__ unsigned warp_acquire(const unsigned *p, unsigned lan
     if (lane == 0) v = ld_acquire(p);
     return __shfl_sync(0xffffffffu, v, 0);
 }
+// the smallest of the first k counters of the other role (lanes < k read one each)
+__device__ __forceinline__ unsigned warp_acquire_min(const unsigned *p, unsigned k, unsigned lane)
+{
+    unsigned v = 0xffffffffu;
+    if (lane < k) v = ld_acquire(p + lane);
+    return __reduce_min_sync(0xffffffffu, v);
+}
 // lane 0 publishes a counter after the whole warp has passed this point
 __device__ __forceinline__ void warp_release(unsigned *p, unsigned v, unsigned lane)
 {
@@ -110,8 +119,9 @@ struct Producer {
     PairSmem &ps;
     unsigned lane;
     unsigned tail;        // ring entries written (absolute)
-    unsigned head_seen;   // last value read from ctrl.head_pub
+    unsigned head_seen;   // smallest value last read from ctrl.head_pub[0 .. split)
     unsigned pub;         // last value stored to ctrl.tail_pub
+    unsigned split;       // consumer warps that read this ring
 
     __device__ __forceinline__ void publish(unsigned v)
     {
@@ -131,14 +141,14 @@ struct Producer {
         const unsigned want = n > (unsigned)kRing / 2 - 64u ? n : (unsigned)kRing / 2 - 64u;
         while (true) {
             __nanosleep(BH_SLEEP_FULL);
-            head_seen = warp_acquire(&ps.ctrl.head_pub, lane);
+            head_seen = warp_acquire_min(ps.ctrl.head_pub, split, lane);
             if (tail + want - head_seen <= (unsigned)kRing) break;
         }
     }
     __device__ __forceinline__ void reserve(unsigned n)
     {
         if (tail + n - head_seen <= (unsigned)kRing) return;
-        head_seen = warp_acquire(&ps.ctrl.head_pub, lane);
+        head_seen = warp_acquire_min(ps.ctrl.head_pub, split, lane);
         if (tail + n - head_seen <= (unsigned)kRing) return;
         reserve_slow(n);
     }
@@ -184,7 +194,7 @@ template <bool POT>
 __device__ void produce(PairSmem &ps, DevState *st, const unsigned *__restrict__ gstart,
                         const double4 *__restrict__ sbody, const double *__restrict__ gbox,
                         const uint4 *__restrict__ winfo, const double4 *__restrict__ mono, double theta2,
-                        unsigned *__restrict__ cnt_mono, unsigned *__restrict__ cnt_direct, uint2 *slab)
+                        unsigned *__restrict__ cnt_mono, unsigned *__restrict__ cnt_direct, uint2 *slab, unsigned split)
 {
     const unsigned lane = lane_id();
     const unsigned lt = (1u << lane) - 1u;
@@ -192,7 +202,7 @@ __device__ void produce(PairSmem &ps, DevState *st, const unsigned *__restrict__
     const int s2_base = (2 * st->e + 1023) << 20;   // high word of L^2; a level down is 2^-2: subtract 2 << 20 (|e| <= 301 is checked by cube_kernel, so the exponent field stays in range)
     unsigned long long tot_mono = 0, tot_direct = 0, tot_inter = 0, tot_tested = 0;
     unsigned tot_spills = 0;   // times the shared stack overflowed into the global slab (stats[4])
-    Producer P{ps, lane, 0u, 0u, 0u};
+    Producer P{ps, lane, 0u, 0u, 0u, split};
     uint2 *stack = ps.stack;
     unsigned k = 0;   // groups started by this pair
 
@@ -201,7 +211,7 @@ __device__ void produce(PairSmem &ps, DevState *st, const unsigned *__restrict__
         if (lane == 0) g = atomicAdd(&st->walk_queue, 1u);
         g = __shfl_sync(0xffffffffu, g, 0);
         if (g >= ngroups) g = kNoGroup;
-        while (k - warp_acquire(&ps.ctrl.consumed, lane) >= (unsigned)kDesc) __nanosleep(256);
+        while (k - warp_acquire_min(ps.ctrl.consumed, split, lane) >= (unsigned)kDesc) __nanosleep(256);
         P.tail = (P.tail + 7u) & ~7u;          // a group's sources start on a chunk boundary
         if (lane == 0) {
             ps.ctrl.desc_g[k % kDesc] = g;
@@ -210,7 +220,7 @@ __device__ void produce(PairSmem &ps, DevState *st, const unsigned *__restrict__
         warp_release(&ps.ctrl.started, k + 1, lane);
         if (g == kNoGroup) {
             // the last producer warp of the grid to run out of groups leaves the queue ready for the next walk
-            if (lane == 0 && atomicAdd(&st->walk_done, 1u) == gridDim.x * (unsigned)kPairs - 1u) {
+            if (lane == 0 && atomicAdd(&st->walk_done, 1u) == gridDim.x * ((unsigned)kPairs / split) - 1u) {
                 st->walk_queue = 0u;
                 st->walk_done = 0u;
             }
@@ -375,17 +385,38 @@ __device__ void produce(PairSmem &ps, DevState *st, const unsigned *__restrict__
 }
 
 // ------------------------------------------------------------------------------------------ consumer
-// one group: evaluate its sources as the producer publishes them, then write the accelerations
+// A consumer that holds none of the group's bodies (split walk, group of fewer bodies than consumers): it only
+// follows the producer so that the ring space it is counted for is released.
+__device__ __forceinline__ void drain_group(PairSmem &ps, unsigned k, unsigned sub)
+{
+    const unsigned lane = lane_id();
+    while (true) {
+        unsigned lim = 0;
+        bool fin = false;
+        if (lane == 0) {
+            const unsigned tp = ld_acquire(&ps.ctrl.tail_pub);      // tail_pub first, then finished (see consume_group)
+            fin = (int)(ld_acquire(&ps.ctrl.finished) - k) > 0;
+            lim = fin ? ps.ctrl.desc_end[k % kDesc] : tp;
+            if (fin || (int)(lim - ps.ctrl.desc_begin[k % kDesc]) > 0) st_release(&ps.ctrl.head_pub[sub], lim);
+        }
+        if (__shfl_sync(0xffffffffu, (int)fin, 0)) break;
+        __nanosleep(256);
+    }
+}
+
+// one group: evaluate its sources as the producer publishes them, then write the accelerations.
+// This consumer holds NS slots of eight bodies: slots sub, sub + split, ... of the group (split = 1: all of them).
 template <bool GUARD, int NS, int MODE>
 __device__ __forceinline__ void consume_group(PairSmem &ps, unsigned k, unsigned head, long long gb, long long ge,
                                               const double4 *__restrict__ sbody, const unsigned *__restrict__ perm,
-                                              double eps2, double G, double *__restrict__ acc, double *__restrict__ phi)
+                                              double eps2, double G, double *__restrict__ acc, double *__restrict__ phi,
+                                              unsigned sub, unsigned split)
 {
     const unsigned lane = lane_id(), quarter = lane >> 3, r = lane & 7u;
     Bodies<NS> B;
 #pragma unroll
     for (int s = 0; s < NS; ++s) {
-        const long long j = gb + r + 8 * s;
+        const long long j = gb + r + 8 * (sub + s * split);
         const double4 bd = sbody[j < ge ? j : gb];
         B.x[s] = bd.x; B.y[s] = bd.y; B.z[s] = bd.z;
         B.ax[s] = B.ay[s] = B.az[s] = B.ph[s] = 0.0;
@@ -424,10 +455,10 @@ __device__ __forceinline__ void consume_group(PairSmem &ps, unsigned k, unsigned
                 for (int s = 0; s < NS; ++s) interact_any<GUARD, MODE>(B.x[s], B.y[s], B.z[s], eps2, s1, B.ax[s], B.ay[s], B.az[s], B.ph[s]);
                 head += rest;
             }
-            warp_release(&ps.ctrl.head_pub, head, lane);
+            warp_release(&ps.ctrl.head_pub[sub], head, lane);
             break;
         }
-        warp_release(&ps.ctrl.head_pub, head, lane);
+        warp_release(&ps.ctrl.head_pub[sub], head, lane);
     }
     if constexpr (MODE != 0) {
         // pairs inside the group: quarter q takes the group's bodies gb + q, gb + q + 4, ...; a body skips itself
@@ -436,12 +467,12 @@ __device__ __forceinline__ void consume_group(PairSmem &ps, unsigned k, unsigned
 #pragma unroll
             for (int s = 0; s < NS; ++s) {
                 double4 src = sk;
-                if (k == gb + r + 8 * s) src.w = 0.0;
+                if (k == gb + r + 8 * (sub + s * split)) src.w = 0.0;
                 interact_any<true, MODE>(B.x[s], B.y[s], B.z[s], eps2, src, B.ax[s], B.ay[s], B.az[s], B.ph[s]);
             }
         }
     }
-    // add the four quarter-warp partial sums; lane 8 q + r then writes body r + 8 q
+    // add the four quarter-warp partial sums; lane 8 q + r then writes the body of slot q: r + 8 (sub + q split)
     double ox = 0.0, oy = 0.0, oz = 0.0, op = 0.0;
 #pragma unroll
     for (int s = 0; s < NS; ++s) {
@@ -460,8 +491,8 @@ __device__ __forceinline__ void consume_group(PairSmem &ps, unsigned k, unsigned
         tz += __shfl_xor_sync(0xffffffffu, tz, 16);
         if ((int)quarter == s) { ox = tx; oy = ty; oz = tz; }
     }
-    const long long j = gb + lane;
-    if (j < ge) {
+    const long long j = gb + r + 8 * (sub + quarter * split);
+    if ((int)quarter < NS && j < ge) {
         const unsigned i = perm[j];
         if constexpr (MODE == 1) {
             acc[i] = -G * ox;                       // phi, one value per body
@@ -477,7 +508,7 @@ __device__ __forceinline__ void consume_group(PairSmem &ps, unsigned k, unsigned
 template <bool GUARD, int MODE>
 __device__ void consume(PairSmem &ps, const unsigned *__restrict__ gstart, const double4 *__restrict__ sbody,
                         const unsigned *__restrict__ perm, double eps2, double G, double *__restrict__ acc,
-                        double *__restrict__ phi)
+                        double *__restrict__ phi, unsigned sub, unsigned split)
 {
     const unsigned lane = lane_id();
     for (unsigned k = 0;; ++k) {
@@ -487,12 +518,14 @@ __device__ void consume(PairSmem &ps, const unsigned *__restrict__ gstart, const
         const unsigned head = ps.ctrl.desc_begin[k % kDesc];
         const long long gb = gstart[g];
         const long long ge = gstart[g + 1];
-        const int slots = (int)((ge - gb + 7) >> 3);
-        if (slots >= 4) consume_group<GUARD, 4, MODE>(ps, k, head, gb, ge, sbody, perm, eps2, G, acc, phi);
-        else if (slots == 3) consume_group<GUARD, 3, MODE>(ps, k, head, gb, ge, sbody, perm, eps2, G, acc, phi);
-        else if (slots == 2) consume_group<GUARD, 2, MODE>(ps, k, head, gb, ge, sbody, perm, eps2, G, acc, phi);
-        else consume_group<GUARD, 1, MODE>(ps, k, head, gb, ge, sbody, perm, eps2, G, acc, phi);
-        warp_release(&ps.ctrl.consumed, k + 1, lane);
+        const int all = (int)((ge - gb + 7) >> 3);                                    // slots of eight bodies in the group
+        const int slots = all > (int)sub ? (all - (int)sub + (int)split - 1) / (int)split : 0;   // ... that are mine
+        if (slots >= 4) consume_group<GUARD, 4, MODE>(ps, k, head, gb, ge, sbody, perm, eps2, G, acc, phi, sub, split);
+        else if (slots == 3) consume_group<GUARD, 3, MODE>(ps, k, head, gb, ge, sbody, perm, eps2, G, acc, phi, sub, split);
+        else if (slots == 2) consume_group<GUARD, 2, MODE>(ps, k, head, gb, ge, sbody, perm, eps2, G, acc, phi, sub, split);
+        else if (slots == 1) consume_group<GUARD, 1, MODE>(ps, k, head, gb, ge, sbody, perm, eps2, G, acc, phi, sub, split);
+        else drain_group(ps, k, sub);
+        warp_release(&ps.ctrl.consumed[sub], k + 1, lane);
     }
 }
 
@@ -510,8 +543,17 @@ walk_kernel(DevState *st, const unsigned *__restrict__ gstart, const double4 *__
     const unsigned warp = threadIdx.x >> 5;
     const unsigned pair = (warp >> 3) * 4 + (warp & 3u);
     const bool producer = ((warp >> 2) & 1u) == 0;
-    PairSmem &ps = sm.pair[pair];
-    if (producer && lane_id() < sizeof(PairCtrl) / 4) reinterpret_cast<unsigned *>(&ps.ctrl)[lane_id()] = 0u;
+    // Few groups (fewer than half / a quarter of the grid's consumer warps: configs[0], configs[1], PAPER.md:199's
+    // N <= 10^4): `split` = 2 or 4 consumer warps share the ring of ONE producer and divide the group's BODIES
+    // among them (slots of eight: consumer s takes slots s, s + split, ...), so a group's evaluation takes a
+    // half / a quarter of the time and all fp64 pipes stay busy.  Every body still meets every source in the
+    // same order: the results are bit-identical to the unsplit walk.  Pairs p with p % split == 0 lead; the
+    // other producers have nothing to do.
+    const unsigned ngroups = st->n_groups;
+    const unsigned split = ngroups <= gridDim.x * (unsigned)kPairs / 4u ? 4u : (ngroups <= gridDim.x * (unsigned)kPairs / 2u ? 2u : 1u);
+    const unsigned sub = pair % split;
+    PairSmem &ps = sm.pair[pair - sub];
+    if (producer && sub == 0 && lane_id() < sizeof(PairCtrl) / 4) reinterpret_cast<unsigned *>(&ps.ctrl)[lane_id()] = 0u;
     __syncthreads();
 #if BH_REG_PROD > 0
     // the block is launched with 128 registers per thread; the producer warpgroups hand registers to
@@ -519,11 +561,13 @@ walk_kernel(DevState *st, const unsigned *__restrict__ gstart, const double4 *__
     if (producer) asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(BH_REG_PROD));
     else asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(BH_REG_CONS));
 #endif
-    if (producer)
-        produce<MODE != 0>(ps, st, gstart, sbody, gbox, winfo, mono, theta2, cnt_mono, cnt_direct,
-                reinterpret_cast<uint2 *>(walk_stack) + (size_t)(blockIdx.x * kPairs + pair) * kStackSlab);
-    else
-        consume<GUARD, MODE>(ps, gstart, sbody, perm, eps2, G, acc, phi);
+    if (producer) {
+        if (sub == 0)
+            produce<MODE != 0>(ps, st, gstart, sbody, gbox, winfo, mono, theta2, cnt_mono, cnt_direct,
+                    reinterpret_cast<uint2 *>(walk_stack) + (size_t)(blockIdx.x * kPairs + pair) * kStackSlab, split);
+    } else {
+        consume<GUARD, MODE>(ps, gstart, sbody, perm, eps2, G, acc, phi, sub, split);
+    }
 }
 
 // ------------------------------------------------------------------------------------------ a8
