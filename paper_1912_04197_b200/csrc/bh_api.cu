@@ -143,7 +143,8 @@ bh_status do_build(bh_ctx *c, const double *pos, const double *mass, int64_t n, 
     int sort_launches = 0;
     // cleared per build, sized by n (not by max_n): histograms + tickets + look-back words of this n's tiles,
     // and the child masks / arrival counters of the nodes n bodies can make
-    const int64_t tiles = (n + kSortTile - 1) / kSortTile;
+    const int64_t tile_keys = (int64_t)kSortThreads * sort_tile_items(n);
+    const int64_t tiles = (n + tile_keys - 1) / tile_keys;
     cudaMemsetAsync(w.zero_begin, 0, (size_t)((char *)w.lookback - (char *)w.zero_begin) + (size_t)kSortPasses * tiles * kRadix * sizeof(unsigned), s);
     cudaMemsetAsync(w.node_meta, 0, (size_t)node_capacity(n, c->leaf_cap) * sizeof(unsigned), s);
     {
@@ -294,7 +295,11 @@ Workspace carve(char *base, int64_t max_n, int leaf_cap)
     w.group_w = kMaxGroup;
     w.group_cell = BH_GROUP_CELL_DEFAULT;
     w.node_cap = node_capacity(n, leaf_cap);
-    w.sort_tiles = (n + kSortTile - 1) / kSortTile;
+    {   // most tiles any n <= max_n can have (2048-key tiles below kSortSmallTileBelow keys, 4096-key tiles from there)
+        const int64_t small_n = n < kSortSmallTileBelow ? n : kSortSmallTileBelow - 1;
+        const int64_t t8 = (small_n + kSortThreads * 8 - 1) / (kSortThreads * 8), t16 = (n + kSortTile - 1) / kSortTile;
+        w.sort_tiles = t8 > t16 ? t8 : t16;
+    }
     w.tree_tiles = (n + kTreeTile - 1) / kTreeTile;
     w.walk_warps = w.sms * WalkConfig::kPairsPerBlock;
     const int64_t groups = n;   // capacity: a group holds at least one body

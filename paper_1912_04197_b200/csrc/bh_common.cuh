@@ -22,7 +22,11 @@ constexpr int kSortThreads = 256;
 #define BH_SORT_ITEMS 16
 #endif
 constexpr int kSortItems = BH_SORT_ITEMS;   // keys per thread
-constexpr int kSortTile = kSortThreads * kSortItems;   // 4096 keys per tile
+constexpr int kSortTile = kSortThreads * kSortItems;   // 4096 keys per tile (one tile: the one-block build, bh_small.cu)
+#ifndef BH_SORT_SMALL_BELOW
+#define BH_SORT_SMALL_BELOW (1 << 19)
+#endif
+constexpr int64_t kSortSmallTileBelow = BH_SORT_SMALL_BELOW;   // the streaming passes use 2048-key tiles below this many keys
 constexpr int kTreeTile = 1024;           // bodies per block in the tree kernels
 constexpr int kDiagBlocks = 592;          // diagnostics: a FIXED number of partial sums, whatever the device, so that the reduction order is fixed
 constexpr int kStackSlab = 22 * 256;      // walk: spill entries (8 bytes each) per producer warp: <= 32 x 7 ranges per level; overflow sets kStatStack
@@ -121,11 +125,13 @@ Workspace carve(char *base, int64_t max_n, int leaf_cap);
 void launch_cube(const Workspace &w, const double *pos, int64_t n, cudaStream_t s);
 void launch_keys(const Workspace &w, const double *pos, int64_t n, cudaStream_t s);
 int launch_sort(const Workspace &w, int64_t n, cudaStream_t s);   // result in key[0]/idx[0]; returns the launches
+int sort_tile_items(int64_t n);                                    // keys per thread of the streaming passes for n keys
 // steps a1-a6 in one kernel of one block, n <= kSortTile (bh_small.cu); needs no prior clearing
 void launch_build_small(const Workspace &w, const double *pos, const double *mass, int64_t n, cudaStream_t s);
 void launch_gather(const Workspace &w, const double *pos, const double *mass, int64_t n, cudaStream_t s);
 // (x,y,z,m) in the caller's body order with the identity permutation: input of a direct sum without a tree
 void launch_pack(const Workspace &w, const double *pos, const double *mass, int64_t n, cudaStream_t s);
+void launch_iperm(const Workspace &w, int64_t n, cudaStream_t s);   // w.iperm from the permutation of the last build
 void launch_tree(const Workspace &w, int64_t n, int leaf_cap, cudaStream_t s);
 void launch_monopoles(const Workspace &w, int64_t n, cudaStream_t s);
 // mode 0: acc [n][3] accelerations; 1: acc [n] potential; 2: acc [n][3] and phi [n] from one walk (NEXT-1)

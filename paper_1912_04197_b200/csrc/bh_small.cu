@@ -122,7 +122,7 @@ __global__ void __launch_bounds__(kSmallThreads) build_small_kernel(Workspace w,
             v[i] = (unsigned)idx;
         }
         block_radix_sort<ITEMS, kSmallThreads>(k, v, skey, whist, stoff, stmp);
-        // ---- a4: sorted keys, permutation, sorted bodies, inverse permutation
+        // ---- a4: sorted keys, permutation, sorted bodies
 #pragma unroll
         for (int i = 0; i < ITEMS; ++i) {
             const int j = warp * (32 * ITEMS) + i * 32 + lane;
@@ -131,7 +131,6 @@ __global__ void __launch_bounds__(kSmallThreads) build_small_kernel(Workspace w,
                 w.key[0][j] = k[i];
                 w.idx[0][j] = b;
                 w.sbody[j] = make_double4(__ldg(pos + 3 * b), __ldg(pos + 3 * b + 1), __ldg(pos + 3 * b + 2), __ldg(mass + b));
-                w.iperm[b] = (unsigned)j;
             }
         }
         __syncthreads();
@@ -141,7 +140,7 @@ __global__ void __launch_bounds__(kSmallThreads) build_small_kernel(Workspace w,
     const int ntiles = (n + kTreeTile - 1) / kTreeTile;
     for (int t = 0; t < ntiles; ++t) {
         tree_levels_tile(w.key[0], n, C, w.group_cell, w.group_w, w.dlev, w.tile_lvl, ntiles, t,
-                         reinterpret_cast<signed char *>(smem), slv);
+                         reinterpret_cast<unsigned *>(smem), slv);
         __syncthreads();
     }
     tree_scan_block(w.tile_lvl, ntiles, st, w.node_cap, w.gstart, (unsigned)n, slv);
@@ -151,7 +150,7 @@ __global__ void __launch_bounds__(kSmallThreads) build_small_kernel(Workspace w,
     for (int t = tid; t < M; t += kSmallThreads) w.node_meta[t] = 0u;     // child masks and arrival counters
     __syncthreads();
     for (int t = 0; t < ntiles; ++t) {
-        tree_emit_tile(w.key[0], n, w.dlev, w.tile_lvl, ntiles, t, st, w.node_cap, w.nlevel, w.nbegin, w.ncount, w.nfirst,
+        tree_emit_tile(w.key[0], n, w.dlev, w.tile_lvl, ntiles, t, st, w.node_cap, w.nlevel, w.nbegin, w.nfirst,
                        w.nparent, w.node_meta, w.gstart, reinterpret_cast<unsigned(*)[kLevels + 1]>(smem), slv);
         __syncthreads();
     }
@@ -163,7 +162,8 @@ __global__ void __launch_bounds__(kSmallThreads) build_small_kernel(Workspace w,
     for (int l = depth; l >= 0; --l) {
         for (int t = (int)slv[l] + (int)tid; t < (int)slv[l + 1]; t += kSmallThreads) {
             const int first = w.nfirst[t];
-            const unsigned b = w.nbegin[t], c = w.ncount[t];
+            const unsigned b = w.nbegin[t], c = node_count(t, M, (unsigned)n, w.nbegin, w.nparent);
+            w.ncount[t] = c;
             const unsigned kids = (unsigned)__popc(__ldcg(w.node_meta + t) & 0xffu);   // masks were set by atomics (L2)
             w.winfo[t] = make_uint4(b, c, (unsigned)first, (unsigned)l | (kids << 8));
             w.mono[t] = monopole_of(t, w.sbody, w.mono, b, c, first, kids);
@@ -177,7 +177,7 @@ static void launch_small_t(const Workspace &w, const double *pos, const double *
 {
     // sort: keys + per-warp histograms + digit offsets; tree: two window arrays / the emission's chunk counts
     size_t sort_bytes = (size_t)kSmallThreads * ITEMS * 8 + (size_t)(kSmallThreads / 32 + 1) * kRadix * 4;
-    size_t tree_bytes = (size_t)2 * kTreeTile + w.leaf_cap + w.group_cell;
+    size_t tree_bytes = (size_t)tree_levels_smem_words(w.leaf_cap, w.group_cell) * sizeof(unsigned);
     size_t emit_bytes = (size_t)(kTreeTile / 32) * (kLevels + 1) * 4;
     size_t bytes = sort_bytes > tree_bytes ? sort_bytes : tree_bytes;
     if (emit_bytes > bytes) bytes = emit_bytes;

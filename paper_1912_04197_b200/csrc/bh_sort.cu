@@ -23,16 +23,17 @@ __device__ __forceinline__ void st_relaxed(unsigned *p, unsigned v)
     asm volatile("st.relaxed.gpu.global.u32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
 }
 
-#ifndef BH_SORT_MINBLOCKS
-#define BH_SORT_MINBLOCKS 4   // 64 registers (80 bytes spilled): four blocks per SM instead of two; sort at 4M bodies 0.60 -> 0.50 ms, 1M unchanged
-#endif
-template <bool FIRST>
-__global__ void __launch_bounds__(kSortThreads, BH_SORT_MINBLOCKS)
+// ITEMS keys per thread: 16 (tiles of 4096 keys, four blocks per SM at 64 registers) from 512k keys up; 8 (tiles of
+// 2048 keys) below, where 4096-key tiles are too few to fill the machine and the length of one tile's dependent
+// chain (load, rank, look-back, two scatters), not bandwidth, sets a pass's time.  Measured (eight passes):
+// 131072 keys 0.117 -> 0.085 ms with 2048-key tiles; 1M keys 0.171 ms with 4096-key tiles against 0.189 ms.
+template <bool FIRST, int ITEMS>
+__global__ void __launch_bounds__(kSortThreads, ITEMS == 16 ? 4 : 6)
 sort_pass_kernel(const unsigned long long *__restrict__ kin, const unsigned *__restrict__ vin,
                  unsigned long long *__restrict__ kout, unsigned *__restrict__ vout, long long n, int shift,
                  const unsigned *__restrict__ hist, unsigned *lookback, unsigned *ticket)
 {
-    __shared__ unsigned long long skey[kSortTile];          // 32 KB, reused for the values
+    __shared__ unsigned long long skey[(kSortThreads * ITEMS)];          // 32 KB, reused for the values
     __shared__ unsigned whist[kSortThreads / 32][kRadix];   // per-warp digit counts -> offsets
     __shared__ unsigned sbase[kRadix];                      // global position of a digit's run - its tile offset
     __shared__ unsigned stoff[kRadix];                      // tile-local start of a digit's run
@@ -45,14 +46,14 @@ sort_pass_kernel(const unsigned long long *__restrict__ kin, const unsigned *__r
     for (int w = 0; w < kSortThreads / 32; ++w) whist[w][tid] = 0u;
     __syncthreads();
     const unsigned tile = stile;
-    const long long base = (long long)tile * kSortTile;
+    const long long base = (long long)tile * (kSortThreads * ITEMS);
 
-    unsigned long long k[kSortItems];
-    unsigned v[kSortItems];
-    unsigned pos[kSortItems];
+    unsigned long long k[ITEMS];
+    unsigned v[ITEMS];
+    unsigned pos[ITEMS];
 #pragma unroll
-    for (int i = 0; i < kSortItems; ++i) {
-        long long idx = base + warp * (32 * kSortItems) + i * 32 + lane;
+    for (int i = 0; i < ITEMS; ++i) {
+        long long idx = base + warp * (32 * ITEMS) + i * 32 + lane;
         bool valid = idx < n;
         k[i] = valid ? kin[idx] : ~0ull;
         v[i] = FIRST ? (unsigned)idx : (valid ? vin[idx] : 0u);
@@ -60,8 +61,8 @@ sort_pass_kernel(const unsigned long long *__restrict__ kin, const unsigned *__r
     // per-warp stable ranking, one item row at a time
     const unsigned lt = (1u << lane) - 1u;
 #pragma unroll
-    for (int i = 0; i < kSortItems; ++i) {
-        long long idx = base + warp * (32 * kSortItems) + i * 32 + lane;
+    for (int i = 0; i < ITEMS; ++i) {
+        long long idx = base + warp * (32 * ITEMS) + i * 32 + lane;
         bool valid = idx < n;
         unsigned d = (unsigned)(k[i] >> shift) & (kRadix - 1);
         unsigned peers = __match_any_sync(0xffffffffu, valid ? d : (kRadix + lane));
@@ -87,13 +88,29 @@ sort_pass_kernel(const unsigned long long *__restrict__ kin, const unsigned *__r
         st_relaxed(mine, kFlagPre | tot);
     } else {
         st_relaxed(mine, kFlagAgg | tot);
+        // kLook predecessors are read per round trip to the L2 (independent loads), not one: the tiles of a pass
+        // all publish their aggregates at about the same time, and the walk back to the nearest inclusive prefix
+        // would otherwise be a chain of O(sqrt(tiles)) dependent loads
+        constexpr int kLook = 8;
         long long t = (long long)tile - 1;
-        while (true) {
-            unsigned s = ld_relaxed(lookback + (size_t)t * kRadix + tid);
-            if ((s >> 30) == 0u) continue;   // not published yet
-            excl += s & kValMask;
-            if (s & kFlagPre) break;
-            --t;
+        bool done = false;
+        while (!done) {
+            unsigned s[kLook];
+#pragma unroll
+            for (int b = 0; b < kLook; ++b) {
+                const long long u = t - b;
+                s[b] = u >= 0 ? ld_relaxed(lookback + (size_t)u * kRadix + tid) : kFlagPre;   // before tile 0: nothing
+            }
+            int used = 0;
+#pragma unroll
+            for (int b = 0; b < kLook; ++b) {
+                if (done || used != b) continue;     // stop at the first word that is not published yet
+                if ((s[b] >> 30) == 0u) continue;
+                excl += s[b] & kValMask;
+                ++used;
+                if (s[b] & kFlagPre) done = true;
+            }
+            t -= used;
         }
         st_relaxed(mine, kFlagPre | (excl + tot));
     }
@@ -104,8 +121,8 @@ sort_pass_kernel(const unsigned long long *__restrict__ kin, const unsigned *__r
     __syncthreads();
     // tile-local sorted order in shared memory
 #pragma unroll
-    for (int i = 0; i < kSortItems; ++i) {
-        long long idx = base + warp * (32 * kSortItems) + i * 32 + lane;
+    for (int i = 0; i < ITEMS; ++i) {
+        long long idx = base + warp * (32 * ITEMS) + i * 32 + lane;
         if (idx < n) {
             unsigned d = (unsigned)(k[i] >> shift) & (kRadix - 1);
             pos[i] += stoff[d] + whist[warp][d];
@@ -114,10 +131,10 @@ sort_pass_kernel(const unsigned long long *__restrict__ kin, const unsigned *__r
     }
     __syncthreads();
     long long rem = n - base;
-    const unsigned nvalid = rem < kSortTile ? (unsigned)rem : (unsigned)kSortTile;
-    unsigned gpos[kSortItems];
+    const unsigned nvalid = rem < (kSortThreads * ITEMS) ? (unsigned)rem : (unsigned)(kSortThreads * ITEMS);
+    unsigned gpos[ITEMS];
 #pragma unroll
-    for (int j = 0; j < kSortItems; ++j) {
+    for (int j = 0; j < ITEMS; ++j) {
         unsigned i2 = tid + j * kSortThreads;
         if (i2 < nvalid) {
             unsigned long long kk = skey[i2];
@@ -128,32 +145,39 @@ sort_pass_kernel(const unsigned long long *__restrict__ kin, const unsigned *__r
     __syncthreads();
     unsigned *sval = reinterpret_cast<unsigned *>(skey);
 #pragma unroll
-    for (int i = 0; i < kSortItems; ++i) {
-        long long idx = base + warp * (32 * kSortItems) + i * 32 + lane;
+    for (int i = 0; i < ITEMS; ++i) {
+        long long idx = base + warp * (32 * ITEMS) + i * 32 + lane;
         if (idx < n) sval[pos[i]] = v[i];
     }
     __syncthreads();
 #pragma unroll
-    for (int j = 0; j < kSortItems; ++j) {
+    for (int j = 0; j < ITEMS; ++j) {
         unsigned i2 = tid + j * kSortThreads;
         if (i2 < nvalid) vout[gpos[j]] = sval[i2];
     }
 }
 
+// keys per tile of the streaming passes for n keys
+int sort_tile_items(int64_t n) { return n < kSortSmallTileBelow ? 8 : 16; }
+
 int launch_sort(const Workspace &w, int64_t n, cudaStream_t s)
 {
-    const int tiles = (int)((n + kSortTile - 1) / kSortTile);   // one tile: the whole build is one block (bh_small.cu)
+    const int items = sort_tile_items(n);
+    const int tiles = (int)((n + kSortThreads * items - 1) / (kSortThreads * items));
     for (int p = 0; p < kSortPasses; ++p) {
         const int a = p & 1, b = a ^ 1;
         unsigned *lb = w.lookback + (size_t)p * tiles * kRadix;   // [pass][tiles of this n][256]: cleared per build
-        if (p == 0)
-            sort_pass_kernel<true><<<tiles, kSortThreads, 0, s>>>(w.key[a], w.idx[a], w.key[b], w.idx[b], n,
-                                                                 p * kRadixBits, w.hist + p * kRadix, lb,
-                                                                 w.sort_ticket + p);
-        else
-            sort_pass_kernel<false><<<tiles, kSortThreads, 0, s>>>(w.key[a], w.idx[a], w.key[b], w.idx[b], n,
-                                                                  p * kRadixBits, w.hist + p * kRadix, lb,
-                                                                  w.sort_ticket + p);
+#define BH_SORT_PASS(FIRST, ITEMS)                                                                                     \
+    sort_pass_kernel<FIRST, ITEMS><<<tiles, kSortThreads, 0, s>>>(w.key[a], w.idx[a], w.key[b], w.idx[b], n,           \
+                                                                  p * kRadixBits, w.hist + p * kRadix, lb, w.sort_ticket + p)
+        if (items == 8) {
+            if (p == 0) BH_SORT_PASS(true, 8);
+            else BH_SORT_PASS(false, 8);
+        } else {
+            if (p == 0) BH_SORT_PASS(true, 16);
+            else BH_SORT_PASS(false, 16);
+        }
+#undef BH_SORT_PASS
     }
     return kSortPasses;
 }

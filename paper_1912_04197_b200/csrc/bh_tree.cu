@@ -27,7 +27,7 @@ namespace bh {
 __global__ void __launch_bounds__(256) gather_kernel(const double *__restrict__ pos,
                                                      const double *__restrict__ mass,
                                                      const unsigned *__restrict__ perm, long long n,
-                                                     double4 *__restrict__ sbody, unsigned *__restrict__ iperm)
+                                                     double4 *__restrict__ sbody)
 {
     const long long j = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (j >= n) return;
@@ -38,18 +38,25 @@ __global__ void __launch_bounds__(256) gather_kernel(const double *__restrict__ 
     b.z = __ldg(pos + 3ll * i + 2);
     b.w = __ldg(mass + i);
     sbody[j] = b;
-    iperm[i] = (unsigned)j;
+}
+
+// inverse permutation (body index -> sorted position), made only when a call needs it (bh_direct_targets): a
+// scattered 4-byte store per body is not worth paying in every build
+__global__ void __launch_bounds__(256) iperm_kernel(const unsigned *__restrict__ perm, long long n,
+                                                    unsigned *__restrict__ iperm)
+{
+    const long long j = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (j < n) iperm[perm[j]] = (unsigned)j;
 }
 
 __global__ void __launch_bounds__(256) pack_kernel(const double *__restrict__ pos, const double *__restrict__ mass,
                                                    long long n, double4 *__restrict__ sbody,
-                                                   unsigned *__restrict__ perm, unsigned *__restrict__ iperm)
+                                                   unsigned *__restrict__ perm)
 {
     const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n) return;
     sbody[i] = make_double4(pos[3 * i], pos[3 * i + 1], pos[3 * i + 2], mass[i]);
     perm[i] = (unsigned)i;
-    iperm[i] = (unsigned)i;
 }
 
 __global__ void __launch_bounds__(256) group_box_kernel(const DevState *__restrict__ st,
@@ -67,7 +74,7 @@ __global__ void __launch_bounds__(256) tree_levels_kernel(const unsigned long lo
                                                           long long n, int C, int Gc, int W, uchar4 *__restrict__ dlev,
                                                           unsigned *__restrict__ tile_lvl, int ntiles)
 {
-    extern __shared__ signed char sw[];   // [kTreeTile + C] leaf windows, then [kTreeTile + Gc] group windows
+    extern __shared__ unsigned sw[];      // leaf windows, group windows (two copies each), cell starts
     __shared__ unsigned shist[kLevels + 1];
     tree_levels_tile(skey, n, C, Gc, W, dlev, tile_lvl, ntiles, blockIdx.x, sw, shist);
 }
@@ -87,21 +94,21 @@ __global__ void __launch_bounds__(256) tree_emit_kernel(const unsigned long long
                                                         const unsigned *__restrict__ tile_lvl, int ntiles,
                                                         const DevState *__restrict__ st, long long node_cap,
                                                         unsigned char *__restrict__ nlevel,
-                                                        unsigned *__restrict__ nbegin, unsigned *__restrict__ ncount,
+                                                        unsigned *__restrict__ nbegin,
                                                         int *__restrict__ nfirst, int *__restrict__ nparent,
                                                         unsigned *node_meta, unsigned *__restrict__ gstart)
 {
     __shared__ unsigned scnt[kTreeTile / 32][kLevels + 1];  // per chunk, per level (+ group starts): counts -> bases
     __shared__ unsigned sstart[kLevels + 1];
-    tree_emit_tile(skey, n, dlev, tile_lvl, ntiles, blockIdx.x, st, node_cap, nlevel, nbegin, ncount, nfirst, nparent,
+    tree_emit_tile(skey, n, dlev, tile_lvl, ntiles, blockIdx.x, st, node_cap, nlevel, nbegin, nfirst, nparent,
                    node_meta, gstart, scnt, sstart);
 }
 
 // ------------------------------------------------------------------------------------------ a6
-__global__ void __launch_bounds__(256) monopole_kernel(const DevState *__restrict__ st,
+__global__ void __launch_bounds__(256) monopole_kernel(const DevState *__restrict__ st, unsigned n,
                                                        const double4 *__restrict__ sbody,
                                                        const unsigned *__restrict__ nbegin,
-                                                       const unsigned *__restrict__ ncount,
+                                                       unsigned *__restrict__ ncount,
                                                        const int *__restrict__ nfirst,
                                                        const int *__restrict__ nparent, unsigned *node_meta,
                                                        double4 *mono, long long node_cap,
@@ -110,7 +117,7 @@ __global__ void __launch_bounds__(256) monopole_kernel(const DevState *__restric
 {
     const int M = st->n_nodes;
     if ((long long)M > node_cap) return;
-    monopoles_and_records(M, blockIdx.x * blockDim.x + threadIdx.x, gridDim.x * blockDim.x, sbody, nbegin, ncount, nfirst,
+    monopoles_and_records(M, n, blockIdx.x * blockDim.x + threadIdx.x, gridDim.x * blockDim.x, sbody, nbegin, ncount, nfirst,
                           nparent, node_meta, mono, nlevel, winfo);
 }
 
@@ -127,22 +134,27 @@ __global__ void unpack_mask_kernel(const unsigned *__restrict__ node_meta, const
 void launch_gather(const Workspace &w, const double *pos, const double *mass, int64_t n, cudaStream_t s)
 {
     int blocks = (int)((n + 255) / 256);
-    gather_kernel<<<blocks, 256, 0, s>>>(pos, mass, w.idx[0], n, w.sbody, w.iperm);
+    gather_kernel<<<blocks, 256, 0, s>>>(pos, mass, w.idx[0], n, w.sbody);
+}
+
+void launch_iperm(const Workspace &w, int64_t n, cudaStream_t s)
+{
+    iperm_kernel<<<(int)((n + 255) / 256), 256, 0, s>>>(w.idx[0], n, w.iperm);
 }
 
 void launch_pack(const Workspace &w, const double *pos, const double *mass, int64_t n, cudaStream_t s)
 {
-    pack_kernel<<<(int)((n + 255) / 256), 256, 0, s>>>(pos, mass, n, w.sbody, w.idx[0], w.iperm);
+    pack_kernel<<<(int)((n + 255) / 256), 256, 0, s>>>(pos, mass, n, w.sbody, w.idx[0]);
 }
 
 void launch_tree(const Workspace &w, int64_t n, int leaf_cap, cudaStream_t s)
 {
     const int ntiles = (int)((n + kTreeTile - 1) / kTreeTile);
-    size_t smem = (size_t)(2 * kTreeTile + leaf_cap + w.group_cell);
+    size_t smem = (size_t)tree_levels_smem_words(leaf_cap, w.group_cell) * sizeof(unsigned);
     tree_levels_kernel<<<ntiles, 256, smem, s>>>(w.key[0], n, leaf_cap, w.group_cell, w.group_w, w.dlev, w.tile_lvl, ntiles);
     tree_scan_kernel<<<1, (kLevels + 1) * 32, 0, s>>>(w.tile_lvl, ntiles, w.st, w.node_cap, w.gstart, (unsigned)n);
     tree_emit_kernel<<<ntiles, 256, 0, s>>>(w.key[0], n, w.dlev, w.tile_lvl, ntiles, w.st, w.node_cap, w.nlevel,
-                                            w.nbegin, w.ncount, w.nfirst, w.nparent, w.node_meta, w.gstart);
+                                            w.nbegin, w.nfirst, w.nparent, w.node_meta, w.gstart);
     group_box_kernel<<<w.sms * 4, 256, 0, s>>>(w.st, w.gstart, w.sbody, w.gbox);
 }
 
@@ -150,7 +162,7 @@ void launch_monopoles(const Workspace &w, int64_t n, cudaStream_t s)
 {
     const int64_t want = (node_capacity(n, w.leaf_cap) + 255) / 256;
     int blocks = (int)(want < w.sms * 16 ? want : w.sms * 16);
-    monopole_kernel<<<blocks, 256, 0, s>>>(w.st, w.sbody, w.nbegin, w.ncount, w.nfirst, w.nparent, w.node_meta,
+    monopole_kernel<<<blocks, 256, 0, s>>>(w.st, (unsigned)n, w.sbody, w.nbegin, w.ncount, w.nfirst, w.nparent, w.node_meta,
                                            w.mono, w.node_cap, w.nlevel, w.winfo);
 }
 

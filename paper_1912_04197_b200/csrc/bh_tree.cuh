@@ -8,56 +8,86 @@
 
 namespace bh {
 
+// Order-preserving map of a finite double onto an unsigned 64-bit integer (and back): min / max of doubles become
+// integer min / max, which the warp computes with two REDUX instructions per quantity (high words, then the low
+// words of the lanes that tie on the high word) instead of five rounds of 64-bit shuffles and fp64 min / max.
+__device__ __forceinline__ unsigned long long ordered_bits(double x)
+{
+    const unsigned long long u = (unsigned long long)__double_as_longlong(x);
+    return (u >> 63) ? ~u : (u | 0x8000000000000000ull);
+}
+__device__ __forceinline__ double from_ordered_bits(unsigned long long k)
+{
+    const unsigned long long u = (k >> 63) ? (k & 0x7fffffffffffffffull) : ~k;
+    return __longlong_as_double((long long)u);
+}
+__device__ __forceinline__ unsigned long long warp_min_u64(unsigned long long k)
+{
+    const unsigned hi = (unsigned)(k >> 32);
+    const unsigned mh = __reduce_min_sync(0xffffffffu, hi);
+    const unsigned ml = __reduce_min_sync(0xffffffffu, hi == mh ? (unsigned)k : 0xffffffffu);
+    return ((unsigned long long)mh << 32) | ml;
+}
+__device__ __forceinline__ unsigned long long warp_max_u64(unsigned long long k)
+{
+    const unsigned hi = (unsigned)(k >> 32);
+    const unsigned mh = __reduce_max_sync(0xffffffffu, hi);
+    const unsigned ml = __reduce_max_sync(0xffffffffu, hi == mh ? (unsigned)k : 0u);
+    return ((unsigned long long)mh << 32) | ml;
+}
+
 // exact bounding box of every walk group: warp `wid` of `nwarps` takes groups wid, wid + nwarps, ...
 __device__ __forceinline__ void group_boxes(unsigned ng, unsigned wid, unsigned nwarps, const unsigned *gstart,
                                             const double4 *sbody, double *gbox)
 {
     const unsigned lane = lane_id();
-    const double inf = __longlong_as_double(0x7ff0000000000000ll);
     for (unsigned g = wid; g < ng; g += nwarps) {
         const unsigned b = gstart[g], e = gstart[g + 1];
-        double lx = inf, ly = inf, lz = inf, hx = -inf, hy = -inf, hz = -inf;
-        for (unsigned j = b + lane; j < e; j += 32) {
-            const double4 p = sbody[j];
+        // every lane starts from the group's first body, so lanes beyond a short group are neutral
+        double4 p = sbody[b + lane < e ? b + lane : b];
+        double lx = p.x, ly = p.y, lz = p.z, hx = p.x, hy = p.y, hz = p.z;
+        for (unsigned j = b + lane + 32; j < e; j += 32) {      // W <= 32: at most one body per lane; kept general
+            p = sbody[j];
             lx = fmin(lx, p.x); ly = fmin(ly, p.y); lz = fmin(lz, p.z);
             hx = fmax(hx, p.x); hy = fmax(hy, p.y); hz = fmax(hz, p.z);
         }
-#pragma unroll
-        for (int o = 16; o > 0; o >>= 1) {
-            lx = fmin(lx, __shfl_xor_sync(0xffffffffu, lx, o));
-            ly = fmin(ly, __shfl_xor_sync(0xffffffffu, ly, o));
-            lz = fmin(lz, __shfl_xor_sync(0xffffffffu, lz, o));
-            hx = fmax(hx, __shfl_xor_sync(0xffffffffu, hx, o));
-            hy = fmax(hy, __shfl_xor_sync(0xffffffffu, hy, o));
-            hz = fmax(hz, __shfl_xor_sync(0xffffffffu, hz, o));
-        }
+        const unsigned long long rlx = warp_min_u64(ordered_bits(lx)), rly = warp_min_u64(ordered_bits(ly)),
+                                 rlz = warp_min_u64(ordered_bits(lz)), rhx = warp_max_u64(ordered_bits(hx)),
+                                 rhy = warp_max_u64(ordered_bits(hy)), rhz = warp_max_u64(ordered_bits(hz));
         if (lane == 0) {
             double *q = gbox + 6ull * g;
-            q[0] = lx; q[1] = ly; q[2] = lz; q[3] = hx; q[4] = hy; q[5] = hz;
+            q[0] = from_ordered_bits(rlx); q[1] = from_ordered_bits(rly); q[2] = from_ordered_bits(rlz);
+            q[3] = from_ordered_bits(rhx); q[4] = from_ordered_bits(rhy); q[5] = from_ordered_bits(rhz);
         }
     }
 }
 
-// sliding maximum over windows of k consecutive entries of a[0..len): after the call a[i] holds
-// max(a[i .. i+2^p-1]) with p = floor(log2 k); the caller combines a[i] and a[i + k - 2^p].
-__device__ __forceinline__ int window_doubling(signed char *a, int len, int k)
+// Sliding maximum over windows of k consecutive entries of a signed-byte array of nw 32-bit words (entries past
+// the data are -1, the neutral value), four entries per operation: after r rounds x[i] = max(x[i .. i + 2^r - 1]).
+// Runs p = floor(log2 k) rounds, ping-ponging between a and b; *out is the array that holds the result, and the
+// caller combines out[i] and out[i + k - 2^p].  Returns 2^p.
+__device__ __forceinline__ int window_doubling(unsigned *a, unsigned *b, int nw, int k, const signed char **out)
 {
     int p = 0;
     while ((2 << p) <= k) ++p;
     for (int r = 0; r < p; ++r) {
-        const int h = 1 << r;
-        signed char v[12];   // len <= kTreeTile + kMaxGroupCell, >= 256 threads
-        int c = 0;
-        for (int i = threadIdx.x; i < len; i += blockDim.x, ++c) {
-            signed char x = a[i];
-            if (i + h < len) x = max(x, a[i + h]);
-            v[c] = x;
+        const int h = 1 << r;                 // entries (bytes) to look ahead
+        for (int i = threadIdx.x; i < nw; i += blockDim.x) {
+            const unsigned x = a[i];
+            unsigned y;
+            if (h >= 4) {
+                const int j = i + (h >> 2);
+                y = j < nw ? a[j] : 0xffffffffu;
+            } else {
+                const unsigned nxt = i + 1 < nw ? a[i + 1] : 0xffffffffu;
+                y = __funnelshift_r(x, nxt, 8 * h);     // entries 4 i + h .. 4 i + h + 3 (little endian)
+            }
+            b[i] = __vmaxs4(x, y);
         }
         __syncthreads();
-        c = 0;
-        for (int i = threadIdx.x; i < len; i += blockDim.x, ++c) a[i] = v[c];
-        __syncthreads();
+        unsigned *t = a; a = b; b = t;
     }
+    *out = reinterpret_cast<const signed char *>(a);
     return 1 << p;
 }
 
@@ -106,46 +136,95 @@ __device__ __forceinline__ unsigned range_end(const unsigned long long *skey, un
     return hi;
 }
 
-// Tile `tile` of kTreeTile bodies, any block size >= 256: per body (d+1, leaf, group-start flag, group-cell level) and the
-// tile's counts of nodes per level and of group starts.  sw: kTreeTile + C + kTreeTile + Gc bytes of shared
+// words of shared memory tree_levels_tile needs for leaf capacity C and group-cell capacity Gc
+__host__ __device__ inline int tree_levels_smem_words(int C, int Gc)
+{
+    return 2 * ((kTreeTile + C + 3) / 4) + 2 * ((kTreeTile + Gc + 3) / 4) + kTreeTile + 64;
+}
+
+// Tile `tile` of kTreeTile bodies, any block size >= 256: per body (d+1, leaf, group-start flag, group-cell level)
+// and the tile's counts of nodes per level and of group starts.  sw: tree_levels_smem_words(C, Gc) words of shared
 // memory; shist: kLevels + 1 words.
 __device__ __forceinline__ void tree_levels_tile(const unsigned long long *skey, long long n, int C, int Gc, int W,
                                                  uchar4 *dlev, unsigned *tile_lvl, int ntiles, int tile,
-                                                 signed char *sw, unsigned *shist)
+                                                 unsigned *sw, unsigned *shist)
 {
-    signed char *swc = sw;
-    signed char *swg = sw + kTreeTile + C;
+    const int nwc = (kTreeTile + C + 3) / 4, nwg = (kTreeTile + Gc + 3) / 4;
+    unsigned *wc0 = sw, *wc1 = wc0 + nwc, *wg0 = wc1 + nwc, *wg1 = wg0 + nwg;
+    int *cellpos = reinterpret_cast<int *>(wg1 + nwg);          // [kTreeTile] then [32] chunk maxima, [1] tile's cell begin
+    int *chunkmax = cellpos + kTreeTile;
+    signed char *bc = reinterpret_cast<signed char *>(wc0), *bg = reinterpret_cast<signed char *>(wg0);
     const long long t0 = (long long)tile * kTreeTile;
+    const unsigned lane = lane_id(), warp = threadIdx.x >> 5;
+    const int nwarps = blockDim.x >> 5;
     if (threadIdx.x <= kLevels) shist[threadIdx.x] = 0u;
-    for (int k = threadIdx.x; k < kTreeTile + C; k += blockDim.x) {
+    for (int k = threadIdx.x; k < 4 * nwc; k += blockDim.x) {
         long long s = t0 - C + k;
         int wv = -1;
-        if (s >= 0 && s + C < n) wv = common_levels(skey[s], skey[s + C]);
-        swc[k] = (signed char)wv;
+        if (k < kTreeTile + C && s >= 0 && s + C < n) wv = common_levels(skey[s], skey[s + C]);
+        bc[k] = (signed char)wv;
     }
-    for (int k = threadIdx.x; k < kTreeTile + Gc; k += blockDim.x) {
+    for (int k = threadIdx.x; k < 4 * nwg; k += blockDim.x) {
         long long s = t0 - Gc + k;
         int wv = -1;
-        if (s >= 0 && s + Gc < n) wv = common_levels(skey[s], skey[s + Gc]);
-        swg[k] = (signed char)wv;
+        if (k < kTreeTile + Gc && s >= 0 && s + Gc < n) wv = common_levels(skey[s], skey[s + Gc]);
+        bg[k] = (signed char)wv;
     }
     __syncthreads();
-    const int pc = window_doubling(swc, kTreeTile + C, C + 1);
-    const int pg = window_doubling(swg, kTreeTile + Gc, Gc + 1);
-    for (int k = threadIdx.x; k < kTreeTile; k += blockDim.x) {
-        long long j = t0 + k;
-        if (j >= n) break;
-        // windows of C+1 (Gc+1) bodies that start at j-C .. j  (j-Gc .. j)
-        const int mw = max((int)swc[k], (int)swc[k + C + 1 - pc]);
-        const int mg = max((int)swg[k], (int)swg[k + Gc + 1 - pg]);
-        const int leaf = min(kMaxLevel, mw + 1);
-        const int glev = min(leaf, mg + 1);
-        const int d = (j == 0) ? -1 : common_levels(skey[j - 1], skey[j]);
-        const unsigned cb = range_begin(skey, (unsigned)j, glev);
-        const bool gs = (((unsigned)j - cb) % (unsigned)W) == 0u;
-        dlev[j] = make_uchar4((unsigned char)(d + 1), (unsigned char)leaf, gs ? 1 : 0, (unsigned char)glev);
-        for (int l = d + 1; l <= leaf; ++l) atomicAdd(&shist[l], 1u);
-        if (gs) atomicAdd(&shist[kLevels], 1u);
+    const signed char *swc, *swg;
+    const int pc = window_doubling(wc0, wc1, nwc, C + 1, &swc);
+    const int pg = window_doubling(wg0, wg1, nwg, Gc + 1, &swg);
+    // per body: levels, and where its group cell begins.  Body s is the first of its group cell iff it shares fewer
+    // than glev_s digits with its predecessor (d_s < glev_s); the cell of body j begins at the last such s <= j:
+    // an inclusive maximum scan of (first ? s : -1) over the tile.  Bodies before the tile's first cell start
+    // belong to the cell of the tile's first body, whose beginning one thread finds by search.
+    for (int c = warp; c < kTreeTile / 32; c += nwarps) {
+        const int k = c * 32 + (int)lane;
+        const long long j = t0 + k;
+        int d = -1, leaf = 0, glev = 0, mark = -1;
+        if (j < n) {
+            // windows of C+1 (Gc+1) bodies that start at j-C .. j  (j-Gc .. j)
+            const int mw = max((int)swc[k], (int)swc[k + C + 1 - pc]);
+            const int mg = max((int)swg[k], (int)swg[k + Gc + 1 - pg]);
+            leaf = min(kMaxLevel, mw + 1);
+            glev = min(leaf, mg + 1);
+            d = (j == 0) ? -1 : common_levels(skey[j - 1], skey[j]);
+            if (d < glev) mark = k;
+            if (k == 0) chunkmax[32] = (int)range_begin(skey, (unsigned)j, glev);
+        }
+        int run = mark;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const int t = __shfl_up_sync(0xffffffffu, run, o);
+            if (lane >= (unsigned)o) run = max(run, t);
+        }
+        cellpos[k] = run;
+        if (lane == 31) chunkmax[c] = run;
+        // level histogram: one ballot per level that occurs in this chunk
+        const int lo = __reduce_min_sync(0xffffffffu, j < n ? d + 1 : kLevels), hi = __reduce_max_sync(0xffffffffu, j < n ? leaf : -1);
+        for (int l = lo; l <= hi; ++l) {
+            const unsigned m = __ballot_sync(0xffffffffu, j < n && d + 1 <= l && l <= leaf);
+            if (lane == 0 && m) atomicAdd(&shist[l], (unsigned)__popc(m));
+        }
+        // keep (d + 1, leaf, glev) for the second pass in the output array itself
+        if (j < n) dlev[j] = make_uchar4((unsigned char)(d + 1), (unsigned char)leaf, 0, (unsigned char)glev);
+    }
+    __syncthreads();
+    for (int c = warp; c < kTreeTile / 32; c += nwarps) {
+        const int k = c * 32 + (int)lane;
+        const long long j = t0 + k;
+        int before = -1;                                   // last cell start in the chunks before this one
+        for (int q = (int)lane; q < c; q += 32) before = max(before, chunkmax[q]);
+        before = __reduce_max_sync(0xffffffffu, before);
+        bool gs = false;
+        if (j < n) {
+            const int at = max(cellpos[k], before);
+            const unsigned cb = at >= 0 ? (unsigned)(t0 + at) : (unsigned)chunkmax[32];
+            gs = (((unsigned)j - cb) % (unsigned)W) == 0u;
+            if (gs) reinterpret_cast<unsigned char *>(dlev + j)[2] = 1;
+        }
+        const unsigned m = __ballot_sync(0xffffffffu, gs);
+        if (lane == 0 && m) atomicAdd(&shist[kLevels], (unsigned)__popc(m));
     }
     __syncthreads();
     if (threadIdx.x <= kLevels) tile_lvl[(size_t)threadIdx.x * ntiles + tile] = shist[threadIdx.x];
@@ -199,7 +278,7 @@ __device__ __forceinline__ void tree_scan_block(unsigned *tile_lvl, int ntiles, 
 __device__ __forceinline__ void tree_emit_tile(const unsigned long long *skey, long long n, const uchar4 *dlev,
                                                const unsigned *tile_lvl, int ntiles, int tile, const DevState *st,
                                                long long node_cap, unsigned char *nlevel, unsigned *nbegin,
-                                               unsigned *ncount, int *nfirst, int *nparent, unsigned *node_meta,
+                                               int *nfirst, int *nparent, unsigned *node_meta,
                                                unsigned *gstart, unsigned (*scnt)[kLevels + 1], unsigned *sstart)
 {
     constexpr int kChunks = kTreeTile / 32;          // 32 chunks of 32 bodies
@@ -209,11 +288,14 @@ __device__ __forceinline__ void tree_emit_tile(const unsigned long long *skey, l
     if (threadIdx.x <= kLevels) sstart[threadIdx.x] = st->lvl_start[threadIdx.x];
     if ((long long)st->n_nodes > node_cap) return;   // flagged by the scan; stay in bounds (uniform over the block)
     // phase 1: per chunk level counts
+    // (only the levels that occur in a chunk of 32 sorted bodies are visited: a handful of the 22)
     for (int c = warp; c < kChunks; c += nwarps) {
         long long j = t0 + c * 32 + lane;
         uchar4 dl = j < n ? dlev[j] : make_uchar4(255, 0, 0, 0);
-#pragma unroll
-        for (int l = 0; l < kLevels; ++l) {
+        if (lane < (unsigned)kLevels) scnt[c][lane] = 0u;
+        __syncwarp();
+        const int lo = __reduce_min_sync(0xffffffffu, (int)dl.x), hi = __reduce_max_sync(0xffffffffu, j < n ? (int)dl.y : -1);
+        for (int l = lo; l <= hi; ++l) {
             unsigned b = __ballot_sync(0xffffffffu, (int)dl.x <= l && l <= (int)dl.y);
             if (lane == 0) scnt[c][l] = __popc(b);
         }
@@ -240,14 +322,19 @@ __device__ __forceinline__ void tree_emit_tile(const unsigned long long *skey, l
             const unsigned bg = __ballot_sync(0xffffffffu, dl.z != 0);
             if (dl.z) gstart[scnt[c][kLevels] + __popc(bg & le) - 1u] = (unsigned)j;
         }
-        // inclusive per-level counts at this body: prev (l-1), cur (l), next (l+1)
-        unsigned pprev = 0, pcur, pnext;
-        {
-            unsigned b = __ballot_sync(0xffffffffu, first <= 0 && 0 <= leaf);
-            pcur = scnt[c][0] + __popc(b & le);
+        // inclusive per-level counts at this body: prev (l-1), cur (l), next (l+1); levels lo .. hi of this chunk
+        const int lo = __reduce_min_sync(0xffffffffu, first), hi = __reduce_max_sync(0xffffffffu, j < n ? leaf : -1);
+        unsigned pprev = 0, pcur = 0, pnext;
+        if (lo <= hi) {
+            if (lo > 0) {
+                unsigned b = __ballot_sync(0xffffffffu, first <= lo - 1 && lo - 1 <= leaf);   // none starts there; bodies inside count
+                pprev = scnt[c][lo - 1] + __popc(b & le);
+            }
+            unsigned b = __ballot_sync(0xffffffffu, first <= lo && lo <= leaf);
+            pcur = scnt[c][lo] + __popc(b & le);
         }
 #pragma unroll 1
-        for (int l = 0; l < kLevels; ++l) {
+        for (int l = lo; l <= hi; ++l) {
             pnext = 0;
             if (l + 1 < kLevels) {
                 unsigned b = __ballot_sync(0xffffffffu, first <= l + 1 && l + 1 <= leaf);
@@ -258,8 +345,7 @@ __device__ __forceinline__ void tree_emit_tile(const unsigned long long *skey, l
                 const int par = l ? (int)(sstart[l - 1] + pprev - 1u) : -1;
                 const bool internal = l < leaf;
                 nlevel[id] = (unsigned char)l;
-                nbegin[id] = (unsigned)j;
-                ncount[id] = range_end(skey, (unsigned)n, (unsigned)j, l) - (unsigned)j;
+                nbegin[id] = (unsigned)j;                 // its count follows from its siblings (node_count, below)
                 nfirst[id] = internal ? (int)(sstart[l + 1] + pnext - 1u) : -1;
                 nparent[id] = par;
                 if (l) {   // record my octant in the parent's child mask
@@ -270,6 +356,21 @@ __device__ __forceinline__ void tree_emit_tile(const unsigned long long *skey, l
             pprev = pcur;
             pcur = pnext;
         }
+    }
+}
+
+// Bodies of node t.  The children of a node tile its range of sorted bodies, and siblings have consecutive ids:
+// a node ends where its next sibling begins, a last child ends where its parent ends, the root at n.  (Replaces a
+// galloping search over the keys per emitted node: a handful of dependent loads instead of 2 log2(count).)
+__device__ __forceinline__ unsigned node_count(int t, int M, unsigned n, const unsigned *nbegin, const int *nparent)
+{
+    const unsigned b = nbegin[t];
+    int u = t;
+    while (true) {
+        const int p = nparent[u];
+        if (p < 0) return n - b;
+        if (u + 1 < M && nparent[u + 1] == p) return nbegin[u + 1] - b;
+        u = p;
     }
 }
 
@@ -285,8 +386,8 @@ __device__ __forceinline__ double4 ldcg4(const double4 *p)
 }
 
 // thread `gtid` of `gthreads` takes nodes gtid, gtid + gthreads, ...
-__device__ __forceinline__ void monopoles_and_records(int M, int gtid, int gthreads, const double4 *sbody,
-                                                      const unsigned *nbegin, const unsigned *ncount,
+__device__ __forceinline__ void monopoles_and_records(int M, unsigned n, int gtid, int gthreads, const double4 *sbody,
+                                                      const unsigned *nbegin, unsigned *ncount,
                                                       const int *nfirst, const int *nparent, unsigned *node_meta,
                                                       double4 *mono, const unsigned char *nlevel, uint4 *winfo)
 {
@@ -295,9 +396,10 @@ __device__ __forceinline__ void monopoles_and_records(int M, int gtid, int gthre
         // written by the emission)
         const int first = nfirst[t];
         const unsigned kids = (unsigned)__popc(__ldcg(node_meta + t) & 0xffu);
-        winfo[t] = make_uint4(nbegin[t], ncount[t], (unsigned)first, (unsigned)nlevel[t] | (kids << 8));
+        const unsigned b = nbegin[t], c = node_count(t, M, n, nbegin, nparent);
+        ncount[t] = c;
+        winfo[t] = make_uint4(b, c, (unsigned)first, (unsigned)nlevel[t] | (kids << 8));
         if (first >= 0) continue;   // internal nodes are computed by their last child
-        const unsigned b = nbegin[t], c = ncount[t];
         double4 r;
         if (c == 1) {
             r = sbody[b];

@@ -721,6 +721,7 @@ int launch_direct(const Workspace &w, int64_t n, const int32_t *tgt, int64_t nt,
     splits = (tiles + tps - 1) / tps;
     const double eps2 = eps * eps;
     dim3 grid(tblocks, splits);
+    if (tgt) launch_iperm(w, n, s);   // sampled targets are named by body index: sorted position = iperm[index]
 #define BH_DIRECT(GUARD, POT)                                                                                          \
     do {                                                                                                               \
         if (per == 4)                                                                                                  \
@@ -741,7 +742,7 @@ int launch_direct(const Workspace &w, int64_t n, const int32_t *tgt, int64_t nt,
     if (splits > 1)
         direct_reduce_kernel<<<w.sms * 2, 256, 0, s>>>(w.stage_pos, rows, splits, potential ? -G : G,
                                                      potential ? 1 : 3, w.idx[0], tgt != nullptr, acc);
-    return splits > 1 ? 2 : 1;
+    return (splits > 1 ? 2 : 1) + (tgt ? 1 : 0);
 }
 
 void launch_kick_drift(double *pos, double *vel, const double *acc, int64_t n, double dt, cudaStream_t s)
