@@ -476,7 +476,7 @@ def run_own(args):
         te = (time.perf_counter() - t0) / ke
         out["e2e"] = {"value": w.n / te, "unit": UNIT, "h2d_bytes_per_step": 32 * w.n, "d2h_bytes_per_step": 24 * w.n,
                       "ms_per_step": te * 1e3, "call": "bh_eval_host (pinned host pos+mass in, acc out; mass upload beside the "
-                              "first build kernels; one code path, no state between calls)"}
+                              "first build kernels; the walk stores into the pinned output, no D2H copy; no state between calls)"}
 
         # ---- rows "next" of SURVEY.md 8(f), timed beside the headline ----
         if not args.no_next:

@@ -199,9 +199,13 @@ bh_status bh_aggregates(bh_ctx *ctx, int64_t n, const int32_t *pairs_dev, int64_
 double bh_gravity_dt(double G, double rho);
 
 /* End-to-end evaluation from HOST buffers: copies pos_host [n][3] and mass_host [n] to the GPU,
- * builds, walks, copies the accelerations to acc_host [n][3] and waits.  Pinned host memory makes the
+ * builds, walks, delivers the accelerations in acc_host [n][3] and waits.  Pinned host memory makes the
  * copies asynchronous; pageable memory works too.  The masses travel on a second stream beside the first
- * build kernels (they are first needed after the sort).  One code path, no state carried between calls. */
+ * build kernels (they are first needed after the sort).  If acc_host is pinned (cudaHostAlloc /
+ * cudaHostRegister, e.g. a torch pin_memory() tensor) the walk kernel stores the accelerations straight into
+ * it while it computes (the 24 bytes of a body in one store instruction of three adjacent lanes) and no copy
+ * follows; otherwise they are staged in the workspace and copied.  Nothing else decides the path and no state
+ * is carried between calls; both paths give the same bits. */
 bh_status bh_eval_host(bh_ctx *ctx, const double *pos_host, const double *mass_host, int64_t n,
                        double theta, double eps, double G, double *acc_host);
 

@@ -739,6 +739,17 @@ bh_status bh_copy_state_acc(bh_ctx *c, double *acc_dev)
                                          c->stream), "bh_copy_state_acc");
 }
 
+// device alias of a pinned (page-locked, mapped) host buffer, or nullptr for pageable memory
+static double *mapped_alias(const void *host)
+{
+    cudaPointerAttributes a{};
+    if (cudaPointerGetAttributes(&a, host) != cudaSuccess) {
+        cudaGetLastError();
+        return nullptr;
+    }
+    return a.type == cudaMemoryTypeHost ? static_cast<double *>(a.devicePointer) : nullptr;
+}
+
 bh_status bh_eval_host(bh_ctx *c, const double *pos_host, const double *mass_host, int64_t n, double theta,
                        double eps, double G, double *acc_host)
 {
@@ -759,11 +770,17 @@ bh_status bh_eval_host(bh_ctx *c, const double *pos_host, const double *mass_hos
     if (e != cudaSuccess) return cuda_check(c, e, "bh_eval_host H2D");
     bh_status st;
     if ((st = do_build(c, w.stage_pos, w.stage_mass, n, c->ev_copy[1])) != BH_OK) return st;
-    if ((st = do_accel(c, theta, eps, G, w.acc)) != BH_OK) return st;
+    // Pinned output (cudaHostAlloc / cudaHostRegister, e.g. a torch pin_memory() tensor): the walk stores the
+    // accelerations straight into it, 24 bytes per body in one or two write segments, while it computes, and
+    // no copy follows.  Pageable output: staged in the workspace and copied.
+    double *direct_out = mapped_alias(acc_host);
+    if ((st = do_accel(c, theta, eps, G, direct_out ? direct_out : w.acc)) != BH_OK) return st;
     c->have_acc = false;   // the internal acc buffer no longer belongs to the bound state
     c->acc_filled = false;
-    e = cudaMemcpyAsync(acc_host, w.acc, 3 * n * sizeof(double), cudaMemcpyDeviceToHost, c->stream);
-    if (e != cudaSuccess) return cuda_check(c, e, "bh_eval_host D2H");
+    if (!direct_out) {
+        e = cudaMemcpyAsync(acc_host, w.acc, 3 * n * sizeof(double), cudaMemcpyDeviceToHost, c->stream);
+        if (e != cudaSuccess) return cuda_check(c, e, "bh_eval_host D2H");
+    }
     return fetch_state(c);
 }
 

@@ -492,15 +492,26 @@ __device__ __forceinline__ void consume_group(PairSmem &ps, unsigned k, unsigned
         if ((int)quarter == s) { ox = tx; oy = ty; oz = tz; }
     }
     const long long j = gb + r + 8 * (sub + quarter * split);
-    if ((int)quarter < NS && j < ge) {
-        const unsigned i = perm[j];
-        if constexpr (MODE == 1) {
-            acc[i] = -G * ox;                       // phi, one value per body
-        } else {
-            if constexpr (MODE == 2) phi[i] = -G * op;
-            acc[3ll * i + 0] = G * ox;
-            acc[3ll * i + 1] = G * oy;
-            acc[3ll * i + 2] = G * oz;
+    const bool mine = (int)quarter < NS && j < ge;
+    const unsigned i = mine ? perm[j] : 0xffffffffu;
+    if constexpr (MODE == 1) {
+        if (mine) acc[i] = -G * ox;                 // phi, one value per body
+    } else {
+        if constexpr (MODE == 2) {
+            if (mine) phi[i] = -G * op;
+        }
+        // The three components of a body go out in ONE store instruction from three adjacent lanes (value
+        // v = 32 k + lane of instruction k is component v % 3 of the body held by lane v / 3), so the 24 bytes of a
+        // body leave as one or two write segments instead of three: it matters when acc is pinned host memory
+        // (bh_eval_host) and every segment is a PCIe write.
+        const double a0 = G * ox, a1 = G * oy, a2 = G * oz;
+#pragma unroll
+        for (int k = 0; k < 3; ++k) {
+            const unsigned v = 32u * k + lane, src = v / 3u, c = v - 3u * src;
+            const unsigned is = __shfl_sync(0xffffffffu, i, src);
+            const double b0 = __shfl_sync(0xffffffffu, a0, src), b1 = __shfl_sync(0xffffffffu, a1, src),
+                         b2 = __shfl_sync(0xffffffffu, a2, src);
+            if (is != 0xffffffffu) acc[3ll * is + c] = c == 0u ? b0 : (c == 1u ? b1 : b2);
         }
     }
 }

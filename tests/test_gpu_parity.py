@@ -264,8 +264,9 @@ def test_full_size_headline_config():
 
 
 def test_eval_host_pageable_and_pinned_agree():
-    """bh_eval_host has one code path: pageable and pinned host buffers, first and later calls, many and few
-    interactions per body all give the same accelerations bit for bit (no state is carried between calls)."""
+    """bh_eval_host: a pinned output is written by the walk kernel itself, a pageable one is staged and copied;
+    nothing else decides the path.  Pageable and pinned buffers, first and later calls, many and few interactions
+    per body all give the same accelerations bit for bit (no state is carried between calls)."""
     w = wl.make("c4", 20000)
     ctx = bh.Context(w.n, 16)
     pos_h, mass_h = torch.as_tensor(w.pos), torch.as_tensor(w.mass)
