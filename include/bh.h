@@ -11,7 +11,7 @@
  *     ("full double precision").  Arrays are dense, row-major: pos/vel/acc are [n][3].
  *   - Every call enqueues its work on the context's stream and returns without waiting for the
  *     GPU, except the calls documented as synchronising (bh_synchronize, bh_eval_host and the
- *     bh_get_* / bh_measure_* calls marked so below).  A context is not thread-safe.
+ *     bh_get_* calls marked so below).  A context is not thread-safe.
  *   - Return value: BH_OK (0) or a negative bh_status.  No exceptions, no abort().  Data errors that
  *     only the GPU can see (non-finite coordinates, node capacity) are sticky: they are reported by
  *     the next synchronising call.  bh_last_error() gives a human-readable message.
