@@ -68,7 +68,7 @@ class Microbench:
         from paper_1912_04197_b200 import build as pbuild
         self.C = C
         self.lib = C.CDLL(pbuild.MICRO_LIB)
-        for name in ("bhmb_fp64_peak", "bhmb_issue_model"):
+        for name in ("bhmb_fp64_peak", "bhmb_issue_model", "bhmb_fp64_mma"):
             getattr(self.lib, name).restype = C.c_int
             getattr(self.lib, name).argtypes = [C.c_void_p, C.POINTER(C.c_double)]
 
@@ -77,6 +77,13 @@ class Microbench:
         if self.lib.bhmb_fp64_peak(stream.cuda_stream, self.C.byref(v)) != 0:
             raise RuntimeError("bhmb_fp64_peak failed")
         return v.value
+
+    def fp64_mma(self, stream):
+        """The fp64 tensor-core MMA against the vector fp64 pipe: rates alone and whether they overlap."""
+        v = (self.C.c_double * 3)()
+        if self.lib.bhmb_fp64_mma(stream.cuda_stream, v) != 0:
+            raise RuntimeError("bhmb_fp64_mma failed")
+        return {"dfma_tflops": v[0], "dmma_m8n8k4_tflops": v[1], "interleaved_time_over_sum_of_times_alone": v[2]}
 
     def issue_model(self, stream):
         v = (self.C.c_double * 3)()
@@ -408,7 +415,7 @@ def run_own(args):
                 "peak_nominal": FP64_NOMINAL_TFLOPS, "frac_of_nominal": achieved / FP64_NOMINAL_TFLOPS,
                 "flops_per_interaction": FLOPS_PER_INTERACTION, "interactions_per_launch": inter_avg,
                 "interactions_per_s": inter_avg / (walk_avg_ms * 1e-3), "kernel_ms": walk_avg_ms,
-                "issue_model_interactions_per_s": issue,
+                "issue_model_interactions_per_s": issue, "fp64_tensor_core": mb.fp64_mma(stream),
                 "frac_of_eval_loop_alone": inter_avg / (walk_avg_ms * 1e-3) / issue["eval_loop_alone"],
                 "traffic": float(prof["dram_bytes_per_launch"]) if prof else None,
                 "l2_hit_rate": float(prof["l2_hit_pct"]) / 100.0 if prof else None,

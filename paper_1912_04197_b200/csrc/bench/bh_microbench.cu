@@ -3,6 +3,9 @@
 //                      denominator of the walk (a7) and direct (a8) kernels (MEASURED_PEAKS.json has no fp64 entry);
 //   bhmb_issue_model   the walk's own evaluation loop (bh_eval.cuh) alone on a sub-partition and beside
 //                      integer-issuing warps: what a warp-specialised walk can reach.
+//   bhmb_fp64_mma      the fp64 tensor-core MMA (mma.sync m8n8k4 f64 = DMMA.8) alone and interleaved with DFMA
+//                      chains: on sm_100 it runs at the vector fp64 rate AND on the same datapath (times add),
+//                      so recasting r^2 or the accumulation as a contraction cannot relieve the fp64 pipe.
 // Built into libbh_microbench.so by paper_1912_04197_b200/build.py; loaded by bench.py only.
 #include "../bh_eval.cuh"
 
@@ -64,6 +67,49 @@ __global__ void __launch_bounds__(512, 1) issue_model_kernel(double *sink, int i
     }
 }
 
+
+// MODE 0: eight DFMA chains per thread; 1: eight independent m8n8k4 f64 MMAs per warp; 2: both interleaved
+template <int MODE>
+__global__ void __launch_bounds__(256) fp64_mma_kernel(double *sink, int iters, double seed)
+{
+    double f[8], c[8][2];
+    const double m = 0.999999, q = 1e-9;
+    for (int i = 0; i < 8; ++i) { f[i] = seed + threadIdx.x + i; c[i][0] = seed * i; c[i][1] = seed + i; }
+    const double a = seed * 1e-3 + threadIdx.x * 1e-6, b = 1e-3;
+    for (int it = 0; it < iters; ++it) {
+        if (MODE != 1) {
+#pragma unroll
+            for (int i = 0; i < 8; ++i) f[i] = fma(f[i], m, q);
+        }
+        if (MODE != 0) {
+#pragma unroll
+            for (int i = 0; i < 8; ++i)
+                asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"
+                             : "+d"(c[i][0]), "+d"(c[i][1]) : "d"(a), "d"(b));
+        }
+    }
+    double s = 0;
+    for (int i = 0; i < 8; ++i) s += f[i] + c[i][0] + c[i][1];
+    if (s == 123456.789) sink[0] = s;
+}
+
+template <int MODE>
+static float run_fp64_mma_one(double *sink, int blocks, int iters, cudaStream_t s)
+{
+    cudaEvent_t a, b;
+    cudaEventCreate(&a);
+    cudaEventCreate(&b);
+    fp64_mma_kernel<MODE><<<blocks, 256, 0, s>>>(sink, 64, 1.0);
+    cudaEventRecord(a, s);
+    fp64_mma_kernel<MODE><<<blocks, 256, 0, s>>>(sink, iters, 1.0);
+    cudaEventRecord(b, s);
+    cudaEventSynchronize(b);
+    float ms = 0.f;
+    cudaEventElapsedTime(&ms, a, b);
+    cudaEventDestroy(a);
+    cudaEventDestroy(b);
+    return ms;
+}
 
 static int device_sms()
 {
@@ -139,6 +185,24 @@ int bhmb_issue_model(void *cuda_stream, double out_host[3])
     out_host[1] = run_issue_model_one<1>(sink, s);
     out_host[2] = run_issue_model_one<2>(sink, s);
     cudaFree(sink);
+    return cudaGetLastError() == cudaSuccess ? 0 : -1;
+}
+
+// out[0] = DFMA alone, out[1] = fp64 MMA alone (TFLOP/s, 2 flops per FMA), out[2] = time of both interleaved in
+// one warp divided by the sum of the two times alone (1.0: they share a datapath; 0.5: they overlap fully)
+int bhmb_fp64_mma(void *cuda_stream, double out_host[3])
+{
+    cudaStream_t s = (cudaStream_t)cuda_stream;
+    double *sink = nullptr;
+    if (!out_host || cudaMalloc(&sink, 256) != cudaSuccess) return -1;
+    const int blocks = device_sms() * 8, iters = 4000;
+    const double work = (double)blocks * 256 * iters;
+    const float t0 = run_fp64_mma_one<0>(sink, blocks, iters, s), t1 = run_fp64_mma_one<1>(sink, blocks, iters, s),
+                t2 = run_fp64_mma_one<2>(sink, blocks, iters, s);
+    cudaFree(sink);
+    out_host[0] = work * 16.0 / (t0 * 1e-3) / 1e12;     // 8 FMA per thread and iteration
+    out_host[1] = work * 128.0 / (t1 * 1e-3) / 1e12;    // 8 MMAs of 8 x 8 x 4 FMA per warp and iteration
+    out_host[2] = t2 / (t0 + t1);
     return cudaGetLastError() == cudaSuccess ? 0 : -1;
 }
 

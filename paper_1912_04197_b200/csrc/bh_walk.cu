@@ -231,7 +231,7 @@ __device__ void produce(PairSmem &ps, DevState *st, const unsigned *__restrict__
         const double glx = gbox[6 * g + 0], gly = gbox[6 * g + 1], glz = gbox[6 * g + 2];
         const double ghx = gbox[6 * g + 3], ghy = gbox[6 * g + 4], ghz = gbox[6 * g + 5];
         unsigned bot = 0, top = 1, gsp = 0;    // shared stack = [bot, top) mod kStack; gsp entries in the slab
-        unsigned n_mono = 0, n_direct = 0, my_tested = 0;
+        unsigned n_mono = 0, n_direct = 0, n_opened = 0;   // n_opened: nodes opened (internal + leaves); every tested node is accepted or opened
         if (lane == 0) stack[0] = make_uint2(0u, 1u);   // the root, as a range of one
         __syncwarp();
         unsigned tail_prev = P.tail;           // ring fill at the end of the previous trip
@@ -273,7 +273,6 @@ __device__ void produce(PairSmem &ps, DevState *st, const unsigned *__restrict__
                 const bool accept = have && !overlap && (s2 < __dmul_rn(theta2, d2));
                 const bool open_int = have && !accept && internal;
                 const bool open_leaf = have && !accept && !internal;
-                my_tested += have ? 1u : 0u;
                 // ---- accepted nodes -> ring ----
                 {
                     const unsigned m = __ballot_sync(0xffffffffu, accept);
@@ -300,6 +299,7 @@ __device__ void produce(PairSmem &ps, DevState *st, const unsigned *__restrict__
                         }
                         if (open_int) stack[(top + __popc(m & lt)) & (kStack - 1)] = make_uint2(cur.info.z, (cur.info.w >> 8) & 0xffu);
                         top += __popc(m);
+                        n_opened += __popc(m);
                     }
                 }
                 // ---- opened leaves -> their bodies, asynchronously into the ring ----
@@ -343,6 +343,7 @@ __device__ void produce(PairSmem &ps, DevState *st, const unsigned *__restrict__
                             P.tail += n;
                         }
                         n_direct += total;
+                        n_opened += __popc(m);
                         __syncwarp();                                  // the scratch row is read before it is rewritten
                     }
                 }
@@ -371,10 +372,8 @@ __device__ void produce(PairSmem &ps, DevState *st, const unsigned *__restrict__
         tot_mono += n_mono;
         tot_direct += n_direct;
         tot_inter += (unsigned long long)(n_mono + n_direct) * (unsigned long long)(ge - gb);
-        tot_tested += my_tested;               // per lane; summed over the warp by the atomics below
+        tot_tested += n_mono + n_opened;       // warp-uniform
     }
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) tot_tested += __shfl_xor_sync(0xffffffffu, tot_tested, o);
     if (lane == 0) {
         atomicAdd(&st->stats[0], tot_mono);
         atomicAdd(&st->stats[1], tot_direct);

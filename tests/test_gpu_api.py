@@ -116,3 +116,6 @@ def test_roofline_microbenchmarks_are_sane():
     bound = 148 * 4 * 1.965e9                         # one interaction per cycle per sub-partition
     assert 0.6 * bound < m["beside_low_duty_integer_warps"] < m["eval_loop_alone"] <= 1.02 * bound
     assert m["beside_full_rate_integer_warps"] < m["eval_loop_alone"]
+    t = mb.fp64_mma(stream)
+    # on sm_100 the fp64 MMA runs at the vector fp64 rate and does not overlap with it
+    assert 0.8 * peak < t["dmma_m8n8k4_tflops"] < 1.2 * peak and t["interleaved_time_over_sum_of_times_alone"] > 0.85
