@@ -420,6 +420,36 @@ def test_c5_after_fifty_kdk_steps():
     ctx.close()
 
 
+def test_scale_16m_bodies():
+    """Beyond the largest BASELINE.json configuration: configs[4]'s cloud at N = 16 777 216 (7 GB of workspace; the
+    arrays no longer fit the L2, 4096 sort tiles per pass, 590 000 groups).  Tree bit for bit, sampled groups
+    against the oracle's walk, the walk's totals consistent with the per-group counts."""
+    w = wl.make("c5", 16777216)
+    t = orc.build(w.pos, w.mass, w.leaf_cap)
+    ctx = gpu_build(w.pos, w.mass, w.leaf_cap)
+    g = ctx.tree()
+    assert g["lo"] == list(t.lo) and g["L"] == t.L and (g["M"], g["depth"]) == (t.M, t.depth)
+    for key, ref, view in [("skey", t.skey, np.uint64), ("perm", t.perm, np.uint32), ("begin", t.begin, np.uint32),
+                           ("count", t.count, np.uint32), ("gstart", t.gstart, np.uint32)]:
+        assert np.array_equal(g[key].cpu().numpy().view(view), ref), key
+    for key, ref in [("level", t.level), ("first_child", t.first_child), ("child_mask", t.child_mask), ("parent", t.parent)]:
+        assert np.array_equal(g[key].cpu().numpy(), ref), key
+    assert np.array_equal(g["mono"].cpu().numpy().view(np.uint64), t.mono.view(np.uint64))
+    assert np.array_equal(g["glo"].cpu().numpy(), t.glo) and np.array_equal(g["ghi"].cpu().numpy(), t.ghi)
+    del g
+    a = ctx.accel(w.theta, w.eps, w.G).cpu().numpy()
+    gm, gd = (x.cpu().numpy().view(np.uint32) for x in ctx.counts())
+    ng = t.ngroups
+    for g0 in list(range(0, ng, ng // 6))[:6] + [ng - 2]:
+        ref, nm, nd, _ = orc.accel(t, w.theta, w.eps, w.G, g0, g0 + 2)
+        rows = t.perm[t.gstart[g0]:t.gstart[g0 + 2]]
+        assert np.array_equal(gm[g0:g0 + 2], nm) and np.array_equal(gd[g0:g0 + 2], nd)
+        assert relerr(a[rows], ref[rows]).max() <= TOL
+    st = bh.bh_get_stats(ctx.ctx)
+    assert st["interactions"] == int(((gm.astype(np.int64) + gd) * np.diff(t.gstart.astype(np.int64))).sum())
+    ctx.close()
+
+
 @pytest.mark.parametrize("name,n,C,theta,sampled", [("c4", 30000, 1, 0.1, False), ("c3", 131072, 4, 0.0, True),
                                                      ("c4", 100000, 1, 0.0, True)])
 def test_stack_spill_path(name, n, C, theta, sampled):
