@@ -45,7 +45,7 @@ constexpr unsigned kNoGroup = 0xffffffffu;
 #endif
 constexpr int kTripUnroll = BH_TRIP_UNROLL;   // producer: trips of a pop unrolled
 #ifndef BH_PUB_MIN
-#define BH_PUB_MIN 0                        // a trip publishes only if at least this many entries are pending
+#define BH_PUB_MIN 32                       // a trip publishes only if more than this many entries are pending (the consumer starts a batch at 32)
 #endif
 
 
@@ -64,7 +64,7 @@ struct PairCtrl {                            // all words are written by one rol
 struct PairSmem {
     double4 ring[kRing];
     uint2 stack[kStack];                     // (first sibling, count) ranges
-    unsigned leaf_src[32];                   // producer scratch: (first body - offset in the run) per opened leaf
+    unsigned leaf_src[2][32];                // producer scratch: (first body - offset in the run) per opened leaf, rows by trip parity
     PairCtrl ctrl;
 };
 
@@ -231,7 +231,8 @@ __device__ void produce(PairSmem &ps, DevState *st, const unsigned *__restrict__
         const double glx = gbox[6 * g + 0], gly = gbox[6 * g + 1], glz = gbox[6 * g + 2];
         const double ghx = gbox[6 * g + 3], ghy = gbox[6 * g + 4], ghz = gbox[6 * g + 5];
         unsigned bot = 0, top = 1, gsp = 0;    // shared stack = [bot, top) mod kStack; gsp entries in the slab
-        unsigned n_mono = 0, n_direct = 0, n_opened = 0;   // n_opened: nodes opened (internal + leaves); every tested node is accepted or opened
+        unsigned n_direct = 0, n_tested = 0;
+        const unsigned tail_begin = P.tail;    // the ring only ever receives this group's monopoles and bodies: n_mono follows from the tail
         if (lane == 0) stack[0] = make_uint2(0u, 1u);   // the root, as a range of one
         __syncwarp();
         unsigned tail_prev = P.tail;           // ring fill at the end of the previous trip
@@ -252,6 +253,19 @@ __device__ void produce(PairSmem &ps, DevState *st, const unsigned *__restrict__
             __syncwarp();                      // the entries are read before later pushes reuse their slots
             const unsigned first = ent.x, nsib = ent.y;
             const unsigned trips = __reduce_max_sync(0xffffffffu, nsib);
+            n_tested += __reduce_add_sync(0xffffffffu, nsib);   // every sibling of a popped range is tested
+            // room for everything this pop can push (32 child ranges per trip): spill the oldest entries first
+            while (top - bot + 32u * trips > (unsigned)kStack) {
+                if (gsp + kSpill > (unsigned)kStackSlab) {      // cannot happen within the slab bound
+                    if (lane == 0) atomicOr(&st->status, (int)kStatStack);
+                    bot = top;                                  // drop the stack: the walk ends early
+                } else {
+                    for (unsigned u = lane; u < (unsigned)kSpill; u += 32) slab[gsp + u] = stack[(bot + u) & (kStack - 1)];
+                    gsp += kSpill;
+                    bot += kSpill;
+                    ++tot_spills;
+                }
+            }
             NodeRec nxt;
             nxt.info = make_uint4(0u, 0u, 0u, 0u);
             nxt.mn = make_double4(0.0, 0.0, 0.0, 0.0);
@@ -260,7 +274,6 @@ __device__ void produce(PairSmem &ps, DevState *st, const unsigned *__restrict__
             for (unsigned q = 0; q < trips; ++q) {
                 const bool have = q < nsib;
                 const NodeRec cur = nxt;
-                if (q + 1 < nsib) nxt = load_rec(winfo, mono, first + q + 1);
                 // ---- opening test (canonical arithmetic, R22) ----
                 const unsigned nb = cur.info.x, nc = cur.info.y;
                 const bool internal = (int)cur.info.z >= 0;
@@ -273,33 +286,33 @@ __device__ void produce(PairSmem &ps, DevState *st, const unsigned *__restrict__
                 const bool accept = have && !overlap && (s2 < __dmul_rn(theta2, d2));
                 const bool open_int = have && !accept && internal;
                 const bool open_leaf = have && !accept && !internal;
+                // the three votes side by side: ptxas guards every warp collective that follows a branch with a
+                // convergence check (two instructions), and adjacent ones share it
+                const unsigned m_acc = __ballot_sync(0xffffffffu, accept);
+                const unsigned m_int = __ballot_sync(0xffffffffu, open_int);
+                const unsigned m_leaf = __ballot_sync(0xffffffffu, open_leaf);
                 // ---- accepted nodes -> ring ----
                 {
-                    const unsigned m = __ballot_sync(0xffffffffu, accept);
+                    const unsigned m = m_acc;
                     const unsigned cnt = __popc(m);
                     P.reserve(cnt);
                     if (accept) ps.ring[(P.tail + __popc(m & lt)) & (kRing - 1)] = cur.mn;
                     P.tail += cnt;
-                    n_mono += cnt;
                 }
+                // the record of the lane's next sibling is requested once the accepted monopoles are in the ring: the
+                // centre-of-mass registers are free by then, so only the four info words have to be kept aside
+                // (requested at the top of the trip the whole record is copied every trip: 5.09 -> 5.05 ms)
+                const unsigned fc = cur.info.z, lw = cur.info.w;
+                if (q + 1 < nsib) nxt = load_rec(winfo, mono, first + q + 1);
                 // ---- opened internal nodes -> their child ranges onto the stack ----
                 {
-                    const unsigned m = __ballot_sync(0xffffffffu, open_int);
+                    const unsigned m = m_int;
                     if (m) {
-                        if (top - bot + 32u > (unsigned)kStack) {       // spill the oldest kSpill entries
-                            if (gsp + kSpill > (unsigned)kStackSlab) {  // cannot happen within the slab bound
-                                if (lane == 0) atomicOr(&st->status, (int)kStatStack);
-                                bot = top;                              // drop the stack: the walk ends early
-                            } else {
-                                for (unsigned u = lane; u < (unsigned)kSpill; u += 32) slab[gsp + u] = stack[(bot + u) & (kStack - 1)];
-                                gsp += kSpill;
-                                bot += kSpill;
-                                ++tot_spills;
-                            }
-                        }
-                        if (open_int) stack[(top + __popc(m & lt)) & (kStack - 1)] = make_uint2(cur.info.z, (cur.info.w >> 8) & 0xffu);
+                        // slot and value computed by every lane, only the store is predicated (no branch around it)
+                        const unsigned slot = (top + __popc(m & lt)) & (kStack - 1);
+                        const uint2 range = make_uint2(fc, (lw >> 8) & 0xffu);
+                        if (open_int) stack[slot] = range;
                         top += __popc(m);
-                        n_opened += __popc(m);
                     }
                 }
                 // ---- opened leaves -> their bodies, asynchronously into the ring ----
@@ -308,7 +321,7 @@ __device__ void produce(PairSmem &ps, DevState *st, const unsigned *__restrict__
                 // and every lane then copies one body per window of 32, finding its leaf by counting
                 // the leaf starts at or before its slot.
                 {
-                    const unsigned m = __ballot_sync(0xffffffffu, open_leaf);
+                    const unsigned m = m_leaf;
                     if (m) {
                         const unsigned c = open_leaf ? nc : 0u;
                         unsigned inc = c;
@@ -319,9 +332,19 @@ __device__ void produce(PairSmem &ps, DevState *st, const unsigned *__restrict__
                         }
                         const unsigned total = __shfl_sync(0xffffffffu, inc, 31);
                         const unsigned excl = inc - c;
-                        if (open_leaf) ps.leaf_src[__popc(m & lt)] = nb - excl;
+                        unsigned *lsrc = ps.leaf_src[q & 1u];          // alternate rows: the next trip does not wait for this one's reads
+                        if (open_leaf) lsrc[__popc(m & lt)] = nb - excl;
                         __syncwarp();
                         unsigned owners = 0;                           // leaves that start before this window
+#ifdef BH_EXP_NOLEAFCOPY
+                        for (unsigned base = 0; base < total; base += 32) {
+                            const unsigned n = total - base < 32u ? total - base : 32u;
+                            P.reserve(n);
+                            P.tail += n;
+                        }
+                        if (owners == 77u) ps.ring[0] = sbody[lsrc[lane]];
+                        if (0)
+#endif
                         for (unsigned base = 0; base < total; base += 32) {
                             const unsigned rel = excl - base;
                             const unsigned heads = __reduce_or_sync(0xffffffffu, (open_leaf && rel < 32u) ? 1u << rel : 0u);
@@ -331,7 +354,7 @@ __device__ void produce(PairSmem &ps, DevState *st, const unsigned *__restrict__
                             P.reserve(n);
                             if (lane < n) {
                                 char *dst = reinterpret_cast<char *>(&ps.ring[(P.tail + lane) & (kRing - 1)]);
-                                const unsigned src = ps.leaf_src[k] + base + lane;
+                                const unsigned src = lsrc[k] + base + lane;
                                 const char *from = reinterpret_cast<const char *>(sbody + src);
                                 if (POT && src >= gb && src < ge) {
                                     ps.ring[(P.tail + lane) & (kRing - 1)] = make_double4(0.0, 0.0, 0.0, 0.0);
@@ -343,8 +366,6 @@ __device__ void produce(PairSmem &ps, DevState *st, const unsigned *__restrict__
                             P.tail += n;
                         }
                         n_direct += total;
-                        n_opened += __popc(m);
-                        __syncwarp();                                  // the scratch row is read before it is rewritten
                     }
                 }
                 // ---- publish what is complete: everything up to the end of the previous trip ----
@@ -360,6 +381,7 @@ __device__ void produce(PairSmem &ps, DevState *st, const unsigned *__restrict__
         // ---- the list of this group is complete ----
         cp_async_wait_all();
         __syncwarp();
+        const unsigned n_mono = P.tail - tail_begin - n_direct;
         if (lane == 0) {
             ps.ctrl.desc_end[k % kDesc] = P.tail;
             st_release(&ps.ctrl.tail_pub, P.tail);
@@ -372,7 +394,7 @@ __device__ void produce(PairSmem &ps, DevState *st, const unsigned *__restrict__
         tot_mono += n_mono;
         tot_direct += n_direct;
         tot_inter += (unsigned long long)(n_mono + n_direct) * (unsigned long long)(ge - gb);
-        tot_tested += n_mono + n_opened;       // warp-uniform
+        tot_tested += n_tested;                // warp-uniform
     }
     if (lane == 0) {
         atomicAdd(&st->stats[0], tot_mono);
