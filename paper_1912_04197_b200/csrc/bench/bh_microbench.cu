@@ -48,7 +48,7 @@ __global__ void __launch_bounds__(512, 1) issue_model_kernel(double *sink, int i
             B.x[s] = 0.1 * lane + s; B.y[s] = 0.2 * s; B.z[s] = 0.05 * lane;
             B.ax[s] = B.ay[s] = B.az[s] = B.ph[s] = 0.0;
         }
-        for (int it = 0; it < iters; ++it) eval_chunks<false, 4, 0>(ring, 0u, 512u, quarter, eps2, B);
+        for (int it = 0; it < iters; ++it) eval_blocks<false, 4, 0>(ring, 0u, 512u, quarter, eps2, B);
         double s = 0.0;
         for (int q = 0; q < 4; ++q) s += B.ax[q] + B.ay[q] + B.az[q];
         if (s == 123.456) sink[0] = s;

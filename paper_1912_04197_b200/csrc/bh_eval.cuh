@@ -11,10 +11,6 @@ constexpr int kRing = 512;                  // sources per producer/consumer pai
 #ifndef BH_SEED_LOWWORD
 #define BH_SEED_LOWWORD 1                   // rsqrt seed: low word taken from a dead register pair (see interact)
 #endif
-#ifndef BH_EVAL_UNROLL
-#define BH_EVAL_UNROLL 4
-#endif
-constexpr int kEvalUnroll = BH_EVAL_UNROLL;   // consumer: chunks of eight sources unrolled
 // GUARD (chosen by the launchers when eps^2 is below the smallest normal double, eps = 0 included): a softened
 // squared distance that is zero or subnormal adds nothing.  rsqrt.approx.ftz flushes a subnormal argument to
 // zero and would return infinity, and with it 0 * inf = NaN for a coincident pair (R13; bh.h preconditions).
@@ -119,12 +115,12 @@ struct Bodies {
     double x[NS], y[NS], z[NS], ax[NS], ay[NS], az[NS], ph[NS];   // ph only lives in MODE 2
 };
 
-// evaluate n8 (a multiple of 8) sources starting at ring position head (a multiple of 8)
+// evaluate n8 (a multiple of 8) sources starting at ring position head (a multiple of 8): the end of a list
 template <bool GUARD, int NS, int MODE>
 __device__ __forceinline__ void eval_chunks(const double4 *ring, unsigned head, unsigned n8, unsigned quarter,
                                             double eps2, Bodies<NS> &B)
 {
-#pragma unroll kEvalUnroll
+#pragma unroll 1
     for (unsigned i = 0; i < n8; i += 8) {
         const double4 *p = ring + ((head + i) & (kRing - 1)) + quarter;
         const double4 s0 = p[0], s1 = p[4];
@@ -132,6 +128,27 @@ __device__ __forceinline__ void eval_chunks(const double4 *ring, unsigned head, 
         for (int k = 0; k < NS; ++k) interact_any<GUARD, MODE>(B.x[k], B.y[k], B.z[k], eps2, s0, B.ax[k], B.ay[k], B.az[k], B.ph[k]);
 #pragma unroll
         for (int k = 0; k < NS; ++k) interact_any<GUARD, MODE>(B.x[k], B.y[k], B.z[k], eps2, s1, B.ax[k], B.ay[k], B.az[k], B.ph[k]);
+    }
+}
+
+// the same over n32 (a multiple of 32) sources starting at a ring position that is a multiple of 32: a block of
+// four chunks never wraps, so it has ONE ring address and constant offsets (the chunk-wise loop computes a masked
+// address per chunk: 13 more integer instructions per 512 fp64 ones, and every one of them takes an issue slot)
+template <bool GUARD, int NS, int MODE>
+__device__ __forceinline__ void eval_blocks(const double4 *ring, unsigned head, unsigned n32, unsigned quarter,
+                                            double eps2, Bodies<NS> &B)
+{
+#pragma unroll 1
+    for (unsigned i = 0; i < n32; i += 32) {
+        const double4 *p = ring + ((head + i) & (kRing - 1)) + quarter;
+#pragma unroll
+        for (int c = 0; c < 4; ++c) {
+            const double4 s0 = p[8 * c], s1 = p[8 * c + 4];
+#pragma unroll
+            for (int k = 0; k < NS; ++k) interact_any<GUARD, MODE>(B.x[k], B.y[k], B.z[k], eps2, s0, B.ax[k], B.ay[k], B.az[k], B.ph[k]);
+#pragma unroll
+            for (int k = 0; k < NS; ++k) interact_any<GUARD, MODE>(B.x[k], B.y[k], B.z[k], eps2, s1, B.ax[k], B.ay[k], B.az[k], B.ph[k]);
+        }
     }
 }
 

@@ -212,7 +212,7 @@ __device__ void produce(PairSmem &ps, DevState *st, const unsigned *__restrict__
         g = __shfl_sync(0xffffffffu, g, 0);
         if (g >= ngroups) g = kNoGroup;
         while (k - warp_acquire_min(ps.ctrl.consumed, split, lane) >= (unsigned)kDesc) __nanosleep(256);
-        P.tail = (P.tail + 7u) & ~7u;          // a group's sources start on a chunk boundary
+        P.tail = (P.tail + 31u) & ~31u;        // a group's sources start on a block boundary (eval_blocks)
         if (lane == 0) {
             ps.ctrl.desc_g[k % kDesc] = g;
             ps.ctrl.desc_begin[k % kDesc] = P.tail;
@@ -461,10 +461,15 @@ __device__ __forceinline__ void consume_group(PairSmem &ps, unsigned k, unsigned
             __nanosleep(32);
             continue;
         }
-        const unsigned n8 = avail > 0 ? ((unsigned)avail & ~7u) : 0u;
-        eval_chunks<GUARD, NS, MODE>(ps.ring, head, n8, quarter, eps2, B);
-        head += n8;
+        // whole blocks of 32 sources (the group's list starts on a multiple of 32 in the ring, so head stays one
+        // until the list ends); the chunks of eight that are left once the list is complete
+        const unsigned n32 = avail > 0 ? ((unsigned)avail & ~31u) : 0u;
+        eval_blocks<GUARD, NS, MODE>(ps.ring, head, n32, quarter, eps2, B);
+        head += n32;
         if (fin) {
+            const unsigned n8 = (unsigned)(avail > 0 ? avail : 0) & 24u;
+            eval_chunks<GUARD, NS, MODE>(ps.ring, head, n8, quarter, eps2, B);
+            head += n8;
             const unsigned rest = (unsigned)(avail > 0 ? avail : 0) & 7u;
             if (rest) {                             // last, partial chunk: absent sources are massless
                 const double4 *p = ps.ring + (head & (kRing - 1)) + quarter;
