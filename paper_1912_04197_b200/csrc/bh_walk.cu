@@ -336,15 +336,6 @@ __device__ void produce(PairSmem &ps, DevState *st, const unsigned *__restrict__
                         if (open_leaf) lsrc[__popc(m & lt)] = nb - excl;
                         __syncwarp();
                         unsigned owners = 0;                           // leaves that start before this window
-#ifdef BH_EXP_NOLEAFCOPY
-                        for (unsigned base = 0; base < total; base += 32) {
-                            const unsigned n = total - base < 32u ? total - base : 32u;
-                            P.reserve(n);
-                            P.tail += n;
-                        }
-                        if (owners == 77u) ps.ring[0] = sbody[lsrc[lane]];
-                        if (0)
-#endif
                         for (unsigned base = 0; base < total; base += 32) {
                             const unsigned rel = excl - base;
                             const unsigned heads = __reduce_or_sync(0xffffffffu, (open_leaf && rel < 32u) ? 1u << rel : 0u);
