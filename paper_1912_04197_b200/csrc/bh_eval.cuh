@@ -138,17 +138,26 @@ template <bool GUARD, int NS, int MODE>
 __device__ __forceinline__ void eval_blocks(const double4 *ring, unsigned head, unsigned n32, unsigned quarter,
                                             double eps2, Bodies<NS> &B)
 {
+    // the first two sources of the NEXT block are requested while the last chunk of this one is evaluated, so a
+    // block does not start with an exposed shared-memory latency (the slots beyond the published limit are only
+    // read, never used: the loop ends first)
+    if (n32 == 0) return;
+    const double4 *p = ring + (head & (kRing - 1)) + quarter;
+    double4 s0 = p[0], s1 = p[4];
 #pragma unroll 1
     for (unsigned i = 0; i < n32; i += 32) {
-        const double4 *p = ring + ((head + i) & (kRing - 1)) + quarter;
+        const double4 *pn = ring + ((head + i + 32) & (kRing - 1)) + quarter;
 #pragma unroll
         for (int c = 0; c < 4; ++c) {
-            const double4 s0 = p[8 * c], s1 = p[8 * c + 4];
+            const double4 a0 = s0, a1 = s1;
+            if (c < 3) { s0 = p[8 * c + 8]; s1 = p[8 * c + 12]; }
+            else { s0 = pn[0]; s1 = pn[4]; }
 #pragma unroll
-            for (int k = 0; k < NS; ++k) interact_any<GUARD, MODE>(B.x[k], B.y[k], B.z[k], eps2, s0, B.ax[k], B.ay[k], B.az[k], B.ph[k]);
+            for (int k = 0; k < NS; ++k) interact_any<GUARD, MODE>(B.x[k], B.y[k], B.z[k], eps2, a0, B.ax[k], B.ay[k], B.az[k], B.ph[k]);
 #pragma unroll
-            for (int k = 0; k < NS; ++k) interact_any<GUARD, MODE>(B.x[k], B.y[k], B.z[k], eps2, s1, B.ax[k], B.ay[k], B.az[k], B.ph[k]);
+            for (int k = 0; k < NS; ++k) interact_any<GUARD, MODE>(B.x[k], B.y[k], B.z[k], eps2, a1, B.ax[k], B.ay[k], B.az[k], B.ph[k]);
         }
+        p = pn;
     }
 }
 
