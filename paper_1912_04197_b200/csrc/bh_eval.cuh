@@ -139,14 +139,14 @@ __device__ __forceinline__ void eval_blocks(const double4 *ring, unsigned head, 
                                             double eps2, Bodies<NS> &B)
 {
     // the first two sources of the NEXT block are requested while the last chunk of this one is evaluated, so a
-    // block does not start with an exposed shared-memory latency (the slots beyond the published limit are only
-    // read, never used: the loop ends first)
+    // block does not start with an exposed shared-memory latency
     if (n32 == 0) return;
     const double4 *p = ring + (head & (kRing - 1)) + quarter;
     double4 s0 = p[0], s1 = p[4];
 #pragma unroll 1
     for (unsigned i = 0; i < n32; i += 32) {
-        const double4 *pn = ring + ((head + i + 32) & (kRing - 1)) + quarter;
+        // (after the last block of the batch the request goes to this block again: nothing beyond the published limit is read)
+        const double4 *pn = ring + ((head + (i + 32 < n32 ? i + 32 : i)) & (kRing - 1)) + quarter;
 #pragma unroll
         for (int c = 0; c < 4; ++c) {
             const double4 a0 = s0, a1 = s1;
