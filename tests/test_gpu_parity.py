@@ -81,6 +81,39 @@ def test_accel_counts_exact_and_values_within_tolerance(name, n, C):
     ctx.close()
 
 
+def _tested_nodes_from_lists(t, theta):
+    """Nodes the opening criterion is applied to, from the oracle's lists alone: every tested node is accepted
+    (it is in a monopole list) or opened (it is a strict ancestor of a list entry, or a leaf whose bodies are in a
+    direct list); the root is tested, and so is every child of an opened internal node."""
+    leaves = np.where(t.first_child < 0)[0]
+    order = np.argsort(t.begin[leaves])
+    leaves, lbegin = leaves[order], t.begin[leaves][order]
+    total = 0
+    for g in range(t.ngroups):
+        mono, direct = orc.walk_lists(t, g, theta)
+        opened_leaves = np.unique(leaves[np.searchsorted(lbegin, direct, side="right") - 1]) if len(direct) else []
+        opened = set(int(x) for x in opened_leaves)
+        for x in list(mono) + list(opened_leaves):
+            x = int(t.parent[int(x)])
+            while x >= 0 and x not in opened:
+                opened.add(x)
+                x = int(t.parent[x])
+        total += len(mono) + len(opened)
+    return total
+
+
+@pytest.mark.parametrize("name,n,C,theta", [("c4", 5000, 16, 0.5), ("c1", 1024, 8, 0.5), ("c3", 3000, 4, 0.0),
+                                            ("c5", 4000, 32, 0.9)])
+def test_tested_node_count_follows_from_the_oracle_lists(name, n, C, theta):
+    # stats[3] is counted by the producer at every pop (all siblings of a popped range are tested)
+    w = wl.make(name, n)
+    t = orc.build(w.pos, w.mass, C)
+    ctx = gpu_build(w.pos, w.mass, C)
+    ctx.accel(theta, w.eps, w.G)
+    assert bh.bh_get_stats(ctx.ctx)["nodes_tested"] == _tested_nodes_from_lists(t, theta)
+    ctx.close()
+
+
 @pytest.mark.parametrize("name,n,C", [("c1", 1024, 8), ("c2", 16384, 16), ("c4", 5000, 16), ("c1", 300, 8)])
 def test_direct_sum(name, n, C):
     w = wl.make(name, n)
