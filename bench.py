@@ -46,6 +46,14 @@ def workload_desc(w):
             f"W=32, Gc=512, KDK dt={w.dt:g}")
 
 
+def config_dict(w, world: int):
+    """The `config` object of BOTH arms (the driver compares them): the workload and how the timed region treats the
+    caches.  What a run found out about the workload (tree size, sample) goes into other keys."""
+    return {"workload": workload_desc(w), "parallelism": "replicas only" if world > 1 else "1 gpu",
+            "l2": "own arm: L2 flushed between steps (256 MiB write), per-step CUDA events summed; "
+                  "reference arm: the oracle on host cores, bounded sample of the workload"}
+
+
 def profile_row(kernel: str, config: str):
     """Profiler figures of one kernel launch (dram bytes, L2 hit rate, ...) from the committed summary of the
     ncu --set full captures, profiles/r02_roofline.csv (its .md names the commands and the commit)."""
@@ -242,7 +250,7 @@ def run_reference(args):
             "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": 1e3 * (time.perf_counter() - t_all0) / (args.steps + args.warmup),
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
-            "data": "synthetic", "config": {"workload": workload_desc(w), "sampled": True},
+            "data": "synthetic", "config": config_dict(w, args.gpus),
             "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc},
             "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "gpu_launches": 0}
@@ -437,9 +445,7 @@ def run_own(args):
     out = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
            "warmup": max(3, args.warmup), "ms_per_step": total_ms / args.steps, "higher_is_better": True,
            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-           "config": {"workload": workload_desc(w), "parallelism": "replicas only" if world > 1 else "1 gpu",
-                      "l2": "flushed between steps (256 MiB write); per-step CUDA events summed",
-                      "nodes": M, "depth": depth, "groups": ng},
+           "config": config_dict(w, world), "tree": {"nodes": M, "depth": depth, "groups": ng},
            "clocks": clocks, "gpu_launches": int(launches), "wall_s": wall,
            "phases_ms": phases, "roofline": roofline, "build_roofline": build_roof,
            "interactions_per_body": st["interactions"] / w.n}
