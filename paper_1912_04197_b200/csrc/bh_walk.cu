@@ -12,13 +12,15 @@
 //             node that holds a body of the group); the results are appended by ballot/prefix:
 //             accepted nodes -> their (cx,cy,cz,m) into the ring; opened internal nodes -> their child
 //             range onto the stack; opened leaves -> their bodies (x,y,z,m) into the ring (cp.async,
-//             straight from L2).  The record of a lane's next sibling is loaded while the current one
-//             is tested.  The producer is written for instruction count: on sm_100 every instruction
-//             another warp issues costs the fp64 warps of the same sub-partition an issue slot.
+//             straight from L2).  The record of a lane's next sibling is requested as soon as the accepted
+//             monopoles of the trip are in the ring.  The producer is written for instruction count: on
+//             sm_100 every integer / move / branch instruction another warp issues costs the fp64 warps of
+//             the same sub-partition a dispatch cycle (loads, stores and shuffles do not).
 //   consumer  lanes = bodies.  It evaluates the sources the producer has published, in fp64: every
 //             lane carries FOUR bodies of the group (lane l: bodies l%8 + 8k) and the four quarter-warps
 //             take alternate sources, so one shared-memory read of a source feeds four interactions and
-//             the fp64 pipe, not the load-store path, sets the pace.
+//             the fp64 pipe, not the load-store path, sets the pace.  Sources are taken in blocks of 32
+//             from a block-aligned ring position (bh_eval.cuh).
 // The two roles meet only through release/acquire counters in shared memory, so the fp64 pipe of an SM
 // sub-partition is fed by its two consumers while its two producers wait on L2.
 // The test arithmetic is the canonical one (each operation rounded once, fma where stated) so that
