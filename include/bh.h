@@ -246,7 +246,9 @@ bh_status bh_get_launches(bh_ctx *ctx, uint64_t *count_host);
 /* Phase timing with CUDA events on the context's stream.  After bh_set_timing(ctx, 1) every
  * bh_build/bh_accel/bh_direct records events; bh_get_phase_ms (synchronising) returns the last
  * durations in ms: [0] cube, [1] keys+histogram, [2] sort, [3] gather+boxes, [4] tree,
- * [5] monopoles, [6] walk, [7] direct, [8] kick/drift kernels of the last bh_kdk_step. */
+ * [5] monopoles, [6] walk, [7] direct, [8] kick/drift kernels of the last bh_kdk_step.  A build of at most
+ * 1024 bodies per multiprocessor is ONE kernel (one block up to 4096 bodies, one co-resident grid with grid
+ * barriers above): its whole duration is reported as [4] and [0]-[3], [5] are 0. */
 #define BH_NUM_PHASES 9
 bh_status bh_set_timing(bh_ctx *ctx, int enable);
 bh_status bh_get_phase_ms(bh_ctx *ctx, float ms_host[BH_NUM_PHASES]);

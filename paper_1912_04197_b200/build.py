@@ -13,6 +13,9 @@ NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", 
               "--fmad=true", "-Xcompiler", "-fPIC", "-shared", "-cudart", "static"]
 
 
+PER_FILE_FLAGS = {}    # extra nvcc flags of single translation units (none at present)
+
+
 def sources():
     return sorted(glob.glob(os.path.join(HERE, "csrc", "*.cu")))
 
@@ -43,7 +46,8 @@ def build(force: bool = False, verbose: bool = False) -> str:
     jobs = []
     for src in sources() + micro_sources():
         obj = os.path.join(objdir, os.path.basename(src)[:-3] + ".o")
-        jobs.append((src, obj, subprocess.Popen([nvcc] + flags + ["-c", "-o", obj, src])))
+        jobs.append((src, obj, subprocess.Popen([nvcc] + flags + PER_FILE_FLAGS.get(os.path.basename(src), []) +
+                                                ["-c", "-o", obj, src])))
     if any(j.wait() != 0 for _, _, j in jobs):
         raise RuntimeError("nvcc failed")
     objs = {src: obj for src, obj, _ in jobs}

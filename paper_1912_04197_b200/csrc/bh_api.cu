@@ -19,6 +19,7 @@ struct bh_ctx {
     int64_t n = 0;          // bodies of the last build
     bool built = false;
     bool walked = false;
+    bool no_mid = false;     // the one-kernel build of mid-size sets is not available (cooperative launch refused)
     // bound leapfrog state
     double *pos = nullptr, *vel = nullptr;
     const double *mass = nullptr;
@@ -139,6 +140,24 @@ bh_status do_build(bh_ctx *c, const double *pos, const double *mass, int64_t n, 
         c->built = true;
         c->launches += 1;
         return BH_OK;
+    }
+    if (n <= mid_build_limit(w) && !c->no_mid) {   // one co-resident kernel with grid barriers instead of seventeen launches
+        if (mass_ready) cudaStreamWaitEvent(s, mass_ready, 0);
+        int launched;
+        {
+            Phase p(c, 4);
+            launched = launch_build_mid(w, pos, mass, n, s);
+        }
+        if (launched > 0) {
+            bh_status st1 = cuda_check(c, cudaGetLastError(), "bh_build launch");
+            if (st1 != BH_OK) return st1;
+            c->n = n;
+            c->built = true;
+            c->launches += 1;
+            return BH_OK;
+        }
+        cudaGetLastError();     // cooperative launch not available here: the streaming kernels from now on
+        c->no_mid = true;
     }
     int sort_launches = 0;
     // cleared per build, sized by n (not by max_n): histograms + tickets + look-back words of this n's tiles,

@@ -50,6 +50,7 @@ struct DevState {
     unsigned walk_queue;   // dynamic group counter of the walk (reset by the walk's last producer warp)
     unsigned walk_done;    // producer warps that have left the walk
     unsigned ticket_diag;  // last-block election of the diagnostics reduction (resets itself)
+    unsigned mid_bar[4];   // two grid barriers of the one-kernel build of mid-size sets (arrivals, generation; they reset themselves)
     unsigned long long pair_count;     // broad phase: candidate pairs found (may exceed the caller's capacity)
     unsigned long long agg_counts[3];  // aggregates: connected components, aggregates (size > 1), bad pairs
     unsigned long long stats[kNumStats];   // n_mono, n_direct, interactions, nodes tested, stack spills
@@ -128,6 +129,10 @@ int launch_sort(const Workspace &w, int64_t n, cudaStream_t s);   // result in k
 int sort_tile_items(int64_t n);                                    // keys per thread of the streaming passes for n keys
 // steps a1-a6 in one kernel of one block, n <= kSortTile (bh_small.cu); needs no prior clearing
 void launch_build_small(const Workspace &w, const double *pos, const double *mass, int64_t n, cudaStream_t s);
+// steps a1-a6 in one co-resident kernel with grid barriers, kSortTile < n <= mid_build_limit (bh_mid.cu); needs no prior
+// clearing; returns the launches (1) or -1 if the cooperative launch was refused
+int64_t mid_build_limit(const Workspace &w);
+int launch_build_mid(const Workspace &w, const double *pos, const double *mass, int64_t n, cudaStream_t s);
 void launch_gather(const Workspace &w, const double *pos, const double *mass, int64_t n, cudaStream_t s);
 // (x,y,z,m) in the caller's body order with the identity permutation: input of a direct sum without a tree
 void launch_pack(const Workspace &w, const double *pos, const double *mass, int64_t n, cudaStream_t s);

@@ -51,7 +51,7 @@ def test_other_stream_and_two_contexts():
 
 
 def test_phase_timing_and_launch_count():
-    w = wl.make("c4", 50000)
+    w = wl.make("c4", 200000)     # above one tree tile per SM: the streaming kernels
     ctx = bh.Context(w.n, 16)
     pos, vel, mass = dev(w.pos), dev(w.vel), dev(w.mass)
     bh.bh_set_timing(ctx.ctx, True)
@@ -78,6 +78,13 @@ def test_phase_timing_and_launch_count():
     small.build(dev(w2.pos), dev(w2.mass))
     assert bh.bh_get_launches(small.ctx) - l0 == 1
     small.close()
+    # up to one tree tile (1024 bodies) per SM: one co-resident kernel with grid barriers
+    mid = bh.Context(50000, 16)
+    w3 = wl.make("c4", 50000)
+    l0 = bh.bh_get_launches(mid.ctx)
+    mid.build(dev(w3.pos), dev(w3.mass))
+    assert bh.bh_get_launches(mid.ctx) - l0 == 1
+    mid.close()
     ctx.close()
 
 

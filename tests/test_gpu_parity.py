@@ -81,6 +81,47 @@ def test_accel_counts_exact_and_values_within_tolerance(name, n, C):
     ctx.close()
 
 
+@pytest.mark.parametrize("name,n,C", [("c4", 4097, 16), ("c2", 6000, 16), ("c4", 30000, 1), ("c5", 100000, 32),
+                                      ("c3", 148 * 1024, 16), ("c3", 148 * 1024 + 1, 16)])
+def test_one_kernel_build_of_mid_size_sets_is_bit_exact(name, n, C):
+    # 4096 < n <= 1024 bodies per SM: cube, keys, eight digit passes, gather, tree and monopoles in one co-resident
+    # kernel with grid barriers (bh_mid.cu); one body more and the streaming kernels take over.  Same arrays, bit for bit;
+    # a second build in the same context (the barrier words and the look-back rows are reused) gives them again.
+    w = wl.make(name, n)
+    t = orc.build(w.pos, w.mass, C)
+    ctx = gpu_build(w.pos, w.mass, C)
+    l0 = bh.bh_get_launches(ctx.ctx)
+    ctx.build(dev(w.pos), dev(w.mass))
+    launches = bh.bh_get_launches(ctx.ctx) - l0
+    sms = torch.cuda.get_device_properties(0).multi_processor_count
+    assert launches == (1 if n <= sms * 1024 else 16)     # cube, keys, 8 passes, gather, tree x3, boxes, monopoles
+    assert_tree_equal(ctx, t)
+    ref, nm, nd, _ = orc.accel(t, w.theta, w.eps, w.G, 0, min(t.ngroups, 64))
+    a = ctx.accel(w.theta, w.eps, w.G).cpu().numpy()
+    rows = t.perm[: t.gstart[min(t.ngroups, 64)]]
+    assert relerr(a[rows], ref[rows]).max() <= TOL
+    ctx.close()
+
+
+def test_two_contexts_build_mid_size_sets_at_the_same_time():
+    # two co-resident kernels with their own grid barriers on two streams
+    ws = [wl.make("c3", 20000), wl.make("c4", 50000)]
+    streams = [torch.cuda.Stream(), torch.cuda.Stream()]
+    ctxs, ts = [], []
+    for w, s in zip(ws, streams):
+        ctxs.append(bh.Context(w.n, w.leaf_cap, stream=s))
+        ts.append(orc.build(w.pos, w.mass, w.leaf_cap))
+    bufs = [(dev(w.pos), dev(w.mass)) for w in ws]
+    torch.cuda.synchronize()
+    for rep in range(5):
+        for ctx, (p, m) in zip(ctxs, bufs):
+            ctx.build(p, m)
+    torch.cuda.synchronize()
+    for ctx, t in zip(ctxs, ts):
+        assert_tree_equal(ctx, t)
+        ctx.close()
+
+
 def _tested_nodes_from_lists(t, theta):
     """Nodes the opening criterion is applied to, from the oracle's lists alone: every tested node is accepted
     (it is in a monopole list) or opened (it is a strict ancestor of a list entry, or a leaf whose bodies are in a
