@@ -229,7 +229,7 @@ def test_steppers_with_direct_gravity():
     ctx.close()
 
 
-@pytest.mark.parametrize("n,method", [(3000, 0), (500, 1), (40000, 0)])
+@pytest.mark.parametrize("n,method", [(3000, 0), (500, 1), (40000, 0), (6000, 0), (200000, 0)])
 def test_cuda_graph_steppers_bit_identical(n, method):
     """bh_set_graph: captured / replayed steps equal plain steps bit for bit, across steppers and dt changes."""
     w = wl.make("c4", n)
