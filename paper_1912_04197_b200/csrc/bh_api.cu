@@ -141,7 +141,7 @@ bh_status do_build(bh_ctx *c, const double *pos, const double *mass, int64_t n, 
         c->launches += 1;
         return BH_OK;
     }
-    if (n <= mid_build_limit(w) && !c->no_mid) {   // one co-resident kernel with grid barriers instead of seventeen launches
+    if (n <= mid_build_limit(w) && !c->no_mid) {   // one co-resident kernel with grid barriers instead of sixteen launches and two memsets
         if (mass_ready) cudaStreamWaitEvent(s, mass_ready, 0);
         int launched;
         {

@@ -1,7 +1,7 @@
 // bh_mid.cu — steps a1-a6 for a mid-size body set (one sort tile < n <= one tree tile per SM) in ONE kernel.
 //
 // Between the one-block build (n <= 4096, bh_small.cu) and the sizes where the streaming kernels are bound by
-// work, a build is bound by its seventeen dependent launches: a kernel of a few thousand bodies per SM ends a few
+// work, a build is bound by its sixteen dependent launches (and two memsets): a kernel of a few thousand bodies per SM ends a few
 // microseconds after it starts, and the next one cannot start before (N = 16 384: 135 us for ~15 us of work; the
 // paper's own regime is N <= 10^4 .. 10^5).  Here the same phases — cube, keys + histograms,
 // eight digit passes, gather, tree levels / scan / emission, group boxes, monopoles — run in one co-resident grid
