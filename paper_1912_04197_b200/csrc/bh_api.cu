@@ -179,13 +179,13 @@ bh_status do_build(bh_ctx *c, const double *pos, const double *mass, int64_t n, 
         sort_launches = launch_sort(w, n, s);
     }
     {
-        Phase p(c, 3);
-        if (mass_ready) cudaStreamWaitEvent(s, mass_ready, 0);   // masses copied on another stream
-        launch_gather(w, pos, mass, n, s);
+        Phase p(c, 4);
+        launch_tree(w, n, c->leaf_cap, s);                       // from the sorted keys alone
     }
     {
-        Phase p(c, 4);
-        launch_tree(w, n, c->leaf_cap, s);
+        Phase p(c, 3);
+        if (mass_ready) cudaStreamWaitEvent(s, mass_ready, 0);   // masses copied on another stream
+        launch_gather_boxes(w, pos, mass, n, s);                 // sorted bodies + group boxes, a warp per group
     }
     {
         Phase p(c, 5);
@@ -195,7 +195,7 @@ bh_status do_build(bh_ctx *c, const double *pos, const double *mass, int64_t n, 
     if (st != BH_OK) return st;
     c->n = n;
     c->built = true;
-    c->launches += 2 + sort_launches + 1 + 4 + 1;   // cube, keys, sort passes, gather, tree (3) + boxes, monopoles
+    c->launches += 2 + sort_launches + 3 + 1 + 1;   // cube, keys, sort passes, tree (3), gather + boxes, monopoles
     return BH_OK;
 }
 

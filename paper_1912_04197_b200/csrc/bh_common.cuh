@@ -133,7 +133,8 @@ void launch_build_small(const Workspace &w, const double *pos, const double *mas
 // clearing; returns the launches (1) or -1 if the cooperative launch was refused
 int64_t mid_build_limit(const Workspace &w);
 int launch_build_mid(const Workspace &w, const double *pos, const double *mass, int64_t n, cudaStream_t s);
-void launch_gather(const Workspace &w, const double *pos, const double *mass, int64_t n, cudaStream_t s);
+// sorted bodies AND group boxes in one pass, after launch_tree (which then only builds the tree from the keys)
+void launch_gather_boxes(const Workspace &w, const double *pos, const double *mass, int64_t n, cudaStream_t s);
 // (x,y,z,m) in the caller's body order with the identity permutation: input of a direct sum without a tree
 void launch_pack(const Workspace &w, const double *pos, const double *mass, int64_t n, cudaStream_t s);
 void launch_iperm(const Workspace &w, int64_t n, cudaStream_t s);   // w.iperm from the permutation of the last build

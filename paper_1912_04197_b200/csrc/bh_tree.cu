@@ -24,22 +24,6 @@
 namespace bh {
 
 // ------------------------------------------------------------------------------------------ a4
-__global__ void __launch_bounds__(256) gather_kernel(const double *__restrict__ pos,
-                                                     const double *__restrict__ mass,
-                                                     const unsigned *__restrict__ perm, long long n,
-                                                     double4 *__restrict__ sbody)
-{
-    const long long j = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    if (j >= n) return;
-    const unsigned i = perm[j];
-    double4 b;
-    b.x = __ldg(pos + 3ll * i + 0);
-    b.y = __ldg(pos + 3ll * i + 1);
-    b.z = __ldg(pos + 3ll * i + 2);
-    b.w = __ldg(mass + i);
-    sbody[j] = b;
-}
-
 // inverse permutation (body index -> sorted position), made only when a call needs it (bh_direct_targets): a
 // scattered 4-byte store per body is not worth paying in every build
 __global__ void __launch_bounds__(256) iperm_kernel(const unsigned *__restrict__ perm, long long n,
@@ -59,12 +43,43 @@ __global__ void __launch_bounds__(256) pack_kernel(const double *__restrict__ po
     perm[i] = (unsigned)i;
 }
 
-__global__ void __launch_bounds__(256) group_box_kernel(const DevState *__restrict__ st,
-                                                        const unsigned *__restrict__ gstart,
-                                                        const double4 *__restrict__ sbody,
-                                                        double *__restrict__ gbox)
+// a4 + group boxes in one pass (streaming build): the tree only needs the sorted keys, so the bodies are gathered AFTER
+// it, a warp per walk group (at most 32 bodies: one per lane), and the group's box is reduced from the registers that
+// are being stored — the sorted bodies are not read back for it (32 B per body less than gather + group_box_kernel).
+__global__ void __launch_bounds__(256) gather_box_kernel(const DevState *__restrict__ st, const double *__restrict__ pos,
+                                                         const double *__restrict__ mass,
+                                                         const unsigned *__restrict__ perm,
+                                                         const unsigned *__restrict__ gstart,
+                                                         double4 *__restrict__ sbody, double *__restrict__ gbox)
 {
-    group_boxes(st->n_groups, (blockIdx.x * blockDim.x + threadIdx.x) >> 5, (gridDim.x * blockDim.x) >> 5, gstart, sbody, gbox);
+    const unsigned lane = lane_id();
+    const unsigned ng = st->n_groups;
+    const unsigned nwarps = (gridDim.x * blockDim.x) >> 5;
+    for (unsigned g = (blockIdx.x * blockDim.x + threadIdx.x) >> 5; g < ng; g += nwarps) {
+        const unsigned b = gstart[g], e = gstart[g + 1];
+        const double inf = __longlong_as_double(0x7ff0000000000000ll);
+        double lx = inf, ly = inf, lz = inf, hx = -inf, hy = -inf, hz = -inf;
+        for (unsigned j = b + lane; j < e; j += 32) {           // W <= 32: at most one body per lane; kept general
+            const unsigned i = perm[j];
+            double4 p;
+            p.x = __ldg(pos + 3ll * i + 0);
+            p.y = __ldg(pos + 3ll * i + 1);
+            p.z = __ldg(pos + 3ll * i + 2);
+            p.w = __ldg(mass + i);
+            sbody[j] = p;
+            lx = fmin(lx, p.x); ly = fmin(ly, p.y); lz = fmin(lz, p.z);
+            hx = fmax(hx, p.x); hy = fmax(hy, p.y); hz = fmax(hz, p.z);
+        }
+        // min / max are exact and order-free: the box equals group_boxes' (lanes without a body hold the neutral values)
+        const unsigned long long rlx = warp_min_u64(ordered_bits(lx)), rly = warp_min_u64(ordered_bits(ly)),
+                                 rlz = warp_min_u64(ordered_bits(lz)), rhx = warp_max_u64(ordered_bits(hx)),
+                                 rhy = warp_max_u64(ordered_bits(hy)), rhz = warp_max_u64(ordered_bits(hz));
+        if (lane == 0) {
+            double *q = gbox + 6ull * g;
+            q[0] = from_ordered_bits(rlx); q[1] = from_ordered_bits(rly); q[2] = from_ordered_bits(rlz);
+            q[3] = from_ordered_bits(rhx); q[4] = from_ordered_bits(rhy); q[5] = from_ordered_bits(rhz);
+        }
+    }
 }
 
 // ------------------------------------------------------------------------------------------ a5
@@ -131,12 +146,6 @@ __global__ void unpack_mask_kernel(const unsigned *__restrict__ node_meta, const
 }
 
 // ------------------------------------------------------------------------------------------ launchers
-void launch_gather(const Workspace &w, const double *pos, const double *mass, int64_t n, cudaStream_t s)
-{
-    int blocks = (int)((n + 255) / 256);
-    gather_kernel<<<blocks, 256, 0, s>>>(pos, mass, w.idx[0], n, w.sbody);
-}
-
 void launch_iperm(const Workspace &w, int64_t n, cudaStream_t s)
 {
     iperm_kernel<<<(int)((n + 255) / 256), 256, 0, s>>>(w.idx[0], n, w.iperm);
@@ -155,7 +164,15 @@ void launch_tree(const Workspace &w, int64_t n, int leaf_cap, cudaStream_t s)
     tree_scan_kernel<<<1, (kLevels + 1) * 32, 0, s>>>(w.tile_lvl, ntiles, w.st, w.node_cap, w.gstart, (unsigned)n);
     tree_emit_kernel<<<ntiles, 256, 0, s>>>(w.key[0], n, w.dlev, w.tile_lvl, ntiles, w.st, w.node_cap, w.nlevel,
                                             w.nbegin, w.nfirst, w.nparent, w.node_meta, w.gstart);
-    group_box_kernel<<<w.sms * 4, 256, 0, s>>>(w.st, w.gstart, w.sbody, w.gbox);
+}
+
+// sorted bodies + group boxes, after launch_tree (needs the group starts)
+void launch_gather_boxes(const Workspace &w, const double *pos, const double *mass, int64_t n, cudaStream_t s)
+{
+    int64_t want = (n + 7) / 8;                   // about a warp per 32 bodies, eight warps per block
+    int blocks = (int)(want < (int64_t)w.sms * 32 ? want : (int64_t)w.sms * 32);
+    if (blocks < 1) blocks = 1;
+    gather_box_kernel<<<blocks, 256, 0, s>>>(w.st, pos, mass, w.idx[0], w.gstart, w.sbody, w.gbox);
 }
 
 void launch_monopoles(const Workspace &w, int64_t n, cudaStream_t s)
