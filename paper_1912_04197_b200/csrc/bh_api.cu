@@ -176,8 +176,9 @@ bh_status do_build(bh_ctx *c, const double *pos, const double *mass, int64_t n, 
     }
     {
         Phase p(c, 2);
-        sort_launches = launch_sort(w, n, s);
+        sort_launches = launch_sort(w, pos, n, s);
     }
+    if (sort_launches < 0) return fail(c, BH_ERR_CUDA, "bh_build: the sort's fallback kernel could not be launched");
     {
         Phase p(c, 4);
         launch_tree(w, n, c->leaf_cap, s);                       // from the sorted keys alone
@@ -195,7 +196,7 @@ bh_status do_build(bh_ctx *c, const double *pos, const double *mass, int64_t n, 
     if (st != BH_OK) return st;
     c->n = n;
     c->built = true;
-    c->launches += 2 + sort_launches + 3 + 1 + 1;   // cube, keys, sort passes, tree (3), gather + boxes, monopoles
+    c->launches += 2 + sort_launches + 3 + 1 + 1;   // cube, keys, sort (5 passes + repair + fallback), tree (3), gather + boxes, monopoles
     return BH_OK;
 }
 

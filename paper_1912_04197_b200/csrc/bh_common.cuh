@@ -31,7 +31,8 @@ constexpr int kTreeTile = 1024;           // bodies per block in the tree kernel
 constexpr int kDiagBlocks = 592;          // diagnostics: a FIXED number of partial sums, whatever the device, so that the reduction order is fixed
 constexpr int kStackSlab = 22 * 256;      // walk: spill entries (8 bytes each) per producer warp: <= 32 x 7 ranges per level; overflow sets kStatStack
 
-enum StatusBits : int { kStatNonFinite = 1, kStatCapacity = 2, kStatStack = 4, kStatRange = 8, kStatBpStack = 16 };
+enum StatusBits : int { kStatNonFinite = 1, kStatCapacity = 2, kStatStack = 4, kStatRange = 8, kStatBpStack = 16,
+                        kStatLongRun = 32 /* internal to the one-kernel sort: not an error, cleared by it */ };
 constexpr int kMaxExtentExp = 300;        // largest extent must lie in [2^-300, 2^300] (or be 0): bh.h preconditions
 constexpr int kNumStats = BH_NUM_STATS;
 
@@ -125,7 +126,7 @@ Workspace carve(char *base, int64_t max_n, int leaf_cap);
 // launchers (each enqueues on `s`)
 void launch_cube(const Workspace &w, const double *pos, int64_t n, cudaStream_t s);
 void launch_keys(const Workspace &w, const double *pos, int64_t n, cudaStream_t s);
-int launch_sort(const Workspace &w, int64_t n, cudaStream_t s);   // result in key[0]/idx[0]; returns the launches
+int launch_sort(const Workspace &w, const double *pos, int64_t n, cudaStream_t s);   // result in key[0]/idx[0]; returns the launches
 int sort_tile_items(int64_t n);                                    // keys per thread of the streaming passes for n keys
 // steps a1-a6 in one kernel of one block, n <= kSortTile (bh_small.cu); needs no prior clearing
 void launch_build_small(const Workspace &w, const double *pos, const double *mass, int64_t n, cudaStream_t s);

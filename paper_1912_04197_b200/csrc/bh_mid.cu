@@ -18,36 +18,13 @@
 #include "bh_keys.cuh"
 #include "bh_sort.cuh"
 #include "bh_tree.cuh"
+#include "bh_grid.cuh"
 
 namespace bh {
 
 constexpr int kMidThreads = kSortThreads;   // 256: the sort tile's block size
 constexpr int kMidItems = 8;                // 2048-key sort tiles, as the streaming passes below kSortSmallTileBelow keys (1024- and 512-key
                                             // tiles change a pass by < 0.5 us: a pass is 3 us of tile chain + 2.3 us of barrier)
-
-// Barrier of the first `nblocks` blocks of the (co-resident) grid; bar[0] counts arrivals, bar[1] is the generation.
-// Arrival is an acq_rel atomic (it publishes the block's writes and, for the last block, acquires everybody else's),
-// the last block opens the barrier with a release, the others poll the generation with ld.acquire — on sm_100 an
-// acquire load is LDG.STRONG.GPU + CCTL.IVALL, i.e. it also drops the SM's L1, which is what makes the plain loads
-// of the next phase safe.
-__device__ __forceinline__ void grid_barrier(unsigned *bar, unsigned nblocks)
-{
-    __syncthreads();
-    if (threadIdx.x == 0) {
-        unsigned gen, old;
-        asm volatile("ld.relaxed.gpu.global.u32 %0, [%1];" : "=r"(gen) : "l"(bar + 1) : "memory");
-        asm volatile("atom.acq_rel.gpu.global.add.u32 %0, [%1], 1;" : "=r"(old) : "l"(bar) : "memory");
-        if (old == nblocks - 1u) {
-            asm volatile("st.relaxed.gpu.global.u32 [%0], %1;" ::"l"(bar), "r"(0u) : "memory");
-            asm volatile("red.release.gpu.global.add.u32 [%0], 1;" ::"l"(bar + 1) : "memory");
-        }
-        unsigned now;
-        do {
-            asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(now) : "l"(bar + 1) : "memory");
-        } while (now == gen);
-    }
-    __syncthreads();
-}
 
 // One thread-block CLUSTER (the whole grid: 8 blocks): the hardware barrier of the cluster.  Its arrive has release,
 // its wait acquire semantics (SASS: MEMBAR.ALL.GPU, UCGABAR_ARV / UCGABAR_WAIT, CCTL.IVALL), so it orders global memory

@@ -4,7 +4,9 @@
 // the tile's global digit offsets with a decoupled look-back over the tiles before it, and scatters
 // through shared memory so that the global writes are runs of consecutive addresses per digit.
 // The global digit histograms of all passes were accumulated by keys_kernel.
+#include "bh_keys.cuh"
 #include "bh_sort.cuh"
+#include "bh_grid.cuh"
 
 namespace bh {
 
@@ -36,13 +38,172 @@ sort_pass_kernel(const unsigned long long *__restrict__ kin, const unsigned *__r
                                        whist, sbase, stmp);
 }
 
+// ------------------------------------------------------------------------------------------ partial-key sort
+// Only the FIVE high digits (the top 39 key bits) go through digit passes.  Stable passes leave every run of keys with
+// equal top bits in index order; a repair pass then ranks each key inside its run by (low 24 bits, position) and writes
+// it to its final place.  Runs are short where bodies are distinct points (longest run 6 at configs[3], 2 at
+// configs[4]: they are the bodies of one level-13 cell), so the repair is one more streaming pass without ranking
+// machinery.  A run longer than kRunMax (coincident bodies share all 63 bits) raises a flag instead, and the last
+// kernel of the sort — a co-resident grid that leaves at once when the flag is down — then sorts from scratch with all
+// eight digits (grid barriers between the passes).  Either way the result is the stable order by the full key: the
+// same permutation, bit for bit.  Five passes end in buffer 1, the repair moves the data to buffer 0.
+constexpr int kHighFirst = 3;                // first digit of the partial sort: digits 3..7 = key bits 24..63
+constexpr int kLowBits = kHighFirst * kRadixBits;
+constexpr unsigned kRunMax = 64;             // longest run the quadratic repair takes
+constexpr int kRepairPer = 4;                // keys per thread of the repair pass, their loads issued together
+
+__global__ void __launch_bounds__(kSortThreads)
+sort_repair_kernel(const unsigned long long *__restrict__ kin, const unsigned *__restrict__ vin,
+                   unsigned long long *__restrict__ kout, unsigned *__restrict__ vout, long long n, DevState *st)
+{
+    const long long j0 = (long long)blockIdx.x * (kSortThreads * kRepairPer) + threadIdx.x;
+    unsigned long long k[kRepairPer], kl[kRepairPer], kr[kRepairPer];
+    unsigned v[kRepairPer];
+#pragma unroll
+    for (int u = 0; u < kRepairPer; ++u) {
+        const long long j = j0 + (long long)u * kSortThreads;
+        const bool in = j < n;
+        k[u] = in ? kin[j] : 0ull;
+        v[u] = in ? vin[j] : 0u;
+        kl[u] = (in && j > 0) ? kin[j - 1] : ~0ull;          // ~0 >> 24 is no valid top: keys have 63 bits
+        kr[u] = (in && j + 1 < n) ? kin[j + 1] : ~0ull;
+    }
+    bool too_long = false;
+#pragma unroll
+    for (int u = 0; u < kRepairPer; ++u) {
+        const long long j = j0 + (long long)u * kSortThreads;
+        if (j >= n) continue;
+        const unsigned long long top = k[u] >> kLowBits;
+        if ((kl[u] >> kLowBits) != top && (kr[u] >> kLowBits) != top) {   // alone in its run (the usual case): it stays
+            kout[j] = k[u];
+            vout[j] = v[u];
+            continue;
+        }
+        long long lo = j, hi = j + 1;        // the run is [lo, hi)
+        while (lo > 0 && j - lo <= (long long)kRunMax && (kin[lo - 1] >> kLowBits) == top) --lo;
+        while (hi < n && hi - j <= (long long)kRunMax && (kin[hi] >> kLowBits) == top) ++hi;
+        if (hi - lo > (long long)kRunMax) {
+            too_long = true;
+            continue;
+        }
+        long long r = lo;
+        for (long long i = lo; i < hi; ++i) {
+            const unsigned long long ki = kin[i];
+            r += (ki < k[u]) || (ki == k[u] && i < j);
+        }
+        kout[r] = k[u];
+        vout[r] = v[u];
+    }
+    if (too_long) atomicOr(&st->status, (int)kStatLongRun);
+}
+
+// The full eight-digit sort in one co-resident kernel; does nothing unless the repair pass raised the flag.
+template <int ITEMS>
+__global__ void __launch_bounds__(kSortThreads, ITEMS == 16 ? 3 : 5)
+sort_fallback_kernel(Workspace w, const double *__restrict__ pos, long long n, int tiles)
+{
+    DevState *st = w.st;
+    if (!(*reinterpret_cast<volatile int *>(&st->status) & (int)kStatLongRun)) return;   // uniform over the grid
+    __shared__ unsigned long long skey[(kSortThreads * ITEMS)];
+    __shared__ unsigned whist[kSortThreads / 32][kRadix];
+    __shared__ unsigned sbase[kRadix];
+    __shared__ unsigned stmp[8];
+    unsigned *bar = st->mid_bar;
+    const unsigned tid = threadIdx.x;
+    const long long gtid = (long long)blockIdx.x * kSortThreads + tid, gthreads = (long long)gridDim.x * kSortThreads;
+    {   // the keys again (buffer 0 holds a partial result) and clean look-back rows
+        const double lx = st->lo[0], ly = st->lo[1], lz = st->lo[2], sc = st->scale;
+        for (long long i = gtid; i < n; i += gthreads)
+            w.key[0][i] = morton_key(__ldg(pos + 3 * i), __ldg(pos + 3 * i + 1), __ldg(pos + 3 * i + 2), lx, ly, lz, sc);
+        for (long long i = gtid; i < (long long)kSortPasses * tiles * kRadix; i += gthreads) w.lookback[i] = 0u;
+    }
+    grid_barrier(bar, gridDim.x);
+    int a = 0;
+    for (int p = 0; p < kSortPasses; ++p) {
+        // Tiles in rounds: block b takes tiles b, b + grid, ...  All blocks are resident and a round's tiles start
+        // together, so the tiles a look-back waits for are running or done.
+        unsigned *lb = w.lookback + (size_t)p * tiles * kRadix;
+        const int b = a ^ 1;
+        for (unsigned tile = blockIdx.x; tile < (unsigned)tiles; tile += gridDim.x) {
+            __syncthreads();
+#pragma unroll
+            for (int q = 0; q < kSortThreads / 32; ++q) whist[q][tid] = 0u;
+            __syncthreads();
+            const long long base = (long long)tile * (kSortThreads * ITEMS);
+            const long long rem = n - base;
+            const unsigned nvalid = rem >= kSortThreads * ITEMS ? (unsigned)(kSortThreads * ITEMS) : (unsigned)rem;
+            if (p == 0) sort_tile<true, ITEMS, false>(w.key[a], w.idx[a], w.key[b], w.idx[b], base, nvalid, tile, 0, w.hist, lb, skey, whist, sbase, stmp);
+            else sort_tile<false, ITEMS, false>(w.key[a], w.idx[a], w.key[b], w.idx[b], base, nvalid, tile, p * kRadixBits, w.hist + p * kRadix, lb, skey, whist, sbase, stmp);
+        }
+        a ^= 1;
+        grid_barrier(bar, gridDim.x);
+    }
+    // the flag has done its work; it is not an error
+    if (gtid == 0) atomicAnd(&st->status, ~(int)kStatLongRun);
+}
+
 // keys per tile of the streaming passes for n keys
 int sort_tile_items(int64_t n) { return n < kSortSmallTileBelow ? 8 : 16; }
 
-int launch_sort(const Workspace &w, int64_t n, cudaStream_t s)
+template <int ITEMS>
+static bool launch_sort_fallback(const Workspace &w, const double *pos, int64_t n, int tiles, cudaStream_t s)
+{
+    static int per_sm = -1;
+    if (per_sm < 0) {
+        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, sort_fallback_kernel<ITEMS>, kSortThreads, 0) != cudaSuccess) per_sm = 0;
+        cudaGetLastError();
+    }
+    if (per_sm < 1) return false;
+    int blocks = per_sm * w.sms;
+    if (blocks > tiles) blocks = tiles;
+    Workspace wc = w;
+    long long nn = n;
+    void *args[] = {&wc, &pos, &nn, &tiles};
+    if (cudaLaunchCooperativeKernel((const void *)sort_fallback_kernel<ITEMS>, dim3(blocks), dim3(kSortThreads), args, 0, s) != cudaSuccess) {
+        cudaGetLastError();
+        return false;
+    }
+    return true;
+}
+
+template <int ITEMS>
+static void launch_sort_pass(const Workspace &w, int64_t n, int tiles, int p, int a, bool first, cudaStream_t s)
+{
+    const int b = a ^ 1;
+    unsigned *lb = w.lookback + (size_t)p * tiles * kRadix;   // [pass][tiles of this n][256]: cleared per build
+    if (first)
+        sort_pass_kernel<true, ITEMS><<<tiles, kSortThreads, 0, s>>>(w.key[a], w.idx[a], w.key[b], w.idx[b], n, p * kRadixBits,
+                                                                     w.hist + p * kRadix, lb, w.sort_ticket + p);
+    else
+        sort_pass_kernel<false, ITEMS><<<tiles, kSortThreads, 0, s>>>(w.key[a], w.idx[a], w.key[b], w.idx[b], n, p * kRadixBits,
+                                                                      w.hist + p * kRadix, lb, w.sort_ticket + p);
+}
+
+// pos: the caller's positions (the fallback recomputes the keys from them)
+int launch_sort(const Workspace &w, const double *pos, int64_t n, cudaStream_t s)
 {
     const int items = sort_tile_items(n);
     const int tiles = (int)((n + kSortThreads * items - 1) / (kSortThreads * items));
+    // the partial-key sort needs its fallback kernel, a cooperative launch: asked once
+    static int partial = -1;
+    if (partial < 0) {
+        int dev = 0, coop = 0;
+        cudaGetDevice(&dev);
+        cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev);
+        partial = coop ? 1 : 0;
+        cudaGetLastError();
+    }
+    if (partial) {
+        int a = 0;
+        for (int p = kHighFirst; p < kSortPasses; ++p, a ^= 1) {
+            if (items == 8) launch_sort_pass<8>(w, n, tiles, p, a, p == kHighFirst, s);
+            else launch_sort_pass<16>(w, n, tiles, p, a, p == kHighFirst, s);
+        }
+        const int rblocks = (int)((n + kSortThreads * kRepairPer - 1) / (kSortThreads * kRepairPer));
+        sort_repair_kernel<<<rblocks, kSortThreads, 0, s>>>(w.key[a], w.idx[a], w.key[a ^ 1], w.idx[a ^ 1], n, w.st);
+        const bool ok = items == 8 ? launch_sort_fallback<8>(w, pos, n, tiles, s) : launch_sort_fallback<16>(w, pos, n, tiles, s);
+        return ok ? (kSortPasses - kHighFirst) + 2 : -1;     // -1: the caller reports a CUDA error
+    }
     for (int p = 0; p < kSortPasses; ++p) {
         const int a = p & 1, b = a ^ 1;
         unsigned *lb = w.lookback + (size_t)p * tiles * kRadix;   // [pass][tiles of this n][256]: cleared per build
