@@ -154,39 +154,55 @@ __global__ void __launch_bounds__(kMidThreads) build_mid_kernel(Workspace w, con
         phase_barrier<CLUSTER>(bar);
     }
 
-    // ---- a3: eight digit passes; block b sorts tiles b, b + grid, ... in ascending order (the look-back of a tile only
-    //      waits for lower tiles, and every block is resident)
+    // ---- a3: the sort, as above 1024 bodies per SM (bh_sort.cu): digit passes over the five high digits, a repair pass that
+    //      orders the runs of equal top bits, and — a uniform branch here, not a kernel — all eight digits from scratch if
+    //      a run was too long.  Block b sorts tiles b, b + grid, ... in ascending order (the look-back of a tile only waits
+    //      for lower tiles, and every block is resident).
     {
         unsigned long long *skey = reinterpret_cast<unsigned long long *>(smem);                          // [256 * 8]
         unsigned(*whist)[kRadix] = reinterpret_cast<unsigned(*)[kRadix]>(skey + kMidThreads * kMidItems);   // [8][256]
         unsigned *sbase = &whist[kMidThreads / 32][0];                                                    // [256]
         const unsigned sorters = (unsigned)sort_tiles < gridDim.x ? (unsigned)sort_tiles : gridDim.x;   // blocks that own tiles
-        for (int p = 0; p < kSortPasses && (CLUSTER || blockIdx.x < sorters); ++p) {
-            const int a = p & 1, b = a ^ 1;
-            unsigned *lb = w.lookback + (size_t)p * sort_tiles * kRadix;
-            for (int tile = blockIdx.x; tile < sort_tiles; tile += gridDim.x) {
+        // digits p0 .. 7 starting from buffer 0 (values = positions in the first of them)
+        auto digit_passes = [&](int p0) {
+            int a = 0;
+            for (int p = p0; p < kSortPasses && (CLUSTER || blockIdx.x < sorters); ++p, a ^= 1) {
+                const int b = a ^ 1;
+                unsigned *lb = w.lookback + (size_t)p * sort_tiles * kRadix;
+                for (int tile = blockIdx.x; tile < sort_tiles; tile += gridDim.x) {
 #pragma unroll
-                for (int q = 0; q < kMidThreads / 32; ++q) whist[q][tid] = 0u;
-                __syncthreads();
-                const long long base = (long long)tile * (kMidThreads * kMidItems);
-                const long long rem = n - base;
-                const bool full = rem >= kMidThreads * kMidItems;
-                const unsigned nvalid = full ? (unsigned)(kMidThreads * kMidItems) : (unsigned)rem;
-                if (p == 0) {
-                    if (full) sort_tile<true, kMidItems, true>(w.key[a], w.idx[a], w.key[b], w.idx[b], base, nvalid, tile, p * kRadixBits, w.hist + p * kRadix, lb, skey, whist, sbase, stmp);
-                    else sort_tile<true, kMidItems, false>(w.key[a], w.idx[a], w.key[b], w.idx[b], base, nvalid, tile, p * kRadixBits, w.hist + p * kRadix, lb, skey, whist, sbase, stmp);
-                } else {
-                    if (full) sort_tile<false, kMidItems, true>(w.key[a], w.idx[a], w.key[b], w.idx[b], base, nvalid, tile, p * kRadixBits, w.hist + p * kRadix, lb, skey, whist, sbase, stmp);
+                    for (int q = 0; q < kMidThreads / 32; ++q) whist[q][tid] = 0u;
+                    __syncthreads();
+                    const long long base = (long long)tile * (kMidThreads * kMidItems);
+                    const long long rem = n - base;
+                    const unsigned nvalid = rem >= kMidThreads * kMidItems ? (unsigned)(kMidThreads * kMidItems) : (unsigned)rem;
+                    if (p == p0) sort_tile<true, kMidItems, false>(w.key[a], w.idx[a], w.key[b], w.idx[b], base, nvalid, tile, p * kRadixBits, w.hist + p * kRadix, lb, skey, whist, sbase, stmp);
                     else sort_tile<false, kMidItems, false>(w.key[a], w.idx[a], w.key[b], w.idx[b], base, nvalid, tile, p * kRadixBits, w.hist + p * kRadix, lb, skey, whist, sbase, stmp);
+                    __syncthreads();
                 }
-                __syncthreads();
+                if (p + 1 < kSortPasses) {     // between passes: the whole cluster, or the sorting blocks of the grid only
+                    if constexpr (CLUSTER) cluster_barrier();
+                    else grid_barrier(bar + 2, sorters);
+                }
             }
-            if (p + 1 < kSortPasses) {     // between passes: the whole cluster, or the sorting blocks of the grid only
-                if constexpr (CLUSTER) cluster_barrier();
-                else grid_barrier(bar + 2, sorters);
-            }
+            phase_barrier<CLUSTER>(bar);       // after the last pass: everybody
+        };
+        digit_passes(kHighFirst);              // five passes: the result is in buffer 1
+        bool too_long = false;
+        for (long long j0 = (long long)blockIdx.x * (kMidThreads * kRepairPer) + tid; j0 < n; j0 += (long long)gridDim.x * (kMidThreads * kRepairPer))
+            too_long |= repair_keys(w.key[1], w.idx[1], w.key[0], w.idx[0], n, j0);
+        if (too_long) atomicOr(&st->status, (int)kStatLongRun);
+        phase_barrier<CLUSTER>(bar);
+        if (*reinterpret_cast<volatile int *>(&st->status) & (int)kStatLongRun) {   // uniform over the grid
+            const double lx = st->lo[0], ly = st->lo[1], lz = st->lo[2], sc = st->scale;
+            for (int i = gtid; i < n; i += gthreads)
+                w.key[0][i] = morton_key(__ldg(pos + 3 * (long long)i), __ldg(pos + 3 * (long long)i + 1),
+                                         __ldg(pos + 3 * (long long)i + 2), lx, ly, lz, sc);
+            for (long long k = gtid; k < (long long)kSortPasses * sort_tiles * kRadix; k += gthreads) w.lookback[k] = 0u;
+            phase_barrier<CLUSTER>(bar);
+            digit_passes(0);                   // eight passes: the result is in buffer 0
+            if (gtid == 0) atomicAnd(&st->status, ~(int)kStatLongRun);   // the flag has done its work; it is not an error
         }
-        phase_barrier<CLUSTER>(bar);                                  // after the last pass: everybody
     }
 
     // ---- a4: sorted bodies

@@ -47,54 +47,12 @@ sort_pass_kernel(const unsigned long long *__restrict__ kin, const unsigned *__r
 // kernel of the sort — a co-resident grid that leaves at once when the flag is down — then sorts from scratch with all
 // eight digits (grid barriers between the passes).  Either way the result is the stable order by the full key: the
 // same permutation, bit for bit.  Five passes end in buffer 1, the repair moves the data to buffer 0.
-constexpr int kHighFirst = 3;                // first digit of the partial sort: digits 3..7 = key bits 24..63
-constexpr int kLowBits = kHighFirst * kRadixBits;
-constexpr unsigned kRunMax = 64;             // longest run the quadratic repair takes
-constexpr int kRepairPer = 4;                // keys per thread of the repair pass, their loads issued together
-
 __global__ void __launch_bounds__(kSortThreads)
 sort_repair_kernel(const unsigned long long *__restrict__ kin, const unsigned *__restrict__ vin,
                    unsigned long long *__restrict__ kout, unsigned *__restrict__ vout, long long n, DevState *st)
 {
-    const long long j0 = (long long)blockIdx.x * (kSortThreads * kRepairPer) + threadIdx.x;
-    unsigned long long k[kRepairPer], kl[kRepairPer], kr[kRepairPer];
-    unsigned v[kRepairPer];
-#pragma unroll
-    for (int u = 0; u < kRepairPer; ++u) {
-        const long long j = j0 + (long long)u * kSortThreads;
-        const bool in = j < n;
-        k[u] = in ? kin[j] : 0ull;
-        v[u] = in ? vin[j] : 0u;
-        kl[u] = (in && j > 0) ? kin[j - 1] : ~0ull;          // ~0 >> 24 is no valid top: keys have 63 bits
-        kr[u] = (in && j + 1 < n) ? kin[j + 1] : ~0ull;
-    }
-    bool too_long = false;
-#pragma unroll
-    for (int u = 0; u < kRepairPer; ++u) {
-        const long long j = j0 + (long long)u * kSortThreads;
-        if (j >= n) continue;
-        const unsigned long long top = k[u] >> kLowBits;
-        if ((kl[u] >> kLowBits) != top && (kr[u] >> kLowBits) != top) {   // alone in its run (the usual case): it stays
-            kout[j] = k[u];
-            vout[j] = v[u];
-            continue;
-        }
-        long long lo = j, hi = j + 1;        // the run is [lo, hi)
-        while (lo > 0 && j - lo <= (long long)kRunMax && (kin[lo - 1] >> kLowBits) == top) --lo;
-        while (hi < n && hi - j <= (long long)kRunMax && (kin[hi] >> kLowBits) == top) ++hi;
-        if (hi - lo > (long long)kRunMax) {
-            too_long = true;
-            continue;
-        }
-        long long r = lo;
-        for (long long i = lo; i < hi; ++i) {
-            const unsigned long long ki = kin[i];
-            r += (ki < k[u]) || (ki == k[u] && i < j);
-        }
-        kout[r] = k[u];
-        vout[r] = v[u];
-    }
-    if (too_long) atomicOr(&st->status, (int)kStatLongRun);
+    if (repair_keys(kin, vin, kout, vout, n, (long long)blockIdx.x * (kSortThreads * kRepairPer) + threadIdx.x))
+        atomicOr(&st->status, (int)kStatLongRun);
 }
 
 // The full eight-digit sort in one co-resident kernel; does nothing unless the repair pass raised the flag.

@@ -295,4 +295,55 @@ __device__ __forceinline__ void sort_tile(const unsigned long long *kin, const u
     }
 }
 
+// ---- the repair pass of the partial-key sort (bh_sort.cu; also a phase of the one-kernel build, bh_mid.cu) ----
+constexpr int kHighFirst = 3;                // first digit of the partial sort: digits 3..7 = key bits 24..63
+constexpr int kLowBits = kHighFirst * kRadixBits;
+constexpr unsigned kRunMax = 64;             // longest run the quadratic repair takes
+constexpr int kRepairPer = 4;                // keys per thread of the repair pass, their loads issued together
+
+// kRepairPer keys j0, j0 + 256, ... of an array that is stably sorted by its top 39 bits: each goes to its place in the
+// order by the full key (ties by position).  Returns true if a run was longer than kRunMax (nothing is written for it).
+__device__ __forceinline__ bool repair_keys(const unsigned long long *kin, const unsigned *vin, unsigned long long *kout,
+                                            unsigned *vout, long long n, long long j0)
+{
+    unsigned long long k[kRepairPer], kl[kRepairPer], kr[kRepairPer];
+    unsigned v[kRepairPer];
+#pragma unroll
+    for (int u = 0; u < kRepairPer; ++u) {
+        const long long j = j0 + (long long)u * kSortThreads;
+        const bool in = j < n;
+        k[u] = in ? kin[j] : 0ull;
+        v[u] = in ? vin[j] : 0u;
+        kl[u] = (in && j > 0) ? kin[j - 1] : ~0ull;          // ~0 >> 24 is no valid top: keys have 63 bits
+        kr[u] = (in && j + 1 < n) ? kin[j + 1] : ~0ull;
+    }
+    bool too_long = false;
+#pragma unroll
+    for (int u = 0; u < kRepairPer; ++u) {
+        const long long j = j0 + (long long)u * kSortThreads;
+        if (j >= n) continue;
+        const unsigned long long top = k[u] >> kLowBits;
+        if ((kl[u] >> kLowBits) != top && (kr[u] >> kLowBits) != top) {   // alone in its run (the usual case): it stays
+            kout[j] = k[u];
+            vout[j] = v[u];
+            continue;
+        }
+        long long lo = j, hi = j + 1;        // the run is [lo, hi)
+        while (lo > 0 && j - lo <= (long long)kRunMax && (kin[lo - 1] >> kLowBits) == top) --lo;
+        while (hi < n && hi - j <= (long long)kRunMax && (kin[hi] >> kLowBits) == top) ++hi;
+        if (hi - lo > (long long)kRunMax) {
+            too_long = true;
+            continue;
+        }
+        long long r = lo;
+        for (long long i = lo; i < hi; ++i) {
+            const unsigned long long ki = kin[i];
+            r += (ki < k[u]) || (ki == k[u] && i < j);
+        }
+        kout[r] = k[u];
+        vout[r] = v[u];
+    }
+    return too_long;
+}
+
 }  // namespace bh

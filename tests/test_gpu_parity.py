@@ -103,9 +103,9 @@ def test_one_kernel_build_of_mid_size_sets_is_bit_exact(name, n, C):
     ctx.close()
 
 
-@pytest.mark.parametrize("n,dup", [(200000, 0), (200000, 40), (200000, 300), (600000, 300)])
+@pytest.mark.parametrize("n,dup", [(200000, 0), (200000, 40), (200000, 300), (600000, 300), (6000, 100), (20000, 40), (20000, 300)])
 def test_partial_key_sort_and_its_fallback(n, dup):
-    # Above 1024 bodies per SM the sort passes only take the five high digits and a repair pass orders the runs of equal
+    # Above 4096 bodies (one-kernel build and streaming sort alike) the sort passes only take the five high digits and a repair pass orders the runs of equal
     # top bits; `dup` coincident bodies share all 63 key bits: 40 are within the repair's reach (run <= 64), 300 raise the
     # flag and the co-resident fallback kernel sorts from scratch with eight digits.  Same permutation either way, and
     # the flag is not an error: the next synchronising call reports success.
