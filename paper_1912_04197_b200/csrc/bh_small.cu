@@ -121,16 +121,52 @@ __global__ void __launch_bounds__(kSmallThreads) build_small_kernel(Workspace w,
             if (idx < n) k[i] = morton_key(__ldg(pos + 3 * idx), __ldg(pos + 3 * idx + 1), __ldg(pos + 3 * idx + 2), lx, ly, lz, sc);
             v[i] = (unsigned)idx;
         }
-        block_radix_sort<ITEMS, kSmallThreads>(k, v, skey, whist, stoff, stmp);
+        // the partial-key sort of bh_sort.cu inside the block: five passes over the high digits, then every key is ranked
+        // within its run of equal top bits (the keys lie in shared memory for that); a run longer than kRunMax makes
+        // the block sort again with all eight digits (uniform branch)
+        block_radix_sort<ITEMS, kSmallThreads>(k, v, skey, whist, stoff, stmp, kHighFirst);
+        int place[ITEMS];
+        bool too_long = false;
+#pragma unroll
+        for (int i = 0; i < ITEMS; ++i) skey[warp * (32 * ITEMS) + i * 32 + lane] = k[i];     // padding keys ~0 sort last
+        __syncthreads();
+#pragma unroll
+        for (int i = 0; i < ITEMS; ++i) {
+            const int j = warp * (32 * ITEMS) + i * 32 + lane;
+            place[i] = j;
+            if (j >= n) continue;
+            const unsigned long long top = k[i] >> kLowBits;
+            int lo = j, hi = j + 1;
+            while (lo > 0 && j - lo <= (int)kRunMax && (skey[lo - 1] >> kLowBits) == top) --lo;
+            while (hi < n && hi - j <= (int)kRunMax && (skey[hi] >> kLowBits) == top) ++hi;
+            if (hi - lo > (int)kRunMax) {
+                too_long = true;
+                continue;
+            }
+            int r = lo;
+            for (int q = lo; q < hi; ++q) r += (skey[q] < k[i]) || (skey[q] == k[i] && q < j);
+            place[i] = r;
+        }
+        if (__syncthreads_or(too_long)) {
+#pragma unroll
+            for (int i = 0; i < ITEMS; ++i) {
+                const int idx = warp * (32 * ITEMS) + i * 32 + lane;
+                k[i] = ~0ull;
+                if (idx < n) k[i] = morton_key(__ldg(pos + 3 * idx), __ldg(pos + 3 * idx + 1), __ldg(pos + 3 * idx + 2), lx, ly, lz, sc);
+                v[i] = (unsigned)idx;
+                place[i] = idx;
+            }
+            block_radix_sort<ITEMS, kSmallThreads>(k, v, skey, whist, stoff, stmp);
+        }
         // ---- a4: sorted keys, permutation, sorted bodies
 #pragma unroll
         for (int i = 0; i < ITEMS; ++i) {
             const int j = warp * (32 * ITEMS) + i * 32 + lane;
             if (j < n) {
                 const unsigned b = v[i];
-                w.key[0][j] = k[i];
-                w.idx[0][j] = b;
-                w.sbody[j] = make_double4(__ldg(pos + 3 * b), __ldg(pos + 3 * b + 1), __ldg(pos + 3 * b + 2), __ldg(mass + b));
+                w.key[0][place[i]] = k[i];
+                w.idx[0][place[i]] = b;
+                w.sbody[place[i]] = make_double4(__ldg(pos + 3 * b), __ldg(pos + 3 * b + 1), __ldg(pos + 3 * b + 2), __ldg(mass + b));
             }
         }
         __syncthreads();

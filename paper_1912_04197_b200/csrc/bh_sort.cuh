@@ -89,14 +89,14 @@ __device__ __forceinline__ unsigned warp_rank(unsigned *cnt, unsigned d, bool va
 template <int ITEMS, int THREADS>
 __device__ __forceinline__ void block_radix_sort(unsigned long long (&k)[ITEMS], unsigned (&v)[ITEMS],
                                                  unsigned long long *skey, unsigned (*whist)[kRadix], unsigned *stoff,
-                                                 unsigned *stmp)
+                                                 unsigned *stmp, int p0 = 0)
 {
     constexpr int kWarps = THREADS / 32;
     const unsigned tid = threadIdx.x, lane = tid & 31u, warp = tid >> 5;
     const unsigned lt = (1u << lane) - 1u;
     unsigned pos[ITEMS];
 #pragma unroll 1
-    for (int p = 0; p < kSortPasses; ++p) {
+    for (int p = p0; p < kSortPasses; ++p) {     // digits p0 .. 7 (p0 = 3: the partial-key sort, see repair_keys)
         const int shift = p * kRadixBits;
         for (int q = tid; q < kWarps * kRadix; q += THREADS) (&whist[0][0])[q] = 0u;
         __syncthreads();
