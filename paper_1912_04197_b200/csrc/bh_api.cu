@@ -122,7 +122,9 @@ bh_status fetch_state(bh_ctx *c)   // synchronising
     return BH_OK;
 }
 
-bh_status do_build(bh_ctx *c, const double *pos, const double *mass, int64_t n, cudaEvent_t mass_ready = nullptr)
+// cube_done: step a1 for these positions has already run (kick_drift_cube_kernel); only the streaming path takes note
+bh_status do_build(bh_ctx *c, const double *pos, const double *mass, int64_t n, cudaEvent_t mass_ready = nullptr,
+                   bool cube_done = false)
 {
     const Workspace &w = c->ws;
     cudaStream_t s = c->stream;
@@ -166,7 +168,7 @@ bh_status do_build(bh_ctx *c, const double *pos, const double *mass, int64_t n, 
     const int64_t tiles = (n + tile_keys - 1) / tile_keys;
     cudaMemsetAsync(w.zero_begin, 0, (size_t)((char *)w.lookback - (char *)w.zero_begin) + (size_t)kSortPasses * tiles * kRadix * sizeof(unsigned), s);
     cudaMemsetAsync(w.node_meta, 0, (size_t)node_capacity(n, c->leaf_cap) * sizeof(unsigned), s);
-    {
+    if (!cube_done) {
         Phase p(c, 0);
         launch_cube(w, pos, n, s);
     }
@@ -196,7 +198,7 @@ bh_status do_build(bh_ctx *c, const double *pos, const double *mass, int64_t n, 
     if (st != BH_OK) return st;
     c->n = n;
     c->built = true;
-    c->launches += 2 + sort_launches + 3 + 1 + 1;   // cube, keys, sort (5 passes + repair + fallback), tree (3), gather + boxes, monopoles
+    c->launches += (cube_done ? 1 : 2) + sort_launches + 3 + 1 + 1;   // cube, keys, sort (5 passes + repair + fallback), tree (3), gather + boxes, monopoles
     return BH_OK;
 }
 
@@ -220,10 +222,10 @@ bh_status do_accel(bh_ctx *c, double theta, double eps, double G, double *acc, i
 
 // One gravity evaluation of the bound state into ws.acc, by the method bh_set_gravity_method chose
 // ("through N^2 interactions or by building the octree").
-bh_status do_eval_state(bh_ctx *c)
+bh_status do_eval_state(bh_ctx *c, bool cube_done = false)
 {
     if (!c->use_direct) {
-        bh_status st = do_build(c, c->pos, c->mass, c->bound_n);
+        bh_status st = do_build(c, c->pos, c->mass, c->bound_n, nullptr, cube_done);
         if (st != BH_OK) return st;
         return do_accel(c, c->theta, c->eps, c->G, c->ws.acc);
     }
@@ -581,12 +583,15 @@ static bh_status kdk_enqueue(bh_ctx *c, double dt)
         c->have_acc = true;
     }
     if (c->timing) cudaEventRecord(c->ev[8][0], c->stream);
-    launch_kick_drift(c->pos, c->vel, c->ws.acc, c->bound_n, dt, c->stream);
+    // above the one-kernel builds' sizes the drift also takes the bounding cube of the positions it writes (step a1)
+    const bool with_cube = !c->use_direct && c->bound_n > mid_build_limit(c->ws);
+    if (with_cube) launch_kick_drift_cube(c->ws, c->pos, c->vel, c->ws.acc, c->bound_n, dt, c->stream);
+    else launch_kick_drift(c->pos, c->vel, c->ws.acc, c->bound_n, dt, c->stream);
     if (c->timing) {
         cudaEventRecord(c->ev[8][1], c->stream);
         c->ev_set[8] = true;
     }
-    if ((st = do_eval_state(c)) != BH_OK) return st;
+    if ((st = do_eval_state(c, with_cube)) != BH_OK) return st;
     launch_kick(c->vel, c->ws.acc, c->bound_n, dt * 0.5, c->stream);
     c->acc_filled = true;
     c->launches += 2;   // kick+drift, kick

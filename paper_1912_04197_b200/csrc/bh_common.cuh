@@ -147,6 +147,9 @@ void launch_walk(const Workspace &w, int64_t n, double theta, double eps, double
 int launch_direct(const Workspace &w, int64_t n, const int32_t *tgt, int64_t nt, double eps, double G,
                   double *acc, bool potential, cudaStream_t s);   // returns the number of kernels launched
 void launch_kick_drift(double *pos, double *vel, const double *acc, int64_t n, double dt, cudaStream_t s);
+// the same update and, in the same pass, step a1 for the new positions (the build that follows skips launch_cube)
+void launch_kick_drift_cube(const Workspace &w, double *pos, double *vel, const double *acc, int64_t n, double dt,
+                            cudaStream_t s);
 void launch_kick(double *vel, const double *acc, int64_t n, double h, cudaStream_t s);
 void launch_unpack_mask(const Workspace &w, unsigned char *mask_out, int64_t cap, cudaStream_t s);
 // rows "next" (bh_diag.cu): results land in w.diag_out

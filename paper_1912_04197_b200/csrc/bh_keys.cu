@@ -6,34 +6,12 @@ namespace bh {
 
 constexpr int kCubeThreads = 192;   // multiple of 3: a thread always sees the same axis
 
-// One pass over the flat [3n] coordinate array; per-block partial (min, max, bad) to part[blk][8];
-// the last block to finish reduces the partials and derives the cube (R11): corner = per-axis
-// minimum, side = smallest power of two strictly above the largest extent (1 if the extent is 0).
-__global__ void __launch_bounds__(kCubeThreads) cube_kernel(const double *__restrict__ pos, long long n3,
-                                                            DevState *st, double *part)
+// The block's share of the extremes (thread t only ever met axis t % 3) -> part[blk][8]; the last block to finish reduces
+// the partials and derives the cube (finish_cube).  Shared by cube_kernel and kick_drift_cube_kernel.
+__device__ __forceinline__ void cube_block_finish(double mn, double mx, int bad, DevState *st, double *part, double *smn,
+                                                  double *smx, int *sbad, bool *is_last_p)
 {
-    __shared__ double smn[kCubeThreads], smx[kCubeThreads];
-    __shared__ int sbad[kCubeThreads];
-    __shared__ bool is_last;
     const int tid = threadIdx.x;
-    const long long stride = (long long)gridDim.x * kCubeThreads;
-    double mn = __longlong_as_double(0x7ff0000000000000ll), mx = -mn;
-    int bad = 0;
-    // four independent loads in flight per thread (the stride is a multiple of 3: same axis)
-    long long k = (long long)blockIdx.x * kCubeThreads + tid;
-    for (; k + 3 * stride < n3; k += 4 * stride) {
-        const double x0 = __ldg(pos + k), x1 = __ldg(pos + k + stride), x2 = __ldg(pos + k + 2 * stride),
-                     x3 = __ldg(pos + k + 3 * stride);
-        bad |= nonfinite(x0) | nonfinite(x1) | nonfinite(x2) | nonfinite(x3);
-        mn = fmin(fmin(mn, x0), fmin(x1, fmin(x2, x3)));
-        mx = fmax(fmax(mx, x0), fmax(x1, fmax(x2, x3)));
-    }
-    for (; k < n3; k += stride) {
-        double x = __ldg(pos + k);
-        bad |= nonfinite(x);
-        mn = fmin(mn, x);
-        mx = fmax(mx, x);
-    }
     smn[tid] = mn;
     smx[tid] = mx;
     sbad[tid] = bad;
@@ -55,9 +33,9 @@ __global__ void __launch_bounds__(kCubeThreads) cube_kernel(const double *__rest
     if (tid == 0) part[blockIdx.x * 8 + 6] = (sbad[0] | sbad[1] | sbad[2]) ? 1.0 : 0.0;
     __threadfence();
     __syncthreads();
-    if (tid == 0) is_last = (atomicAdd(&st->ticket_bbox, 1u) == gridDim.x - 1);
+    if (tid == 0) *is_last_p = (atomicAdd(&st->ticket_bbox, 1u) == gridDim.x - 1);
     __syncthreads();
-    if (!is_last) return;
+    if (!*is_last_p) return;
     __threadfence();
     // final reduction over blocks: thread t takes axis t%3 of blocks t/3, t/3+64, ...
     const int axis = tid % 3;
@@ -92,6 +70,83 @@ __global__ void __launch_bounds__(kCubeThreads) cube_kernel(const double *__rest
     }
 }
 
+// One pass over the flat [3n] coordinate array; per-block partial (min, max, bad) to part[blk][8];
+// the last block to finish reduces the partials and derives the cube (R11): corner = per-axis
+// minimum, side = smallest power of two strictly above the largest extent (1 if the extent is 0).
+__global__ void __launch_bounds__(kCubeThreads) cube_kernel(const double *__restrict__ pos, long long n3,
+                                                            DevState *st, double *part)
+{
+    __shared__ double smn[kCubeThreads], smx[kCubeThreads];
+    __shared__ int sbad[kCubeThreads];
+    __shared__ bool is_last;
+    const int tid = threadIdx.x;
+    const long long stride = (long long)gridDim.x * kCubeThreads;
+    double mn = __longlong_as_double(0x7ff0000000000000ll), mx = -mn;
+    int bad = 0;
+    // four independent loads in flight per thread (the stride is a multiple of 3: same axis)
+    long long k = (long long)blockIdx.x * kCubeThreads + tid;
+    for (; k + 3 * stride < n3; k += 4 * stride) {
+        const double x0 = __ldg(pos + k), x1 = __ldg(pos + k + stride), x2 = __ldg(pos + k + 2 * stride),
+                     x3 = __ldg(pos + k + 3 * stride);
+        bad |= nonfinite(x0) | nonfinite(x1) | nonfinite(x2) | nonfinite(x3);
+        mn = fmin(fmin(mn, x0), fmin(x1, fmin(x2, x3)));
+        mx = fmax(fmax(mx, x0), fmax(x1, fmax(x2, x3)));
+    }
+    for (; k < n3; k += stride) {
+        double x = __ldg(pos + k);
+        bad |= nonfinite(x);
+        mn = fmin(mn, x);
+        mx = fmax(mx, x);
+    }
+    cube_block_finish(mn, mx, bad, st, part, smn, smx, sbad, &is_last);
+}
+
+// Leapfrog kick + drift (R18) and the bounding cube of the NEW positions in one pass: v <- fma(a, dt/2, v); x <- fma(v, dt, x)
+// — the arithmetic of kick_drift_kernel — and the extremes of x as cube_kernel takes them, so that the build that follows
+// a step's drift needs no pass of its own over the positions.
+__global__ void __launch_bounds__(kCubeThreads) kick_drift_cube_kernel(double *__restrict__ pos, double *__restrict__ vel,
+                                                                       const double *__restrict__ acc, long long n3,
+                                                                       double h, double dt, DevState *st, double *part)
+{
+    __shared__ double smn[kCubeThreads], smx[kCubeThreads];
+    __shared__ int sbad[kCubeThreads];
+    __shared__ bool is_last;
+    const long long stride = (long long)gridDim.x * kCubeThreads;     // a multiple of 3: a thread keeps its axis
+    double mn = __longlong_as_double(0x7ff0000000000000ll), mx = -mn;
+    int bad = 0;
+    // four elements per trip, their twelve loads issued together
+    long long k = (long long)blockIdx.x * kCubeThreads + threadIdx.x;
+    for (; k + 3 * stride < n3; k += 4 * stride) {
+        double a[4], v[4], x[4];
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+            a[u] = acc[k + u * stride];
+            v[u] = vel[k + u * stride];
+            x[u] = pos[k + u * stride];
+        }
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+            v[u] = __fma_rn(a[u], h, v[u]);
+            x[u] = __fma_rn(v[u], dt, x[u]);
+            vel[k + u * stride] = v[u];
+            pos[k + u * stride] = x[u];
+            bad |= nonfinite(x[u]);
+            mn = fmin(mn, x[u]);
+            mx = fmax(mx, x[u]);
+        }
+    }
+    for (; k < n3; k += stride) {
+        const double v = __fma_rn(acc[k], h, vel[k]);
+        vel[k] = v;
+        const double x = __fma_rn(v, dt, pos[k]);
+        pos[k] = x;
+        bad |= nonfinite(x);
+        mn = fmin(mn, x);
+        mx = fmax(mx, x);
+    }
+    cube_block_finish(mn, mx, bad, st, part, smn, smx, sbad, &is_last);
+}
+
 // keys + the 8 x 256 digit histograms (shared-memory atomics, flushed once per block)
 __global__ void __launch_bounds__(256) keys_kernel(const double *__restrict__ pos, long long n,
                                                    const DevState *__restrict__ st,
@@ -123,6 +178,17 @@ void launch_cube(const Workspace &w, const double *pos, int64_t n, cudaStream_t 
     if (blocks > kMaxBboxBlocks) blocks = kMaxBboxBlocks;
     if (blocks < 1) blocks = 1;
     cube_kernel<<<blocks, kCubeThreads, 0, s>>>(pos, n3, w.st, w.bbox_part);
+}
+
+void launch_kick_drift_cube(const Workspace &w, double *pos, double *vel, const double *acc, int64_t n, double dt,
+                            cudaStream_t s)
+{
+    long long n3 = 3 * (long long)n;
+    int blocks = (int)((n3 + kCubeThreads * 4 - 1) / (kCubeThreads * 4));
+    if (blocks > w.sms * 4) blocks = w.sms * 4;   // bbox_part holds kMaxBboxBlocks rows
+    if (blocks > kMaxBboxBlocks) blocks = kMaxBboxBlocks;
+    if (blocks < 1) blocks = 1;
+    kick_drift_cube_kernel<<<blocks, kCubeThreads, 0, s>>>(pos, vel, acc, n3, dt * 0.5, dt, w.st, w.bbox_part);
 }
 
 void launch_keys(const Workspace &w, const double *pos, int64_t n, cudaStream_t s)

@@ -69,7 +69,7 @@ def test_phase_timing_and_launch_count():
     l0 = bh.bh_get_launches(ctx.ctx)
     bh.bh_kdk_step(ctx.ctx, 1e-3)                    # first step: a(x0) once more
     bh.bh_kdk_step(ctx.ctx, 1e-3)
-    assert bh.bh_get_launches(ctx.ctx) - l0 == 2 * 17 + 15      # a(x0): build 14 + walk; a step: kick+drift, 14, walk, kick
+    assert bh.bh_get_launches(ctx.ctx) - l0 == 2 * 16 + 15      # a(x0): build 14 + walk; a step: kick+drift (with the cube), 13, walk, kick
     assert bh.bh_get_phase_ms(ctx.ctx)["kick_drift"] > 0.0
     # one sort tile (n <= 4096): the whole build is one launch of one block
     small = bh.Context(2000, 16)
