@@ -162,12 +162,8 @@ bh_status do_build(bh_ctx *c, const double *pos, const double *mass, int64_t n, 
         c->no_mid = true;
     }
     int sort_launches = 0;
-    // cleared per build, sized by n (not by max_n): histograms + tickets + look-back words of this n's tiles,
-    // and the child masks / arrival counters of the nodes n bodies can make
-    const int64_t tile_keys = (int64_t)kSortThreads * sort_tile_items(n);
-    const int64_t tiles = (n + tile_keys - 1) / tile_keys;
-    cudaMemsetAsync(w.zero_begin, 0, (size_t)((char *)w.lookback - (char *)w.zero_begin) + (size_t)kSortPasses * tiles * kRadix * sizeof(unsigned), s);
-    cudaMemsetAsync(w.node_meta, 0, (size_t)node_capacity(n, c->leaf_cap) * sizeof(unsigned), s);
+    // what a build clears (histograms, tickets, look-back rows of this n, child masks / arrival counters, sized by n and
+    // not by max_n) is cleared by its first kernel: cube_kernel, or the drift that took the cube (bh_keys.cu)
     if (!cube_done) {
         Phase p(c, 0);
         launch_cube(w, pos, n, s);

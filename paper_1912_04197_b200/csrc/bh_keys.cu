@@ -70,12 +70,43 @@ __device__ __forceinline__ void cube_block_finish(double mn, double mx, int bad,
     }
 }
 
+// What a streaming build clears before its first kernel needs it (histograms and tickets + the look-back rows of this n;
+// child masks / arrival counters of the nodes n bodies can make): done by the first kernel of the build, grid-wide,
+// instead of two memsets in front of it.
+struct BuildClear {
+    uint4 *a;
+    long long a16;      // 16-byte words
+    uint4 *b;
+    long long b16;
+};
+__device__ __forceinline__ void clear_for_build(const BuildClear &z)
+{
+    const long long g = (long long)blockIdx.x * blockDim.x + threadIdx.x, step = (long long)gridDim.x * blockDim.x;
+    const uint4 zero = make_uint4(0u, 0u, 0u, 0u);
+    for (long long k = g; k < z.a16; k += step) z.a[k] = zero;
+    for (long long k = g; k < z.b16; k += step) z.b[k] = zero;
+}
+static BuildClear build_clear(const Workspace &w, int64_t n)
+{
+    const int64_t tile_keys = (int64_t)kSortThreads * sort_tile_items(n);
+    const int64_t tiles = (n + tile_keys - 1) / tile_keys;
+    const size_t abytes = (size_t)((char *)w.lookback - (char *)w.zero_begin) + (size_t)kSortPasses * tiles * kRadix * sizeof(unsigned);
+    const size_t bbytes = (size_t)node_capacity(n, w.leaf_cap) * sizeof(unsigned);
+    BuildClear z;
+    z.a = reinterpret_cast<uint4 *>(w.zero_begin);
+    z.a16 = (long long)((abytes + 15) / 16);
+    z.b = reinterpret_cast<uint4 *>(w.node_meta);
+    z.b16 = (long long)((bbytes + 15) / 16);
+    return z;
+}
+
 // One pass over the flat [3n] coordinate array; per-block partial (min, max, bad) to part[blk][8];
 // the last block to finish reduces the partials and derives the cube (R11): corner = per-axis
 // minimum, side = smallest power of two strictly above the largest extent (1 if the extent is 0).
 __global__ void __launch_bounds__(kCubeThreads) cube_kernel(const double *__restrict__ pos, long long n3,
-                                                            DevState *st, double *part)
+                                                            DevState *st, double *part, BuildClear zc)
 {
+    clear_for_build(zc);
     __shared__ double smn[kCubeThreads], smx[kCubeThreads];
     __shared__ int sbad[kCubeThreads];
     __shared__ bool is_last;
@@ -106,8 +137,10 @@ __global__ void __launch_bounds__(kCubeThreads) cube_kernel(const double *__rest
 // a step's drift needs no pass of its own over the positions.
 __global__ void __launch_bounds__(kCubeThreads) kick_drift_cube_kernel(double *__restrict__ pos, double *__restrict__ vel,
                                                                        const double *__restrict__ acc, long long n3,
-                                                                       double h, double dt, DevState *st, double *part)
+                                                                       double h, double dt, DevState *st, double *part,
+                                                                       BuildClear zc)
 {
+    clear_for_build(zc);
     __shared__ double smn[kCubeThreads], smx[kCubeThreads];
     __shared__ int sbad[kCubeThreads];
     __shared__ bool is_last;
@@ -177,7 +210,7 @@ void launch_cube(const Workspace &w, const double *pos, int64_t n, cudaStream_t 
     if (blocks > w.sms * 4) blocks = w.sms * 4;   // bbox_part holds kMaxBboxBlocks rows
     if (blocks > kMaxBboxBlocks) blocks = kMaxBboxBlocks;
     if (blocks < 1) blocks = 1;
-    cube_kernel<<<blocks, kCubeThreads, 0, s>>>(pos, n3, w.st, w.bbox_part);
+    cube_kernel<<<blocks, kCubeThreads, 0, s>>>(pos, n3, w.st, w.bbox_part, build_clear(w, n));
 }
 
 void launch_kick_drift_cube(const Workspace &w, double *pos, double *vel, const double *acc, int64_t n, double dt,
@@ -188,7 +221,7 @@ void launch_kick_drift_cube(const Workspace &w, double *pos, double *vel, const 
     if (blocks > w.sms * 4) blocks = w.sms * 4;   // bbox_part holds kMaxBboxBlocks rows
     if (blocks > kMaxBboxBlocks) blocks = kMaxBboxBlocks;
     if (blocks < 1) blocks = 1;
-    kick_drift_cube_kernel<<<blocks, kCubeThreads, 0, s>>>(pos, vel, acc, n3, dt * 0.5, dt, w.st, w.bbox_part);
+    kick_drift_cube_kernel<<<blocks, kCubeThreads, 0, s>>>(pos, vel, acc, n3, dt * 0.5, dt, w.st, w.bbox_part, build_clear(w, n));
 }
 
 void launch_keys(const Workspace &w, const double *pos, int64_t n, cudaStream_t s)
