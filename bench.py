@@ -375,7 +375,6 @@ def run_own(args):
     for _ in range(max(3, args.warmup)):
         bh.bh_kdk_step(ctx.ctx, dt)
     bh.bh_synchronize(ctx.ctx)
-    bh.bh_set_timing(ctx.ctx, True)
     l0 = bh.bh_get_launches(ctx.ctx)
     ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
     phase_sum = {k: 0.0 for k in bh.PHASE_NAMES}
@@ -385,11 +384,15 @@ def run_own(args):
     sampler.start()
     t_wall0 = time.perf_counter()
     for k in range(args.steps):
+        # per-phase events (two per phase inside the step, and a sync to read them) on a sample of the steps only: they
+        # cost the step ~35 us of gaps between its kernels (5.245 against 5.281 ms at c4 with them on every step)
+        sample = args.phases or k < 8 or k == args.steps - 1
+        bh.bh_set_timing(ctx.ctx, sample)
         flush.zero_()                                   # evict L2 between timed iterations
         ev[k][0].record(stream)
         bh.bh_kdk_step(ctx.ctx, dt)
         ev[k][1].record(stream)
-        if args.phases or k < 8 or k == args.steps - 1:   # per-phase events need a sync; sample them
+        if sample:
             ph = bh.bh_get_phase_ms(ctx.ctx)
             st = bh.bh_get_stats(ctx.ctx)
             for name in phase_sum:
