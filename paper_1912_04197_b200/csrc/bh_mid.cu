@@ -4,17 +4,17 @@
 // work, a build is bound by its sixteen dependent launches (and two memsets): a kernel of a few thousand bodies per SM ends a few
 // microseconds after it starts, and the next one cannot start before (N = 16 384: 135 us for ~15 us of work; the
 // paper's own regime is N <= 10^4 .. 10^5).  Here the same phases — cube, keys + histograms,
-// eight digit passes, gather, tree levels / scan / emission, group boxes, monopoles — run in one co-resident grid
+// the digit passes and the repair of the partial-key sort, gather, tree levels / scan / emission, group boxes, monopoles — run in one co-resident grid
 // (at most one 256-thread block per SM, cooperative launch) with a grid barrier where a launch boundary was.
 // Every phase is the tile / block function of the streaming kernels (bh_sort.cuh, bh_tree.cuh, bh_keys.cuh), so every
 // output array is the streaming path's, bit for bit.
 //
 // Coherence.  A phase reads what OTHER blocks wrote in an earlier phase of the same kernel (the sort's ping-pong
-// buffers are read, rewritten by other SMs and read again).  The grid barrier orders the accesses: every block's
-// thread 0 executes __threadfence() before it arrives and again after it has seen the barrier open, and on sm_100
-// that fence is MEMBAR.SC.GPU followed by CCTL.IVALL, which drops every line of the SM's L1 — so the plain loads of
-// the next phase cannot hit a stale line (this is what cooperative-groups grid.sync() rests on as well).  No pointer
-// to data produced here is const __restrict__ / __ldg (only the caller's pos / mass are read that way).
+// buffers are read, rewritten by other SMs and read again).  The barrier between phases orders the accesses and drops
+// the L1: the grid barrier arrives with an acq_rel atomic and waits with ld.acquire.gpu (LDG.STRONG.GPU + CCTL.IVALL on
+// sm_100, bh_grid.cuh), the cluster barrier is MEMBAR.ALL.GPU / UCGABAR / CCTL.IVALL — so the plain loads of the next
+// phase cannot hit a stale line (what cooperative-groups grid.sync() rests on as well).  No pointer to data produced
+// here is const __restrict__ / __ldg (only the caller's pos / mass are read that way).
 #include "bh_keys.cuh"
 #include "bh_sort.cuh"
 #include "bh_tree.cuh"
