@@ -166,6 +166,38 @@ bh_status bh_direct_potential(bh_ctx *ctx, double eps, double G, double *phi_dev
 bh_status bh_diagnostics(bh_ctx *ctx, const double *pos_dev, const double *vel_dev, const double *mass_dev,
                          const double *phi_dev, int64_t n, double out_host[8]);
 
+/* The same eight sums as bh_diagnostics, bit for bit, for callers that have no way to
+ * allocate device memory: no context, no workspace, and no cudaMalloc / cudaFree or other allocating call inside.
+ * That is the situation of code that is only ever handed device pointers: a plug-in or analysis hook inside
+ * a host application whose memory pool owns the whole GPU (whatever such a hook allocated itself would come out
+ * of nobody's budget and can fail once the pool has taken the card), a monitor called from inside a time-step
+ * loop where cudaMalloc / cudaFree would stall every stream of the device, or a process under a fixed memory
+ * quota.  Such a caller cannot provide the workspace bh_create asks for, so bh_diagnostics is out of its reach;
+ * this call takes only the inputs, the output and a stream.
+ *   pos_dev, vel_dev [n][3], mass_dev [n], phi_dev [n] or NULL: device arrays, read only.
+ *   out_dev [8]: DEVICE array owned by the caller, receives ekin, epot, P[3], L[3] as in bh_diagnostics.
+ *   cuda_stream: the cudaStream_t to enqueue on (NULL = legacy default stream).  The call does NOT wait for
+ *   the GPU: read out_dev after synchronising the stream, or from later work on the same stream.
+ * Scratch: the per-block partial sums and the ticket of the reduction sit in one array of
+ * BH_DIAG_STATIC_SCRATCH_BYTES (76 032) bytes of device memory inside the library image; every GPU the process
+ * uses with libbh loaded holds that much from load to exit, whether or not this call is ever made.  The array
+ * is specified for n <= BH_DIAG_STATIC_MAX_N bodies (2^30, the most bodies any libbh call accepts); a larger n
+ * is refused with BH_ERR_CAPACITY and a message naming both numbers.
+ * First call on a device: looks up the device address of the array (cudaGetSymbolAddress, once per device, with
+ * that device current) before it launches.  Make that first call outside any stream capture; later calls on the
+ * same device only enqueue a 4-byte memset (the ticket) and the kernel.
+ * Sharing: there is ONE array per GPU for the whole process and it keeps what the last call left in it.  Calls
+ * that can run on the GPU at the same time (different streams, or different host threads without ordering
+ * between their streams) overwrite each other's partial sums and both results are garbage: keep every use of
+ * this call on one device in one stream order.  Calls on different GPUs do not interact.
+ * Errors: BH_ERR_INVALID_ARG (null pointer other than phi_dev, n < 1), BH_ERR_CAPACITY (n too large),
+ * BH_ERR_CUDA (address lookup, memset or launch failed); bh_last_error(NULL) returns the message (per host
+ * thread).  Pointers are not checked for being device pointers. */
+#define BH_DIAG_STATIC_MAX_N ((int64_t)1 << 30)
+#define BH_DIAG_STATIC_SCRATCH_BYTES 76032
+bh_status bh_diagnostics_static(const double *pos_dev, const double *vel_dev, const double *mass_dev,
+                                const double *phi_dev, int64_t n, double *out_dev, void *cuda_stream);
+
 /* Synchronising. Maximum relative position error in per cent, Eq. (7) PAPER.md:223:
  * max_i 100 |r_i - r_i,ref| / |r_i,ref|, with |.|^2 = fma(z,z,fma(y,y,x*x)), e_i = 100 sqrt(|d|^2/|r_ref|^2),
  * every operation IEEE-rounded once (bit-reproducible); bodies with r_ref at the origin are skipped (R25).

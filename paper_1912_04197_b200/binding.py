@@ -62,6 +62,7 @@ def lib() -> C.CDLL:
             "bh_direct_potential": [vp, dbl, dbl, vp],
             "bh_accel_potential": [vp, dbl, dbl, dbl, vp, vp],
             "bh_diagnostics": [vp, vp, vp, vp, vp, i64, C.POINTER(dbl)],
+            "bh_diagnostics_static": [vp, vp, vp, vp, i64, vp, vp],
             "bh_position_error": [vp, vp, vp, i64, C.POINTER(dbl)],
             "bh_broadphase": [vp, vp, vp, dbl, vp, i64, C.POINTER(i64)],
             "bh_aggregates": [vp, i64, vp, i64, vp, vp, vp, vp, C.POINTER(i64)],
@@ -96,7 +97,7 @@ EXPORTS = ("bh_workspace_bytes", "bh_create", "bh_destroy", "bh_set_stream", "bh
            "bh_get_phase_ms", "bh_set_group_cell", "bh_last_error", "bh_version",
            "bh_euler_step", "bh_multirate_step", "bh_potential", "bh_direct_potential", "bh_diagnostics",
            "bh_position_error", "bh_gravity_dt", "bh_copy_state_acc", "bh_set_gravity_method",
-           "bh_broadphase", "bh_aggregates", "bh_set_graph", "bh_accel_potential")
+           "bh_broadphase", "bh_aggregates", "bh_set_graph", "bh_accel_potential", "bh_diagnostics_static")
 
 
 def _check(ctx, status: int):
@@ -216,6 +217,26 @@ def bh_diagnostics(ctx, pos, vel, mass, phi=None):
                                      _dev(mass, torch.float64, "mass"), _dev(phi, torch.float64, "phi"),
                                      pos.shape[0], out))
     return {"ekin": out[0], "epot": out[1], "P": [out[2], out[3], out[4]], "L": [out[5], out[6], out[7]]}
+
+
+DIAG_STATIC_MAX_N = 1 << 30           # BH_DIAG_STATIC_MAX_N
+DIAG_STATIC_SCRATCH_BYTES = 76032     # BH_DIAG_STATIC_SCRATCH_BYTES
+
+
+def bh_diagnostics_static(pos, vel, mass, phi, out, stream=None, n=None):
+    """bh_diagnostics for callers that cannot allocate device memory (include/bh.h): no context and no
+    workspace; the reduction's scratch is a fixed array inside libbh.  `out` is a CUDA float64 tensor of 8
+    elements that the caller owns; it is filled in stream order (ekin, epot, P[3], L[3]) and the call does
+    not wait: synchronise before reading it on the host.  All calls on one GPU share the scratch, so keep them
+    in one stream order.  This wrapper allocates nothing either."""
+    if out.numel() < 8:
+        raise TypeError("out: expected 8 float64 elements on the GPU")
+    st = lib().bh_diagnostics_static(_dev(pos, torch.float64, "pos"), _dev(vel, torch.float64, "vel"),
+                                     _dev(mass, torch.float64, "mass"), _dev(phi, torch.float64, "phi"),
+                                     pos.shape[0] if n is None else n, _dev(out, torch.float64, "out"),
+                                     _stream_ptr(stream))
+    _check(None, st)
+    return out
 
 
 def bh_position_error(ctx, pos, ref) -> float:

@@ -370,6 +370,9 @@ Workspace carve(char *base, int64_t max_n, int leaf_cap)
 
 }  // namespace bh
 
+// message of a call that has no context (bh_diagnostics_static, bh_diag.cu): what bh_last_error(NULL) returns
+void bh::set_global_error(const char *msg) { snprintf(g_err, 256, "%s", msg); }
+
 extern "C" {
 
 const char *bh_version(void) { return "bh-b200 0.1 (sm_100a)"; }

@@ -161,6 +161,8 @@ int launch_broadphase(const Workspace &w, int64_t n, const double *radius, const
                       int32_t *pairs, int64_t cap, cudaStream_t s);   // count lands in st->pair_count
 int launch_aggregates(const Workspace &w, int64_t n, const int32_t *pairs, int64_t n_pairs, const double *mass_in,
                       int32_t *label, int32_t *size, double *mass, cudaStream_t s);   // counts in st->agg_counts
+// record the message of a context-free call that failed; bh_last_error(NULL) returns it (per host thread)
+void set_global_error(const char *msg);
 void launch_euler_sub(double *pos, double *vel, const double *acc, int64_t n, double dt, int n_sub, cudaStream_t s);
 
 // ---- small device helpers ----

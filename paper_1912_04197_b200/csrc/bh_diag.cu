@@ -9,6 +9,9 @@
 // memory, and by the last block to finish (ticket) over the per-block results in block order.  The
 // result does not depend on scheduling and is good to ~1e-30 relative to the sum of |terms|, then
 // rounded once to fp64.
+#include <cstdio>
+#include <mutex>
+
 #include "bh_common.cuh"
 
 namespace bh {
@@ -186,4 +189,92 @@ void launch_euler_sub(double *pos, double *vel, const double *acc, int64_t n, do
     euler_sub_kernel<<<blocks, 256, 0, s>>>(pos, vel, acc, n3, dt, n_sub);
 }
 
+// ---- bh_diagnostics_static: the conserved quantities without a context, a workspace or any allocation ----
+//
+// diag_kernel needs scratch memory: one row of eight double-double partial sums per block, and the ticket
+// that elects the block which adds the rows up.  bh_diagnostics takes both from the workspace the caller
+// allocated for bh_create.  The scratch below lives in the library image instead, so a caller that owns no
+// device allocator at all can still follow the energy and momenta of bodies somebody else keeps on the GPU.
+// Row layout as in diag_kernel: [block][quantity][hi, lo]; the ticket sits in a 256-byte row of its own
+// after the last partial row.
+constexpr size_t kStaticDiagPartDoubles = (size_t)kDiagBlocks * kDiagQ * 2;          // 592 x 8 x 2 doubles = 75 776 bytes
+constexpr size_t kStaticDiagDoubles = kStaticDiagPartDoubles + 256 / sizeof(double);   // + the ticket's row
+static_assert(kStaticDiagDoubles * sizeof(double) == BH_DIAG_STATIC_SCRATCH_BYTES, "bh.h states the size of the static scratch");
+
+static __device__ __align__(256) double g_static_diag_scratch[kStaticDiagDoubles];
+
+constexpr int kStaticMaxDevices = 64;
+static double *g_static_diag_ptr[kStaticMaxDevices];   // device address of the array, per device ordinal; null = not asked yet
+static std::mutex g_static_diag_mutex;
+
+// Address of g_static_diag_scratch on the CURRENT device.  In host code the array's name is only the handle
+// the runtime registered for it, not somewhere a kernel can read or write: the real address differs from GPU
+// to GPU and has to be asked for with that GPU current, once.
+static cudaError_t static_diag_scratch(double **out)
+{
+    int dev = -1;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    if (dev < 0 || dev >= kStaticMaxDevices) return cudaErrorInvalidDevice;
+    std::lock_guard<std::mutex> hold(g_static_diag_mutex);
+    if (!g_static_diag_ptr[dev]) {
+        void *p = nullptr;
+        e = cudaGetSymbolAddress(&p, g_static_diag_scratch);
+        if (e != cudaSuccess) return e;
+        g_static_diag_ptr[dev] = static_cast<double *>(p);
+    }
+    *out = g_static_diag_ptr[dev];
+    return cudaSuccess;
+}
+
 }  // namespace bh
+
+extern "C" bh_status bh_diagnostics_static(const double *pos_dev, const double *vel_dev, const double *mass_dev,
+                                           const double *phi_dev, int64_t n, double *out_dev, void *cuda_stream)
+{
+    using namespace bh;
+    char msg[256];
+    if (!pos_dev || !vel_dev || !mass_dev || !out_dev) {
+        set_global_error("bh_diagnostics_static: null pointer");
+        return BH_ERR_INVALID_ARG;
+    }
+    if (n < 1) {
+        set_global_error("bh_diagnostics_static: n < 1");
+        return BH_ERR_INVALID_ARG;
+    }
+    if (n > BH_DIAG_STATIC_MAX_N) {
+        snprintf(msg, sizeof msg, "bh_diagnostics_static: n = %lld is above BH_DIAG_STATIC_MAX_N = %lld, the most bodies "
+                 "the fixed scratch array is specified for (use bh_diagnostics with a workspace)",
+                 (long long)n, (long long)BH_DIAG_STATIC_MAX_N);
+        set_global_error(msg);
+        return BH_ERR_CAPACITY;
+    }
+    double *scratch = nullptr;
+    cudaError_t e = static_diag_scratch(&scratch);
+    if (e != cudaSuccess) {
+        snprintf(msg, sizeof msg, "bh_diagnostics_static: address of the static scratch: %s", cudaGetErrorString(e));
+        set_global_error(msg);
+        return BH_ERR_CUDA;
+    }
+    cudaStream_t s = static_cast<cudaStream_t>(cuda_stream);
+    unsigned *ticket = reinterpret_cast<unsigned *>(scratch + kStaticDiagPartDoubles);
+    // The ticket must read 0 when the first block arrives.  A completed call leaves it at 0, but the array is
+    // shared by everybody in the process, so a call that was cut short (a fault, a reset stream) may not have:
+    // clear it every time.  The partial rows need no clearing: a block writes its row before it takes a ticket,
+    // and only rows of this launch's blocks are read.
+    e = cudaMemsetAsync(ticket, 0, sizeof(unsigned), s);
+    if (e == cudaSuccess) {
+        // same grid as launch_diagnostics: the rows, and with them the order of the additions, are those of
+        // bh_diagnostics, so the two calls give the same bits
+        int blocks = (int)((n + kDiagThreads - 1) / kDiagThreads);
+        if (blocks > kDiagBlocks) blocks = kDiagBlocks;
+        diag_kernel<<<blocks, kDiagThreads, 0, s>>>(pos_dev, vel_dev, mass_dev, phi_dev, n, scratch, ticket, out_dev);
+        e = cudaGetLastError();
+    }
+    if (e != cudaSuccess) {
+        snprintf(msg, sizeof msg, "bh_diagnostics_static launch: %s", cudaGetErrorString(e));
+        set_global_error(msg);
+        return BH_ERR_CUDA;
+    }
+    return BH_OK;
+}
