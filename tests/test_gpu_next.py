@@ -180,14 +180,27 @@ def test_stepper_state_errors():
     with pytest.raises(bh.BhError) as ei:
         bh.bh_multirate_step(ctx.ctx, 1e-3, 0)
     assert ei.value.status == bh.BH_ERR_INVALID_ARG
-    # Euler then KDK: the KDK step re-evaluates a(x) (the Euler step leaves a(x_k) behind)
-    bh.bh_euler_step(ctx.ctx, 1e-3)
-    p0, v0 = pos.cpu().numpy().copy(), vel.cpu().numpy().copy()
-    bh.bh_kdk_step(ctx.ctx, 1e-3)
+    # Euler then KDK: the KDK step re-evaluates a(x) (the Euler step leaves a(x_k) behind).  Checked per evaluation on
+    # the GPU's own positions (never trajectory against trajectory): one kick + drift from the oracle's
+    # a(p0) must give the GPU's new positions to what 1e-11 on the accelerations allows, and the stale a(x_k) must not.
+    dt = 1e-3
+    p_before = pos.cpu().numpy().copy()
+    bh.bh_euler_step(ctx.ctx, dt)
     bh.bh_synchronize(ctx.ctx)
-    lf = orc.Leapfrog(p0, v0, w.mass, 0.5, 1e-3, 1.0, 8)
-    lf.step(1e-3)
-    assert np.abs(pos.cpu().numpy() - lf.pos).max() <= 1e-13
+    p0, v0 = pos.cpu().numpy().copy(), vel.cpu().numpy().copy()
+    bh.bh_kdk_step(ctx.ctx, dt)
+    bh.bh_synchronize(ctx.ctx)
+    p1 = pos.cpu().numpy()
+
+    def drifted(a):
+        vh = v0.copy(); orc.kick(vh, a, dt * 0.5)
+        x = p0.copy(); orc.drift(x, vh, dt)
+        return x
+    a0 = orc.accel(orc.build(p0, w.mass, 8), 0.5, 1e-3, 1.0)[0]
+    a_stale = orc.accel(orc.build(p_before, w.mass, 8), 0.5, 1e-3, 1.0)[0]
+    tol_x = TOL * np.abs(a0).max() * dt * dt * 0.5 + 2 * np.finfo(float).eps * np.abs(p1).max()
+    assert np.abs(p1 - drifted(a0)).max() <= tol_x
+    assert np.abs(p1 - drifted(a_stale)).max() > 10 * tol_x
     ctx.close()
 
 
@@ -200,28 +213,49 @@ def test_steppers_with_direct_gravity():
     pos, vel, mass = dev(w.pos), dev(v0), dev(w.mass)
     bh.bh_bind_state(ctx.ctx, pos, vel, mass, w.theta, w.eps, w.G)
     bh.bh_set_gravity_method(ctx.ctx, 1)
-    lf = orc.Leapfrog(w.pos, v0, w.mass, w.theta, w.eps, w.G, 8, use_direct=True)
-    for _ in range(3):
-        bh.bh_kdk_step(ctx.ctx, 1e-3)
-        lf.step(1e-3)
-    bh.bh_synchronize(ctx.ctx)
-    assert np.abs(pos.cpu().numpy() - lf.pos).max() <= 1e-13
-    assert np.abs(vel.cpu().numpy() - lf.vel).max() <= 1e-12
+    # per evaluation, on the GPU's own positions: after every step the accelerations the context holds
+    # are Eq. (1) at the new positions within TOL, and the update is the canonical kick / drift / kick of the GPU's own
+    # accelerations, bit for bit (the first step's a(x0) is not kept: the oracle's stands in, to what TOL allows)
+    dt = 1e-3
     a = torch.empty((600, 3), dtype=torch.float64, device="cuda")
-    bh.bh_copy_state_acc(ctx.ctx, a)
-    ref = orc.direct(lf.pos, w.mass, w.eps, w.G)
-    assert (np.linalg.norm(a.cpu().numpy() - ref, axis=1) / np.linalg.norm(ref, axis=1)).max() <= 1e-10
+    a_prev = None
+    for step in range(3):
+        p_prev, v_prev = pos.cpu().numpy().copy(), vel.cpu().numpy().copy()
+        bh.bh_kdk_step(ctx.ctx, dt)
+        bh.bh_copy_state_acc(ctx.ctx, a)
+        bh.bh_synchronize(ctx.ctx)
+        p, v, a_gpu = pos.cpu().numpy(), vel.cpu().numpy(), a.cpu().numpy().copy()
+        ref = orc.direct(p, w.mass, w.eps, w.G)
+        assert (np.linalg.norm(a_gpu - ref, axis=1) / np.linalg.norm(ref, axis=1)).max() <= TOL
+        first = a_prev is None
+        if first:
+            a_prev = orc.direct(p_prev, w.mass, w.eps, w.G)
+        vh = v_prev.copy(); orc.kick(vh, a_prev, dt * 0.5)
+        x = p_prev.copy(); orc.drift(x, vh, dt)
+        v1 = vh.copy(); orc.kick(v1, a_gpu, dt * 0.5)
+        if first:
+            amax = np.abs(a_prev).max()
+            assert np.abs(p - x).max() <= TOL * amax * dt * dt * 0.5 + 2 * np.finfo(float).eps * np.abs(x).max()
+            assert np.abs(v - v1).max() <= TOL * amax * dt + 2 * np.finfo(float).eps * np.abs(v1).max()
+        else:
+            assert np.array_equal(p, x) and np.array_equal(v, v1)
+        a_prev = a_gpu
     # no tree after a direct evaluation
     with pytest.raises(bh.BhError) as ei:
         ctx.n = 600
         ctx.accel(0.5, 1e-3, 1.0)
     assert ei.value.status == bh.BH_ERR_STATE
-    # Euler with direct gravity, then back to the tree
-    st = orc.Stepper(lf.pos, lf.vel, w.mass, w.theta, w.eps, w.G, 8, use_direct=True)
-    bh.bh_euler_step(ctx.ctx, 1e-3)
-    st.euler(1e-3)
+    # Euler with direct gravity (the context then holds a(x_k) at the positions the step started from), then back to the tree
+    p0, v0 = pos.cpu().numpy().copy(), vel.cpu().numpy().copy()
+    bh.bh_euler_step(ctx.ctx, dt)
+    bh.bh_copy_state_acc(ctx.ctx, a)
     bh.bh_synchronize(ctx.ctx)
-    assert np.abs(pos.cpu().numpy() - st.pos).max() <= 1e-13
+    a_gpu = a.cpu().numpy()
+    ref = orc.direct(p0, w.mass, w.eps, w.G)
+    assert (np.linalg.norm(a_gpu - ref, axis=1) / np.linalg.norm(ref, axis=1)).max() <= TOL
+    v1 = v0.copy(); orc.kick(v1, a_gpu, dt)
+    x1 = p0.copy(); orc.drift(x1, v1, dt)
+    assert np.array_equal(vel.cpu().numpy(), v1) and np.array_equal(pos.cpu().numpy(), x1)
     bh.bh_set_gravity_method(ctx.ctx, 0)
     bh.bh_euler_step(ctx.ctx, 1e-3)
     bh.bh_synchronize(ctx.ctx)

@@ -327,8 +327,8 @@ def test_error_reporting():
 
 def test_full_size_headline_config():
     """configs[3] at its full size (N = 1M Plummer, C=16, theta=0.5), in the launch configuration
-    bench.py times: tree bit-exact against the oracle; accelerations on sampled groups that the
-    oracle can compute one by one; list lengths exact on those groups; totals consistent."""
+    bench.py times: tree bit-exact against the oracle; accelerations of ALL bodies and the list lengths of
+    ALL groups against the oracle's walk; totals consistent."""
     w = wl.make("c4")
     t = orc.build(w.pos, w.mass, w.leaf_cap)
     ctx = gpu_build(w.pos, w.mass, w.leaf_cap)
@@ -338,11 +338,14 @@ def test_full_size_headline_config():
     assert np.isfinite(a).all()
     ng = t.ngroups
     assert gm.shape[0] == ng
-    for g0 in list(range(0, ng, ng // 24))[:24] + [ng - 2]:
-        ref, nm, nd, _ = orc.accel(t, w.theta, w.eps, w.G, g0, g0 + 2)
-        rows = t.perm[t.gstart[g0]:t.gstart[g0 + 2]]
-        assert np.array_equal(gm[g0:g0 + 2], nm) and np.array_equal(gd[g0:g0 + 2], nd)
-        assert relerr(a[rows], ref[rows]).max() <= TOL
+    # north_star's target as stated: the maximum over ALL bodies.  The oracle walks every one of the ~36 000 groups
+    # (about 10 s on 16 cores): list lengths of every group exactly, every body's acceleration within TOL.
+    ref, nm, nd, kappa = orc.accel(t, w.theta, w.eps, w.G, want_kappa=True)
+    assert np.array_equal(gm, nm) and np.array_equal(gd, nd)
+    e = relerr(a, ref)
+    worst = int(e.argmax())
+    assert e.max() <= TOL, f"max rel err {e.max():.3e} at body {worst} (kappa {kappa[worst]:.3g})"
+    print(f"c4 all bodies: max rel err {e.max():.3e} at body {worst} (kappa {kappa[worst]:.3g}), median {np.median(e):.3e}")
     st = bh.bh_get_stats(ctx.ctx)
     assert st["n_mono"] == int(gm.astype(np.int64).sum()) and st["n_direct"] == int(gd.astype(np.int64).sum())
     assert st["interactions"] == int(((gm.astype(np.int64) + gd) * np.diff(t.gstart.astype(np.int64))).sum())
@@ -378,8 +381,8 @@ def test_eval_host_pageable_and_pinned_agree():
 
 
 def test_full_size_largest_config():
-    """configs[4] at its full size (N = 4 194 304 rotating ball, C = 32, theta = 0.6): tree bit-exact, sampled
-    groups against the oracle's walk, and the config's own check — the direct sum on random targets."""
+    """configs[4] at its full size (N = 4 194 304 rotating ball, C = 32, theta = 0.6): tree bit-exact, all
+    groups and all bodies against the oracle's walk, and the config's own check — the direct sum on random targets."""
     w = wl.make("c5")
     t = orc.build(w.pos, w.mass, w.leaf_cap)
     ctx = gpu_build(w.pos, w.mass, w.leaf_cap)
@@ -387,11 +390,14 @@ def test_full_size_largest_config():
     a = ctx.accel(w.theta, w.eps, w.G).cpu().numpy()
     gm, gd = (x.cpu().numpy().view(np.uint32) for x in ctx.counts())
     ng = t.ngroups
-    for g0 in list(range(0, ng, ng // 12))[:12] + [ng - 2]:
-        ref, nm, nd, _ = orc.accel(t, w.theta, w.eps, w.G, g0, g0 + 2)
-        rows = t.perm[t.gstart[g0]:t.gstart[g0 + 2]]
-        assert np.array_equal(gm[g0:g0 + 2], nm) and np.array_equal(gd[g0:g0 + 2], nd)
-        assert relerr(a[rows], ref[rows]).max() <= TOL
+    assert gm.shape[0] == ng
+    # every group, every body (the oracle's walk of all ~147 000 groups: about 20 s on 16 cores)
+    ref, nm, nd, kappa = orc.accel(t, w.theta, w.eps, w.G, want_kappa=True)
+    assert np.array_equal(gm, nm) and np.array_equal(gd, nd)
+    e = relerr(a, ref)
+    worst = int(e.argmax())
+    assert e.max() <= TOL, f"max rel err {e.max():.3e} at body {worst} (kappa {kappa[worst]:.3g})"
+    print(f"c5 all bodies: max rel err {e.max():.3e} at body {worst} (kappa {kappa[worst]:.3g}), median {np.median(e):.3e}")
     tg = np.random.default_rng(5).choice(w.n, size=128, replace=False).astype(np.int32)
     b = ctx.direct(w.eps, w.G, targets=dev(tg, torch.int32)).cpu().numpy()
     refd = orc.direct(w.pos, w.mass, w.eps, w.G, targets=tg)

@@ -176,9 +176,9 @@ def test_accept_rule_on_hand_built_geometry():
     com = t.mono[node, :3]
     assert list(com) == [15.0, 0.0, 0.125]
     theta = s / 15.0          # d = (15,0,0) exactly
-    if (theta * theta) * 225.0 == s * s:
-        lm, _ = orc.walk_lists(t, 0, theta)
-        assert node not in lm
+    assert (theta * theta) * 225.0 == s * s       # the geometry is chosen so that equality is exact in fp64 (R5)
+    lm, _ = orc.walk_lists(t, 0, theta)
+    assert node not in lm
 
 
 # ------------------------------------------------------------------ textbook per-body Barnes-Hut
@@ -452,3 +452,19 @@ def test_kdk_tree_matches_direct_at_theta_zero():
         a.step(1e-3)
         b.step(1e-3)
     assert np.abs(a.pos - b.pos).max() < 1e-14 and np.abs(a.vel - b.vel).max() < 1e-13
+
+
+def test_kappa_hand_case():
+    """The diagnostic kappa = sum |term| / |sum of terms| (reported beside a failing body in the GPU parity tests) on
+    three collinear unit masses at x = 0, 1, -2, eps = 0, G = 1: body 0 is pulled by +1 and -1/4 (kappa = 1.25 / 0.75 =
+    5/3), body 1 by -1 and -1/9 (same direction: kappa = 1), body 2 by +1/4 and +1/9 (kappa = 1); the same from the tree
+    walk at theta = 0 (all sources direct) and from the direct sum."""
+    pos = np.array([[0.0, 0, 0], [1.0, 0, 0], [-2.0, 0, 0]])
+    mass = np.ones(3)
+    acc, kappa = orc.direct(pos, mass, 0.0, 1.0, want_kappa=True)
+    assert np.allclose(acc[:, 0], [0.75, -1.0 - 1.0 / 9.0, 0.25 + 1.0 / 9.0], rtol=1e-15, atol=0)
+    assert np.allclose(kappa, [5.0 / 3.0, 1.0, 1.0], rtol=1e-15, atol=0)
+    t = orc.build(pos, mass, 1)
+    acc_t, _, _, kappa_t = orc.accel(t, 0.0, 0.0, 1.0, want_kappa=True)
+    assert np.allclose(kappa_t, [5.0 / 3.0, 1.0, 1.0], rtol=1e-15, atol=0) and np.allclose(acc_t, acc, rtol=1e-15, atol=0)
+
