@@ -416,34 +416,51 @@ def run_own(args):
     inter_avg = sum(inter) / nph
     achieved = FLOPS_PER_INTERACTION * inter_avg / (walk_avg_ms * 1e-3) / 1e12
     mb = Microbench()
-    peak_meas = mb.fp64_peak(stream)
+    # ONE denominator: the best DFMA rate this run measured (two kernels of libbh_microbench.so time the same eight
+    # register-resident chains per thread; they differ in loop shape only)
+    mma = mb.fp64_mma(stream)
+    peak_meas = max(mb.fp64_peak(stream), mma["dfma_tflops"])
     issue = mb.issue_model(stream)
     prof = profile_row("walk_kernel", w.name)
     roofline = {"bound": "alu", "kernel": "walk_kernel", "achieved": achieved, "peak": peak_meas,
                 "unit": "TFLOP/s", "frac": achieved / peak_meas,
-                "peak_source": "fp64 FMA rate measured in this run (register-resident DFMA chains on every SM, "
-                               "libbh_microbench.so); MEASURED_PEAKS.json has no fp64 entry",
+                "peak_source": "best fp64 FMA rate measured in this run (register-resident DFMA chains on every SM, "
+                               "libbh_microbench.so: max of bhmb_fp64_peak and bhmb_fp64_mma's DFMA leg); "
+                               "MEASURED_PEAKS.json has no fp64 entry",
                 "peak_nominal": FP64_NOMINAL_TFLOPS, "frac_of_nominal": achieved / FP64_NOMINAL_TFLOPS,
                 "flops_per_interaction": FLOPS_PER_INTERACTION, "interactions_per_launch": inter_avg,
                 "interactions_per_s": inter_avg / (walk_avg_ms * 1e-3), "kernel_ms": walk_avg_ms,
-                "issue_model_interactions_per_s": issue, "fp64_tensor_core": mb.fp64_mma(stream),
+                "issue_model_interactions_per_s": issue, "fp64_tensor_core": mma,
                 "frac_of_eval_loop_alone": inter_avg / (walk_avg_ms * 1e-3) / issue["eval_loop_alone"],
                 "traffic": float(prof["dram_bytes_per_launch"]) if prof else None,
                 "l2_hit_rate": float(prof["l2_hit_pct"]) / 100.0 if prof else None,
                 "fp64_pipe_active": float(prof["fp64_pipe_pct"]) / 100.0 if prof else None,
                 "profile_source": (f"profiles/r02_roofline.csv (ncu --set full at commit {prof['commit']}; profiler "
                                    "figures, not measured by this run)") if prof else None}
-    # build kernels against HBM: algorithmic bytes per body over the build time
+    # build kernels against HBM: algorithmic bytes per body over the time of the SAME phases.
+    # Inside a KDK step above the one-kernel builds' sizes the drift kernel takes the bounding cube (step a1): that pass
+    # is timed under "kick_drift", phases["cube"] is 0, and a1's 24 B/body leave the numerator with it.
     build_ms = sum(phases[k] for k in ("cube", "keys", "sort", "gather", "tree", "monopoles"))
-    build_bytes = 390.0 * w.n
-    hbm_peak = 6546.9
+    cube_in_drift = phases["cube"] == 0.0 and phases["keys"] > 0.0
+    survey_bytes = 390 - (24 if cube_in_drift else 0)      # eight sort passes, boxes re-read the bodies
+    executed_bytes = survey_bytes - 32 - 48                # boxes taken from registers (-32), six sort passes of eight (-48)
+    hbm_peak, hbm_source = 6650.0, "B200_PROFILING.md fallback (MEASURED_PEAKS.json absent): of fallback"
     try:
-        hbm_peak = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))["hbm_gbs"]
+        hbm_peak = float(json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))["hbm_gbs"])
+        hbm_source = "MEASURED_PEAKS.json hbm_gbs"
     except Exception:
         pass
-    build_roof = {"bound": "hbm", "achieved": build_bytes / (build_ms * 1e-3) / 1e9, "peak": hbm_peak,
-                  "unit": "GB/s", "frac": build_bytes / (build_ms * 1e-3) / 1e9 / hbm_peak,
-                  "algorithmic_bytes_per_body": 390, "build_ms": build_ms}
+    gbs = lambda b: b * w.n / (build_ms * 1e-3) / 1e9
+    build_roof = {"bound": "hbm", "achieved": gbs(survey_bytes), "peak": hbm_peak, "peak_source": hbm_source,
+                  "unit": "GB/s", "frac": gbs(survey_bytes) / hbm_peak,
+                  "algorithmic_bytes_per_body": survey_bytes,
+                  "count": "SURVEY.md 8(d) count for the phases in build_ms (390 B/body with step a1, 366 without)",
+                  "cube_in_drift": cube_in_drift,
+                  "executed_bytes_per_body": executed_bytes, "achieved_executed": gbs(executed_bytes),
+                  "frac_executed": gbs(executed_bytes) / hbm_peak,
+                  "executed_count": "as executed: group boxes from registers (-32 B), 5 digit passes + repair instead "
+                                    "of 8 passes (-48 B)",
+                  "build_ms": build_ms}
 
     out = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
            "warmup": max(3, args.warmup), "ms_per_step": total_ms / args.steps, "higher_is_better": True,

@@ -120,8 +120,8 @@ bh_status bh_copy_state_acc(bh_ctx *ctx, double *acc_dev);
  * After a direct evaluation the context holds no tree: bh_accel etc. need a new bh_build. */
 bh_status bh_set_gravity_method(bh_ctx *ctx, int method);
 
-/* Replay the steppers through a CUDA graph (enable != 0).  A step at small N is bound by its nineteen
- * kernel launches (the paper sees the same: octree creation dominates for few bodies); with
+/* Replay the steppers through a CUDA graph (enable != 0).  A step at small N is bound by its kernel
+ * launches (sixteen in a streaming build) (the paper sees the same: octree creation dominates for few bodies); with
  * the graph on, the second bh_kdk_step / bh_euler_step / bh_multirate_step call with the same arguments on
  * the same bound state is captured while it is enqueued and later calls replay it with one launch.
  * Results are bit-identical to the plain path.  Ignored while bh_set_timing is on (events are not
@@ -280,7 +280,10 @@ bh_status bh_get_launches(bh_ctx *ctx, uint64_t *count_host);
  * durations in ms: [0] cube, [1] keys+histogram, [2] sort, [3] gather+boxes, [4] tree,
  * [5] monopoles, [6] walk, [7] direct, [8] kick/drift kernels of the last bh_kdk_step.  A build of at most
  * 1024 bodies per multiprocessor is ONE kernel (one block up to 4096 bodies, one co-resident grid with grid
- * barriers above): its whole duration is reported as [4] and [0]-[3], [5] are 0. */
+ * barriers above): its whole duration is reported as [4] and [0]-[3], [5] are 0.  A build reports only the phases
+ * it ran itself: inside a bh_kdk_step above those sizes the drift kernel also takes the bounding cube of the
+ * positions it writes, so [0] is 0 for that step's build and the cube's cost is part of [8]; a stepper that
+ * evaluates gravity by the direct sum reports [7] and 0 for [0]-[6], one that walks the tree 0 for [7]. */
 #define BH_NUM_PHASES 9
 bh_status bh_set_timing(bh_ctx *ctx, int enable);
 bh_status bh_get_phase_ms(bh_ctx *ctx, float ms_host[BH_NUM_PHASES]);

@@ -17,6 +17,9 @@ __global__ void __launch_bounds__(256) fp64_peak_kernel(double *sink, int iters,
     double a0 = seed + threadIdx.x, a1 = a0 + 1, a2 = a0 + 2, a3 = a0 + 3, a4 = a0 + 4, a5 = a0 + 5, a6 = a0 + 6,
            a7 = a0 + 7;
     const double m = 0.999999, c = 1e-9;
+    // sixteen trips per branch: the loop's own integer instructions take issue slots from the DFMAs of the same
+    // sub-partition (34.8 TFLOP/s without the unroll against 36.0 with it, same chip, same minute)
+#pragma unroll 16
     for (int i = 0; i < iters; ++i) {
         a0 = fma(a0, m, c); a1 = fma(a1, m, c); a2 = fma(a2, m, c); a3 = fma(a3, m, c);
         a4 = fma(a4, m, c); a5 = fma(a5, m, c); a6 = fma(a6, m, c); a7 = fma(a7, m, c);

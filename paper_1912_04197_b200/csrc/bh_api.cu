@@ -3,6 +3,7 @@
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <atomic>
 #include <new>
 
 #include "bh_common.cuh"
@@ -15,6 +16,8 @@ struct bh_ctx {
     int group = kMaxGroup;   // W
     int group_cell = BH_GROUP_CELL_DEFAULT;   // Gc
     cudaStream_t stream = nullptr;
+    int device = 0;          // ordinal of the device that was current at bh_create: the workspace, the stream and the
+                             // per-device kernel attributes belong to it
     Workspace ws{};
     int64_t n = 0;          // bodies of the last build
     bool built = false;
@@ -32,7 +35,7 @@ struct bh_ctx {
     bool timing = false;
     cudaEvent_t ev[BH_NUM_PHASES][2]{};
     bool ev_set[BH_NUM_PHASES]{};
-    // CUDA graph of one stepper call (launch-bound at small N: 19 launches per step)
+    // CUDA graph of one stepper call (sixteen launches per step with the streaming build)
     struct StepSig {
         int kind = -1, n_sub = 0;
         double dt = 0, theta = 0, eps = 0, G = 0;
@@ -73,6 +76,22 @@ bh_status cuda_check(bh_ctx *c, cudaError_t e, const char *what)
     if (e == cudaSuccess) return BH_OK;
     snprintf(c->err, 256, "%s: %s", what, cudaGetErrorString(e));
     return BH_ERR_CUDA;
+}
+
+// A context belongs to the device that was current at bh_create (workspace, stream, events, the SM count its grids
+// are sized by).  A call made with another device current would launch there on foreign pointers: refuse it.
+bh_status on_device(bh_ctx *c, const char *who)
+{
+    int dev = -1;
+    if (cudaGetDevice(&dev) != cudaSuccess) {
+        cudaGetLastError();
+        return fail(c, BH_ERR_CUDA, "no current CUDA device");
+    }
+    if (dev != c->device) {
+        snprintf(c->err, 256, "%s: the context was created on device %d, the current device is %d", who, c->device, dev);
+        return BH_ERR_STATE;
+    }
+    return BH_OK;
 }
 
 inline size_t align_up(size_t x) { return (x + 255) & ~(size_t)255; }
@@ -130,6 +149,10 @@ bh_status do_build(bh_ctx *c, const double *pos, const double *mass, int64_t n, 
     cudaStream_t s = c->stream;
     c->built = false;
     c->walked = false;
+    // phases this build does not record read 0 (one-kernel builds record [4] only; a build whose cube came out of the
+    // drift records no [0]), not what an earlier build left
+    if (c->timing)
+        for (int p = 0; p <= 5; ++p) c->ev_set[p] = false;
     if (n <= kSortTile) {   // one block does the whole build (and its own clearing): one launch
         if (mass_ready) cudaStreamWaitEvent(s, mass_ready, 0);   // masses copied on another stream
         {
@@ -176,7 +199,7 @@ bh_status do_build(bh_ctx *c, const double *pos, const double *mass, int64_t n, 
         Phase p(c, 2);
         sort_launches = launch_sort(w, pos, n, s);
     }
-    if (sort_launches < 0) return fail(c, BH_ERR_CUDA, "bh_build: the sort's fallback kernel could not be launched");
+    if (sort_launches < 0) return fail(c, BH_ERR_CUDA, "bh_build: the sort could not be enqueued");
     {
         Phase p(c, 4);
         launch_tree(w, n, c->leaf_cap, s);                       // from the sorted keys alone
@@ -220,6 +243,12 @@ bh_status do_accel(bh_ctx *c, double theta, double eps, double G, double *acc, i
 // ("through N^2 interactions or by building the octree").
 bh_status do_eval_state(bh_ctx *c, bool cube_done = false)
 {
+    if (c->timing) {   // the stepper's evaluation is a tree walk or a direct sum: the other one's phase reads 0
+        if (c->use_direct)
+            for (int p = 0; p <= 6; ++p) c->ev_set[p] = false;
+        else
+            c->ev_set[7] = false;
+    }
     if (!c->use_direct) {
         bh_status st = do_build(c, c->pos, c->mass, c->bound_n, nullptr, cube_done);
         if (st != BH_OK) return st;
@@ -287,20 +316,32 @@ bh_status run_stepper(bh_ctx *c, int kind, double dt, int n_sub, F enqueue)
 
 namespace bh {
 
+int current_device()
+{
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess) {
+        cudaGetLastError();
+        return 0;
+    }
+    return dev >= 0 && dev < kMaxDevices ? dev : 0;
+}
+
 int sm_count()
 {
-    static int sms = 0;
-    if (sms == 0) {
-        int dev = 0, v = 0;
-        if (cudaGetDevice(&dev) == cudaSuccess &&
-            cudaDeviceGetAttribute(&v, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess && v > 0) {
-            sms = v;
+    static std::atomic<int> sms[kMaxDevices];   // per device ordinal; 0 = not asked yet
+    const int dev = current_device();
+    int v = sms[dev].load(std::memory_order_relaxed);
+    if (v == 0) {
+        int cur = 0;
+        if (cudaGetDevice(&cur) == cudaSuccess &&
+            cudaDeviceGetAttribute(&v, cudaDevAttrMultiProcessorCount, cur) == cudaSuccess && v > 0) {
+            sms[dev].store(v, std::memory_order_relaxed);
         } else {
             cudaGetLastError();
             return kDefaultSMs;   // no device (yet): not cached
         }
     }
-    return sms;
+    return v;
 }
 
 Workspace carve(char *base, int64_t max_n, int leaf_cap)
@@ -411,7 +452,8 @@ bh_status bh_create(bh_ctx **out, int64_t max_n, int leaf_cap, int group_size, v
     w.group_w = c->group;
     c->ws = w;
     const size_t hs = (sizeof(DevState) + 63) & ~(size_t)63;
-    cudaError_t e = cudaMallocHost((void **)&c->host_state, hs + 16 * sizeof(double));
+    cudaError_t e = cudaGetDevice(&c->device);
+    if (e == cudaSuccess) e = cudaMallocHost((void **)&c->host_state, hs + 16 * sizeof(double));
     if (e == cudaSuccess) c->host_diag = reinterpret_cast<double *>(reinterpret_cast<char *>(c->host_state) + hs);
     if (e == cudaSuccess) e = cudaMemsetAsync(w.st, 0, sizeof(DevState), c->stream);
     if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&c->copy_stream, cudaStreamNonBlocking);
@@ -456,6 +498,7 @@ bh_status bh_destroy(bh_ctx *c)
 bh_status bh_set_stream(bh_ctx *c, void *cuda_stream)
 {
     if (!c) return BH_ERR_INVALID_ARG;
+    if (bh_status ds = on_device(c, "bh_set_stream")) return ds;
     cudaStreamSynchronize(c->stream);
     c->stream = (cudaStream_t)cuda_stream;
     return BH_OK;
@@ -464,6 +507,7 @@ bh_status bh_set_stream(bh_ctx *c, void *cuda_stream)
 bh_status bh_build(bh_ctx *c, const double *pos_dev, const double *mass_dev, int64_t n)
 {
     if (!c) return BH_ERR_INVALID_ARG;
+    if (bh_status ds = on_device(c, "bh_build")) return ds;
     if (!pos_dev || !mass_dev) return fail(c, BH_ERR_INVALID_ARG, "bh_build: null pointer");
     if (n < 1 || n > c->max_n) return fail(c, BH_ERR_INVALID_ARG, "bh_build: n out of range");
     return do_build(c, pos_dev, mass_dev, n);
@@ -472,6 +516,7 @@ bh_status bh_build(bh_ctx *c, const double *pos_dev, const double *mass_dev, int
 bh_status bh_accel(bh_ctx *c, double theta, double eps, double G, double *acc_dev)
 {
     if (!c) return BH_ERR_INVALID_ARG;
+    if (bh_status ds = on_device(c, "bh_accel")) return ds;
     if (!c->built) return fail(c, BH_ERR_STATE, "bh_accel before bh_build");
     if (!acc_dev) return fail(c, BH_ERR_INVALID_ARG, "bh_accel: null pointer");
     if (!(theta >= 0.0) || !(eps >= 0.0)) return fail(c, BH_ERR_INVALID_ARG, "bh_accel: theta or eps negative");
@@ -481,6 +526,7 @@ bh_status bh_accel(bh_ctx *c, double theta, double eps, double G, double *acc_de
 bh_status bh_direct(bh_ctx *c, double eps, double G, double *acc_dev)
 {
     if (!c) return BH_ERR_INVALID_ARG;
+    if (bh_status ds = on_device(c, "bh_direct")) return ds;
     if (!c->built) return fail(c, BH_ERR_STATE, "bh_direct before bh_build");
     if (!acc_dev) return fail(c, BH_ERR_INVALID_ARG, "bh_direct: null pointer");
     if (!(eps >= 0.0)) return fail(c, BH_ERR_INVALID_ARG, "bh_direct: eps negative");
@@ -494,6 +540,7 @@ bh_status bh_direct(bh_ctx *c, double eps, double G, double *acc_dev)
 bh_status bh_direct_targets(bh_ctx *c, const int32_t *tgt_dev, int64_t nt, double eps, double G, double *acc_dev)
 {
     if (!c) return BH_ERR_INVALID_ARG;
+    if (bh_status ds = on_device(c, "bh_direct_targets")) return ds;
     if (!c->built) return fail(c, BH_ERR_STATE, "bh_direct_targets before bh_build");
     if (!acc_dev || !tgt_dev) return fail(c, BH_ERR_INVALID_ARG, "bh_direct_targets: null pointer");
     if (nt < 1 || !(eps >= 0.0)) return fail(c, BH_ERR_INVALID_ARG, "bh_direct_targets: nt < 1 or eps negative");
@@ -508,6 +555,7 @@ bh_status bh_bind_state(bh_ctx *c, double *pos_dev, double *vel_dev, const doubl
                         double theta, double eps, double G)
 {
     if (!c) return BH_ERR_INVALID_ARG;
+    if (bh_status ds = on_device(c, "bh_bind_state")) return ds;
     if (!pos_dev || !vel_dev || !mass_dev) return fail(c, BH_ERR_INVALID_ARG, "bh_bind_state: null pointer");
     if (n < 1 || n > c->max_n) return fail(c, BH_ERR_INVALID_ARG, "bh_bind_state: n out of range");
     if (!(theta >= 0.0) || !(eps >= 0.0)) return fail(c, BH_ERR_INVALID_ARG, "bh_bind_state: theta or eps negative");
@@ -567,6 +615,7 @@ static void stepper_done(bh_ctx *c, bool acc_is_current)
 bh_status bh_kdk_step(bh_ctx *c, double dt)
 {
     if (!c) return BH_ERR_INVALID_ARG;
+    if (bh_status ds = on_device(c, "bh_kdk_step")) return ds;
     if (!c->bound) return fail(c, BH_ERR_STATE, "bh_kdk_step before bh_bind_state");
     // the first step also evaluates a(x0): not the repeating pattern
     const bh_status st = !c->have_acc ? kdk_enqueue(c, dt) : run_stepper(c, 0, dt, 0, [=]() { return kdk_enqueue(c, dt); });
@@ -603,6 +652,7 @@ static bh_status euler_enqueue(bh_ctx *c, double dt, int n_sub, const char *who)
 static bh_status euler_like(bh_ctx *c, double dt, int n_sub, const char *who)
 {
     if (!c) return BH_ERR_INVALID_ARG;
+    if (bh_status ds = on_device(c, "stepper")) return ds;
     if (!c->bound) return fail(c, BH_ERR_STATE, "stepper called before bh_bind_state");
     if (n_sub < 1) return fail(c, BH_ERR_INVALID_ARG, "n_sub < 1");
     const bh_status st = run_stepper(c, 1, dt, n_sub, [=]() { return euler_enqueue(c, dt, n_sub, who); });
@@ -645,6 +695,7 @@ bh_status bh_multirate_step(bh_ctx *c, double dt_c, int n_sub)
 bh_status bh_potential(bh_ctx *c, double theta, double eps, double G, double *phi_dev)
 {
     if (!c) return BH_ERR_INVALID_ARG;
+    if (bh_status ds = on_device(c, "bh_potential")) return ds;
     if (!c->built) return fail(c, BH_ERR_STATE, "bh_potential before bh_build");
     if (!phi_dev) return fail(c, BH_ERR_INVALID_ARG, "bh_potential: null pointer");
     if (!(theta >= 0.0) || !(eps >= 0.0)) return fail(c, BH_ERR_INVALID_ARG, "bh_potential: theta or eps negative");
@@ -654,6 +705,7 @@ bh_status bh_potential(bh_ctx *c, double theta, double eps, double G, double *ph
 bh_status bh_accel_potential(bh_ctx *c, double theta, double eps, double G, double *acc_dev, double *phi_dev)
 {
     if (!c) return BH_ERR_INVALID_ARG;
+    if (bh_status ds = on_device(c, "bh_accel_potential")) return ds;
     if (!c->built) return fail(c, BH_ERR_STATE, "bh_accel_potential before bh_build");
     if (!acc_dev || !phi_dev) return fail(c, BH_ERR_INVALID_ARG, "bh_accel_potential: null pointer");
     if (!(theta >= 0.0) || !(eps >= 0.0)) return fail(c, BH_ERR_INVALID_ARG, "bh_accel_potential: theta or eps negative");
@@ -663,6 +715,7 @@ bh_status bh_accel_potential(bh_ctx *c, double theta, double eps, double G, doub
 bh_status bh_direct_potential(bh_ctx *c, double eps, double G, double *phi_dev)
 {
     if (!c) return BH_ERR_INVALID_ARG;
+    if (bh_status ds = on_device(c, "bh_direct_potential")) return ds;
     if (!c->built) return fail(c, BH_ERR_STATE, "bh_direct_potential before bh_build");
     if (!phi_dev) return fail(c, BH_ERR_INVALID_ARG, "bh_direct_potential: null pointer");
     if (!(eps >= 0.0)) return fail(c, BH_ERR_INVALID_ARG, "bh_direct_potential: eps negative");
@@ -687,6 +740,7 @@ bh_status bh_diagnostics(bh_ctx *c, const double *pos_dev, const double *vel_dev
                          const double *phi_dev, int64_t n, double out_host[8])
 {
     if (!c) return BH_ERR_INVALID_ARG;
+    if (bh_status ds = on_device(c, "bh_diagnostics")) return ds;
     if (!pos_dev || !vel_dev || !mass_dev || !out_host) return fail(c, BH_ERR_INVALID_ARG, "bh_diagnostics: null pointer");
     if (n < 1) return fail(c, BH_ERR_INVALID_ARG, "bh_diagnostics: n < 1");
     launch_diagnostics(c->ws, pos_dev, vel_dev, mass_dev, phi_dev, n, c->stream);
@@ -699,6 +753,7 @@ bh_status bh_diagnostics(bh_ctx *c, const double *pos_dev, const double *vel_dev
 bh_status bh_position_error(bh_ctx *c, const double *pos_dev, const double *ref_dev, int64_t n, double *err_host)
 {
     if (!c) return BH_ERR_INVALID_ARG;
+    if (bh_status ds = on_device(c, "bh_position_error")) return ds;
     if (!pos_dev || !ref_dev || !err_host) return fail(c, BH_ERR_INVALID_ARG, "bh_position_error: null pointer");
     if (n < 1) return fail(c, BH_ERR_INVALID_ARG, "bh_position_error: n < 1");
     launch_position_error(c->ws, pos_dev, ref_dev, n, c->stream);
@@ -712,6 +767,7 @@ bh_status bh_broadphase(bh_ctx *c, const double *radius_dev, const double *vel_d
                         int64_t capacity, int64_t *count_host)
 {
     if (!c) return BH_ERR_INVALID_ARG;
+    if (bh_status ds = on_device(c, "bh_broadphase")) return ds;
     if (!c->built) return fail(c, BH_ERR_STATE, "bh_broadphase before bh_build");
     if (!radius_dev || !count_host) return fail(c, BH_ERR_INVALID_ARG, "bh_broadphase: null pointer");
     if (capacity < 0 || (capacity > 0 && !pairs_dev)) return fail(c, BH_ERR_INVALID_ARG, "bh_broadphase: bad pair buffer");
@@ -729,6 +785,7 @@ bh_status bh_aggregates(bh_ctx *c, int64_t n, const int32_t *pairs_dev, int64_t 
                         int32_t *label_dev, int32_t *size_dev, double *agg_mass_dev, int64_t counts_host[2])
 {
     if (!c) return BH_ERR_INVALID_ARG;
+    if (bh_status ds = on_device(c, "bh_aggregates")) return ds;
     if (!label_dev || !counts_host) return fail(c, BH_ERR_INVALID_ARG, "bh_aggregates: null pointer");
     if (n < 1 || n > c->max_n) return fail(c, BH_ERR_INVALID_ARG, "bh_aggregates: n out of range");
     if (n_pairs < 0 || (n_pairs > 0 && !pairs_dev)) return fail(c, BH_ERR_INVALID_ARG, "bh_aggregates: bad pair list");
@@ -758,6 +815,7 @@ bh_status bh_get_state_acc(bh_ctx *c, const double **acc_dev)
 bh_status bh_copy_state_acc(bh_ctx *c, double *acc_dev)
 {
     if (!c || !acc_dev) return BH_ERR_INVALID_ARG;
+    if (bh_status ds = on_device(c, "bh_copy_state_acc")) return ds;
     if (!c->bound || !c->acc_filled) return fail(c, BH_ERR_STATE, "no stepper evaluation yet");
     return cuda_check(c, cudaMemcpyAsync(acc_dev, c->ws.acc, (size_t)c->bound_n * 24, cudaMemcpyDeviceToDevice,
                                          c->stream), "bh_copy_state_acc");
@@ -778,6 +836,7 @@ bh_status bh_eval_host(bh_ctx *c, const double *pos_host, const double *mass_hos
                        double eps, double G, double *acc_host)
 {
     if (!c) return BH_ERR_INVALID_ARG;
+    if (bh_status ds = on_device(c, "bh_eval_host")) return ds;
     if (!pos_host || !mass_host || !acc_host) return fail(c, BH_ERR_INVALID_ARG, "bh_eval_host: null pointer");
     if (n < 1 || n > c->max_n) return fail(c, BH_ERR_INVALID_ARG, "bh_eval_host: n out of range");
     if (!(theta >= 0.0) || !(eps >= 0.0)) return fail(c, BH_ERR_INVALID_ARG, "bh_eval_host: theta or eps negative");
@@ -811,12 +870,14 @@ bh_status bh_eval_host(bh_ctx *c, const double *pos_host, const double *mass_hos
 bh_status bh_synchronize(bh_ctx *c)
 {
     if (!c) return BH_ERR_INVALID_ARG;
+    if (bh_status ds = on_device(c, "bh_synchronize")) return ds;
     return fetch_state(c);
 }
 
 bh_status bh_get_cube(bh_ctx *c, double lo_host[3], double *side_host)
 {
     if (!c || !lo_host || !side_host) return BH_ERR_INVALID_ARG;
+    if (bh_status ds = on_device(c, "bh_get_cube")) return ds;
     if (!c->built) return fail(c, BH_ERR_STATE, "no build yet");
     bh_status st = fetch_state(c);
     if (st != BH_OK) return st;
@@ -828,6 +889,7 @@ bh_status bh_get_cube(bh_ctx *c, double lo_host[3], double *side_host)
 bh_status bh_get_keys(bh_ctx *c, uint64_t *sorted_key_dev, uint32_t *perm_dev)
 {
     if (!c) return BH_ERR_INVALID_ARG;
+    if (bh_status ds = on_device(c, "bh_get_keys")) return ds;
     if (!c->built) return fail(c, BH_ERR_STATE, "no build yet");
     cudaError_t e = cudaSuccess;
     if (sorted_key_dev)
@@ -840,6 +902,7 @@ bh_status bh_get_keys(bh_ctx *c, uint64_t *sorted_key_dev, uint32_t *perm_dev)
 bh_status bh_get_node_count(bh_ctx *c, int64_t *m_host, int32_t *depth_host)
 {
     if (!c || !m_host) return BH_ERR_INVALID_ARG;
+    if (bh_status ds = on_device(c, "bh_get_node_count")) return ds;
     if (!c->built) return fail(c, BH_ERR_STATE, "no build yet");
     bh_status st = fetch_state(c);
     if (st != BH_OK) return st;
@@ -852,6 +915,7 @@ bh_status bh_get_nodes(bh_ctx *c, uint8_t *level, uint32_t *begin, uint32_t *cou
                        uint8_t *child_mask, int32_t *parent, double *mono)
 {
     if (!c) return BH_ERR_INVALID_ARG;
+    if (bh_status ds = on_device(c, "bh_get_nodes")) return ds;
     if (!c->built) return fail(c, BH_ERR_STATE, "no build yet");
     bh_status st = fetch_state(c);
     if (st != BH_OK) return st;
@@ -878,6 +942,7 @@ bh_status bh_get_nodes(bh_ctx *c, uint8_t *level, uint32_t *begin, uint32_t *cou
 bh_status bh_get_groups(bh_ctx *c, int64_t *ng_host, uint32_t *gstart_dev)
 {
     if (!c || !ng_host) return BH_ERR_INVALID_ARG;
+    if (bh_status ds = on_device(c, "bh_get_groups")) return ds;
     if (!c->built) return fail(c, BH_ERR_STATE, "no build yet");
     bh_status st = fetch_state(c);
     if (st != BH_OK) return st;
@@ -890,6 +955,7 @@ bh_status bh_get_groups(bh_ctx *c, int64_t *ng_host, uint32_t *gstart_dev)
 bh_status bh_get_bodies(bh_ctx *c, double *sbody_dev, double *glo_dev, double *ghi_dev)
 {
     if (!c) return BH_ERR_INVALID_ARG;
+    if (bh_status ds = on_device(c, "bh_get_bodies")) return ds;
     if (!c->built) return fail(c, BH_ERR_STATE, "no build yet");
     bh_status st = fetch_state(c);
     if (st != BH_OK) return st;
@@ -907,6 +973,7 @@ bh_status bh_get_bodies(bh_ctx *c, double *sbody_dev, double *glo_dev, double *g
 bh_status bh_get_counts(bh_ctx *c, uint32_t *n_mono_dev, uint32_t *n_direct_dev)
 {
     if (!c) return BH_ERR_INVALID_ARG;
+    if (bh_status ds = on_device(c, "bh_get_counts")) return ds;
     if (!c->walked) return fail(c, BH_ERR_STATE, "no bh_accel since the last build");
     bh_status st = fetch_state(c);
     if (st != BH_OK) return st;
@@ -922,6 +989,7 @@ bh_status bh_get_counts(bh_ctx *c, uint32_t *n_mono_dev, uint32_t *n_direct_dev)
 bh_status bh_get_stats(bh_ctx *c, uint64_t stats_host[BH_NUM_STATS])
 {
     if (!c || !stats_host) return BH_ERR_INVALID_ARG;
+    if (bh_status ds = on_device(c, "bh_get_stats")) return ds;
     if (!c->walked) return fail(c, BH_ERR_STATE, "no bh_accel since the last build");
     bh_status st = fetch_state(c);
     if (st != BH_OK) return st;
@@ -947,6 +1015,7 @@ bh_status bh_set_timing(bh_ctx *c, int enable)
 bh_status bh_get_phase_ms(bh_ctx *c, float ms_host[BH_NUM_PHASES])
 {
     if (!c || !ms_host) return BH_ERR_INVALID_ARG;
+    if (bh_status ds = on_device(c, "bh_get_phase_ms")) return ds;
     cudaError_t e = cudaStreamSynchronize(c->stream);
     if (e != cudaSuccess) return cuda_check(c, e, "bh_get_phase_ms");
     for (int p = 0; p < BH_NUM_PHASES; ++p) {

@@ -4,6 +4,8 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
+#include <atomic>
+
 #include "bh.h"
 
 namespace bh {
@@ -13,7 +15,7 @@ constexpr int kLevels = kMaxLevel + 1;    // levels 0..21
 constexpr int kMaxGroup = 32;             // W <= 32: a walk group is evaluated by one warp (run-time, bh_create)
 constexpr int kMaxGroupCell = 2048;       // Gc <= 2048 (run-time, bh_set_group_cell): bounds the window scratch of the tree kernels
 constexpr int kMaxBboxBlocks = 1024;       // rows of the bounding-box partials
-constexpr int kDefaultSMs = 148;          // B200; the real count is queried once (sm_count())
+constexpr int kDefaultSMs = 148;          // B200; the real count is queried once per device (sm_count())
 constexpr int kRadixBits = 8;
 constexpr int kRadix = 1 << kRadixBits;   // 256 bins
 constexpr int kSortPasses = 8;            // 63 key bits
@@ -114,9 +116,13 @@ struct WalkConfig {
     static constexpr int kPairsPerBlock = 8;   // producer/consumer warp pairs in the one block of an SM
 };
 
-// multiprocessors of the current device, queried once; kDefaultSMs when there is no device (host-only
+// multiprocessors of the current device, queried once per device; kDefaultSMs when there is no device (host-only
 // argument checks and size queries still work)
 int sm_count();
+// ordinal of the current CUDA device, 0 when there is none; below kMaxDevices.  What a launcher sets up once
+// (shared-memory attributes, occupancy, cooperative-launch support) it sets up once PER DEVICE, indexed by this.
+constexpr int kMaxDevices = 64;
+int current_device();
 
 inline int64_t node_capacity(int64_t n, int leaf_cap) { return n + 21 * (n / (leaf_cap + 1)) + 1; }
 

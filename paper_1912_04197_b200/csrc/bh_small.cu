@@ -217,10 +217,11 @@ static void launch_small_t(const Workspace &w, const double *pos, const double *
     size_t emit_bytes = (size_t)(kTreeTile / 32) * (kLevels + 1) * 4;
     size_t bytes = sort_bytes > tree_bytes ? sort_bytes : tree_bytes;
     if (emit_bytes > bytes) bytes = emit_bytes;
-    static bool configured = false;
-    if (!configured) {
+    static std::atomic<bool> configured[kMaxDevices];   // the attribute is per device
+    const int dev = current_device();
+    if (!configured[dev].load(std::memory_order_relaxed)) {
         cudaFuncSetAttribute(build_small_kernel<ITEMS>, cudaFuncAttributeMaxDynamicSharedMemorySize, 96 * 1024);
-        configured = true;
+        configured[dev].store(true, std::memory_order_relaxed);
     }
     build_small_kernel<ITEMS><<<1, kSmallThreads, bytes, s>>>(w, pos, mass, n, w.leaf_cap);
 }

@@ -4,6 +4,8 @@
 // the tile's global digit offsets with a decoupled look-back over the tiles before it, and scatters
 // through shared memory so that the global writes are runs of consecutive addresses per digit.
 // The global digit histograms of all passes were accumulated by keys_kernel.
+#include <cstdlib>
+
 #include "bh_keys.cuh"
 #include "bh_sort.cuh"
 #include "bh_grid.cuh"
@@ -106,12 +108,19 @@ int sort_tile_items(int64_t n) { return n < kSortSmallTileBelow ? 8 : 16; }
 template <int ITEMS>
 static bool launch_sort_fallback(const Workspace &w, const double *pos, int64_t n, int tiles, cudaStream_t s)
 {
-    static int per_sm = -1;
+    static std::atomic<int> occupancy[kMaxDevices];   // resident blocks per SM + 1, per device; 0 = not asked yet
+    const int dev = current_device();
+    int per_sm = occupancy[dev].load(std::memory_order_relaxed) - 1;
     if (per_sm < 0) {
         if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, sort_fallback_kernel<ITEMS>, kSortThreads, 0) != cudaSuccess) per_sm = 0;
         cudaGetLastError();
+        occupancy[dev].store(per_sm + 1, std::memory_order_relaxed);
     }
     if (per_sm < 1) return false;
+    // test hook (tests/test_gpu_api.py): behave as if the driver refused the cooperative launch, as it may under MPS or
+    // on a partition without enough free SMs
+    static const bool refuse = getenv("BH_TEST_REFUSE_COOPERATIVE_SORT") != nullptr;
+    if (refuse) return false;
     int blocks = per_sm * w.sms;
     if (blocks > tiles) blocks = tiles;
     Workspace wc = w;
@@ -137,47 +146,55 @@ static void launch_sort_pass(const Workspace &w, int64_t n, int tiles, int p, in
                                                                       w.hist + p * kRadix, lb, w.sort_ticket + p);
 }
 
+// the eight plain digit passes over the full keys (key[0]/idx[0] -> ... -> key[0]/idx[0]); needs no co-resident kernel
+static void launch_sort_eight(const Workspace &w, int64_t n, int items, int tiles, cudaStream_t s)
+{
+    for (int p = 0; p < kSortPasses; ++p) {
+        if (items == 8) launch_sort_pass<8>(w, n, tiles, p, p & 1, p == 0, s);
+        else launch_sort_pass<16>(w, n, tiles, p, p & 1, p == 0, s);
+    }
+}
+
 // pos: the caller's positions (the fallback recomputes the keys from them)
 int launch_sort(const Workspace &w, const double *pos, int64_t n, cudaStream_t s)
 {
     const int items = sort_tile_items(n);
     const int tiles = (int)((n + kSortThreads * items - 1) / (kSortThreads * items));
-    // the partial-key sort needs its fallback kernel, a cooperative launch: asked once
-    static int partial = -1;
-    if (partial < 0) {
-        int dev = 0, coop = 0;
-        cudaGetDevice(&dev);
-        cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev);
-        partial = coop ? 1 : 0;
+    // the partial-key sort needs its fallback kernel, a cooperative launch: asked once per device
+    static std::atomic<int> mode[kMaxDevices];   // 0 = not asked yet, 1 = partial-key sort, 2 = eight plain passes
+    const int dev = current_device();
+    int m = mode[dev].load(std::memory_order_relaxed);
+    if (m == 0) {
+        int cur = 0, coop = 0;
+        cudaGetDevice(&cur);
+        cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, cur);
         cudaGetLastError();
+        m = coop ? 1 : 2;
+        mode[dev].store(m, std::memory_order_relaxed);
     }
-    if (partial) {
-        int a = 0;
-        for (int p = kHighFirst; p < kSortPasses; ++p, a ^= 1) {
-            if (items == 8) launch_sort_pass<8>(w, n, tiles, p, a, p == kHighFirst, s);
-            else launch_sort_pass<16>(w, n, tiles, p, a, p == kHighFirst, s);
-        }
-        const int rblocks = (int)((n + kSortThreads * kRepairPer - 1) / (kSortThreads * kRepairPer));
-        sort_repair_kernel<<<rblocks, kSortThreads, 0, s>>>(w.key[a], w.idx[a], w.key[a ^ 1], w.idx[a ^ 1], n, w.st);
-        const bool ok = items == 8 ? launch_sort_fallback<8>(w, pos, n, tiles, s) : launch_sort_fallback<16>(w, pos, n, tiles, s);
-        return ok ? (kSortPasses - kHighFirst) + 2 : -1;     // -1: the caller reports a CUDA error
+    if (m == 2) {
+        launch_sort_eight(w, n, items, tiles, s);
+        return kSortPasses;
     }
-    for (int p = 0; p < kSortPasses; ++p) {
-        const int a = p & 1, b = a ^ 1;
-        unsigned *lb = w.lookback + (size_t)p * tiles * kRadix;   // [pass][tiles of this n][256]: cleared per build
-#define BH_SORT_PASS(FIRST, ITEMS)                                                                                     \
-    sort_pass_kernel<FIRST, ITEMS><<<tiles, kSortThreads, 0, s>>>(w.key[a], w.idx[a], w.key[b], w.idx[b], n,           \
-                                                                  p * kRadixBits, w.hist + p * kRadix, lb, w.sort_ticket + p)
-        if (items == 8) {
-            if (p == 0) BH_SORT_PASS(true, 8);
-            else BH_SORT_PASS(false, 8);
-        } else {
-            if (p == 0) BH_SORT_PASS(true, 16);
-            else BH_SORT_PASS(false, 16);
-        }
-#undef BH_SORT_PASS
+    int a = 0;
+    for (int p = kHighFirst; p < kSortPasses; ++p, a ^= 1) {
+        if (items == 8) launch_sort_pass<8>(w, n, tiles, p, a, p == kHighFirst, s);
+        else launch_sort_pass<16>(w, n, tiles, p, a, p == kHighFirst, s);
     }
-    return kSortPasses;
+    const int rblocks = (int)((n + kSortThreads * kRepairPer - 1) / (kSortThreads * kRepairPer));
+    sort_repair_kernel<<<rblocks, kSortThreads, 0, s>>>(w.key[a], w.idx[a], w.key[a ^ 1], w.idx[a ^ 1], n, w.st);
+    const bool ok = items == 8 ? launch_sort_fallback<8>(w, pos, n, tiles, s) : launch_sort_fallback<16>(w, pos, n, tiles, s);
+    if (ok) return (kSortPasses - kHighFirst) + 2;
+    // The co-resident kernel could not be launched (the attribute said it could: MPS, a busy partition).  Without it a run of
+    // more than 64 equal top key bits would stay unsorted, so this build starts its sort again with the eight plain passes
+    // — histograms, tickets and look-back rows cleared, keys recomputed from the positions — and so does every later build
+    // on this device.  Same permutation, bit for bit.
+    mode[dev].store(2, std::memory_order_relaxed);
+    const size_t zbytes = (size_t)((char *)w.lookback - (char *)w.hist) + (size_t)kSortPasses * tiles * kRadix * sizeof(unsigned);
+    if (cudaMemsetAsync(w.hist, 0, zbytes, s) != cudaSuccess) return -1;      // -1: the caller reports a CUDA error
+    launch_keys(w, pos, n, s);
+    launch_sort_eight(w, n, items, tiles, s);
+    return (kSortPasses - kHighFirst) + 1 + 1 + kSortPasses;   // five passes + repair, then keys + eight passes
 }
 
 }  // namespace bh

@@ -1,5 +1,5 @@
 // bh_walk.cu — step a7 (group-cooperative tree walk, Eqs. (3)-(6) PAPER.md:84-106), step a8 (direct
-// N^2 sum, Eq. (1)), step a9 (leapfrog kernels) and the fp64 peak microbenchmark.
+// N^2 sum, Eq. (1)) and step a9 (leapfrog kernels).
 //
 // Walk: a group is up to 32 Morton-consecutive bodies of one group cell (R6).  The kernel is warp
 // specialised: one persistent 512-thread block per SM holds eight PAIRS of warps, a producer and a
@@ -705,10 +705,11 @@ __global__ void kick_kernel(double *__restrict__ vel, const double *__restrict__
 template <bool GUARD, int MODE>
 static void launch_walk_t(const Workspace &w, double theta, double eps2, double G, double *out, double *phi, cudaStream_t s)
 {
-    static bool configured = false;
-    if (!configured) {
+    static std::atomic<bool> configured[kMaxDevices];   // the attribute is per device
+    const int dev = current_device();
+    if (!configured[dev].load(std::memory_order_relaxed)) {
         cudaFuncSetAttribute(walk_kernel<GUARD, MODE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(WalkSmem));
-        configured = true;
+        configured[dev].store(true, std::memory_order_relaxed);
     }
     const int blocks = w.walk_warps / kPairs;   // one persistent block per SM
     walk_kernel<GUARD, MODE><<<blocks, kWalkThreads, sizeof(WalkSmem), s>>>(

@@ -70,7 +70,15 @@ def test_phase_timing_and_launch_count():
     bh.bh_kdk_step(ctx.ctx, 1e-3)                    # first step: a(x0) once more
     bh.bh_kdk_step(ctx.ctx, 1e-3)
     assert bh.bh_get_launches(ctx.ctx) - l0 == 2 * 16 + 15      # a(x0): build 14 + walk; a step: kick+drift (with the cube), 13, walk, kick
-    assert bh.bh_get_phase_ms(ctx.ctx)["kick_drift"] > 0.0
+    ph = bh.bh_get_phase_ms(ctx.ctx)
+    assert ph["kick_drift"] > 0.0 and ph["walk"] > 0.0
+    # a build reports the phases it ran: this step's cube was taken by the drift (part of kick_drift), the direct sum
+    # of before is not part of the step
+    assert ph["cube"] == 0.0 and ph["direct"] == 0.0
+    # ... and a one-kernel build on the context that just ran streaming builds reports its one kernel under "tree"
+    ctx.build(pos[:2000].contiguous(), mass[:2000].contiguous())
+    ph = bh.bh_get_phase_ms(ctx.ctx)
+    assert ph["tree"] > 0.0 and all(ph[k] == 0.0 for k in ("cube", "keys", "sort", "gather", "monopoles"))
     # one sort tile (n <= 4096): the whole build is one launch of one block
     small = bh.Context(2000, 16)
     w2 = wl.make("c1", 2000)
@@ -86,6 +94,25 @@ def test_phase_timing_and_launch_count():
     assert bh.bh_get_launches(mid.ctx) - l0 == 1
     mid.close()
     ctx.close()
+
+
+def test_sort_survives_a_refused_cooperative_launch():
+    """The streaming sort ends with a co-resident (cooperative) kernel that a driver may refuse to launch (MPS, a busy
+    partition).  The build must then start its sort again with the eight plain digit passes and keep to them on that
+    device, with the same permutation.  BH_TEST_REFUSE_COOPERATIVE_SORT makes the launcher behave as if refused; the
+    switch is read once per process, hence the subprocess.  The parity test it runs builds twice per context: the first
+    build takes the recovery path, the second the plain passes from the start; 300 coincident bodies need the full
+    eight digits."""
+    import os
+    import subprocess
+    import sys
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    env = dict(os.environ, BH_TEST_REFUSE_COOPERATIVE_SORT="1")
+    r = subprocess.run([sys.executable, "-m", "pytest", "-q", "-x", "-m", "gpu", "-p", "no:cacheprovider",
+                        os.path.join(root, "tests", "test_gpu_parity.py"), "-k",
+                        "test_partial_key_sort_and_its_fallback and (200000 or 600000)"],
+                       env=env, cwd=root, capture_output=True, text=True, timeout=900)
+    assert r.returncode == 0 and "4 passed" in r.stdout, r.stdout[-3000:] + r.stderr[-1000:]
 
 
 def test_state_acc_pointer_and_sorted_bodies():
