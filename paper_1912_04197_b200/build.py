@@ -37,8 +37,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
                          for lib in (LIB, MICRO_LIB)):
         return LIB
     nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
-    extra = os.environ.get("BH_NVCC_EXTRA", "").split()       # extra nvcc flags, e.g. -DBH_TRIP_UNROLL=2
-    flags = [f for f in NVCC_FLAGS if f != "-shared"] + extra + (["-Xptxas", "-v"] if verbose else []) + \
+    flags = [f for f in NVCC_FLAGS if f != "-shared"] + (["-Xptxas", "-v"] if verbose else []) + \
         ["-I", os.path.join(ROOT, "include")]
     objdir = os.path.join(HERE, "build")
     os.makedirs(objdir, exist_ok=True)

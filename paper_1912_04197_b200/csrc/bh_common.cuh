@@ -20,15 +20,9 @@ constexpr int kRadixBits = 8;
 constexpr int kRadix = 1 << kRadixBits;   // 256 bins
 constexpr int kSortPasses = 8;            // 63 key bits
 constexpr int kSortThreads = 256;
-#ifndef BH_SORT_ITEMS
-#define BH_SORT_ITEMS 16
-#endif
-constexpr int kSortItems = BH_SORT_ITEMS;   // keys per thread
+constexpr int kSortItems = 16;              // keys per thread
 constexpr int kSortTile = kSortThreads * kSortItems;   // 4096 keys per tile (one tile: the one-block build, bh_small.cu)
-#ifndef BH_SORT_SMALL_BELOW
-#define BH_SORT_SMALL_BELOW (1 << 19)
-#endif
-constexpr int64_t kSortSmallTileBelow = BH_SORT_SMALL_BELOW;   // the streaming passes use 2048-key tiles below this many keys
+constexpr int64_t kSortSmallTileBelow = 1 << 19;   // the streaming passes use 2048-key tiles below this many keys
 constexpr int kTreeTile = 1024;           // bodies per block in the tree kernels
 constexpr int kDiagBlocks = 592;          // diagnostics: a FIXED number of partial sums, whatever the device, so that the reduction order is fixed
 constexpr int kStackSlab = 22 * 256;      // walk: spill entries (8 bytes each) per producer warp: <= 32 x 7 ranges per level; overflow sets kStatStack

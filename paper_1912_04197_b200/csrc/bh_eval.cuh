@@ -8,9 +8,6 @@
 namespace bh {
 
 constexpr int kRing = 512;                  // sources per producer/consumer pair (power of two, multiple of 8)
-#ifndef BH_SEED_LOWWORD
-#define BH_SEED_LOWWORD 1                   // rsqrt seed: low word taken from a dead register pair (see interact)
-#endif
 // GUARD (chosen by the launchers when eps^2 is below the smallest normal double, eps = 0 included): a softened
 // squared distance that is zero or subnormal adds nothing.  rsqrt.approx.ftz flushes a subnormal argument to
 // zero and would return infinity, and with it 0 * inf = NaN for a coincident pair (R13; bh.h preconditions).
@@ -27,7 +24,6 @@ __device__ __forceinline__ void interact(double px, double py, double pz, double
     const double t2 = fma(dy, dy, fma(dz, dz, eps2));
     const double r2 = fma(dx, dx, t2);
     double y;
-#if BH_SEED_LOWWORD
     // the seed's low word is irrelevant (the series below corrects any y within 2^-19 of r2^-1/2): take it
     // from the dead partial sum, so that MUFU.RSQ64H can write into that register pair without a zero-fill
     {
@@ -35,9 +31,6 @@ __device__ __forceinline__ void interact(double px, double py, double pz, double
         asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y0) : "d"(r2));
         y = __hiloint2double(__double2hiint(y0), __double2loint(t2));
     }
-#else
-    asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(r2));
-#endif
     if (GUARD) y = (r2 >= kTinyR2) ? y : 0.0;  // a pair at zero softened distance adds nothing (R13)
     const double u = y * y;
     const double w = s.w * y;

@@ -35,20 +35,10 @@ constexpr int kStack = 512;                 // sibling ranges per producer in sh
 constexpr int kSpill = 128;                 // spill / refill unit
 constexpr int kDesc = 4;                    // group descriptors in flight per pair
 constexpr unsigned kNoGroup = 0xffffffffu;
-#ifndef BH_SLEEP_FULL
-#define BH_SLEEP_FULL 1000                  // ns a producer sleeps per poll while its ring is full
-#endif
-#ifndef BH_TRIP_UNROLL
-#define BH_TRIP_UNROLL 1
-#endif
-#ifndef BH_REG_PROD
-#define BH_REG_PROD 96                      // registers per thread of the producer warpgroups ...
-#define BH_REG_CONS 160                     // ... and of the consumer warpgroups (launch: 128)
-#endif
-constexpr int kTripUnroll = BH_TRIP_UNROLL;   // producer: trips of a pop unrolled
-#ifndef BH_PUB_MIN
-#define BH_PUB_MIN 32                       // a trip publishes only if more than this many entries are pending (the consumer starts a batch at 32)
-#endif
+constexpr unsigned kSleepFullNs = 1000;     // ns a producer sleeps per poll while its ring is full
+constexpr int kRegProd = 96;                // registers per thread of the producer warpgroups ...
+constexpr int kRegCons = 160;               // ... and of the consumer warpgroups (launch: 128)
+constexpr int kPubMin = 32;                 // a trip publishes only if more than this many entries are pending (the consumer starts a batch at 32)
 
 
 constexpr int kMaxSplit = 4;                 // most consumer warps that share one producer's ring (see walk_kernel)
@@ -142,7 +132,7 @@ struct Producer {
         publish(tail);
         const unsigned want = n > (unsigned)kRing / 2 - 64u ? n : (unsigned)kRing / 2 - 64u;
         while (true) {
-            __nanosleep(BH_SLEEP_FULL);
+            __nanosleep(kSleepFullNs);
             head_seen = warp_acquire_min(ps.ctrl.head_pub, split, lane);
             if (tail + want - head_seen <= (unsigned)kRing) break;
         }
@@ -272,7 +262,7 @@ __device__ void produce(PairSmem &ps, DevState *st, const unsigned *__restrict__
             nxt.info = make_uint4(0u, 0u, 0u, 0u);
             nxt.mn = make_double4(0.0, 0.0, 0.0, 0.0);
             if (nsib > 0) nxt = load_rec(winfo, mono, first);
-#pragma unroll kTripUnroll
+#pragma unroll 1
             for (unsigned q = 0; q < trips; ++q) {
                 const bool have = q < nsib;
                 const NodeRec cur = nxt;
@@ -363,7 +353,7 @@ __device__ void produce(PairSmem &ps, DevState *st, const unsigned *__restrict__
                 }
                 // ---- publish what is complete: everything up to the end of the previous trip ----
                 cp_async_commit();
-                if ((int)(tail_prev - P.pub) > BH_PUB_MIN) {
+                if ((int)(tail_prev - P.pub) > kPubMin) {
                     cp_async_wait_1();
                     P.publish(tail_prev);
                 }
@@ -585,12 +575,10 @@ walk_kernel(DevState *st, const unsigned *__restrict__ gstart, const double4 *__
     PairSmem &ps = sm.pair[pair - sub];
     if (producer && sub == 0 && lane_id() < sizeof(PairCtrl) / 4) reinterpret_cast<unsigned *>(&ps.ctrl)[lane_id()] = 0u;
     __syncthreads();
-#if BH_REG_PROD > 0
     // the block is launched with 128 registers per thread; the producer warpgroups hand registers to
     // the consumer warpgroups (warps 0-3 / 4-7 / 8-11 / 12-15 are the four warpgroups)
-    if (producer) asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(BH_REG_PROD));
-    else asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(BH_REG_CONS));
-#endif
+    if (producer) asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(kRegProd));
+    else asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(kRegCons));
     if (producer) {
         if (sub == 0)
             produce<MODE != 0>(ps, st, gstart, sbody, gbox, winfo, mono, theta2, cnt_mono, cnt_direct,
