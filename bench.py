@@ -15,7 +15,7 @@ e2e     = the same metric through bh_eval_host: pinned host pos/mass in, acc out
 roofline= the walk kernel (dominant): 20 flops per body-source interaction over its
           CUDA-event duration, against the fp64 FMA rate MEASURED in the same run (libbh_microbench.so;
           MEASURED_PEAKS.json has no fp64 entry); the nominal 148 SM x 64 lanes x 2 x 1.965 GHz beside it.
-          traffic and l2_hit_rate are profiler figures read from profiles/r02_roofline.csv (ncu --set full).
+          traffic and l2_hit_rate are profiler figures read from profiles/r03_roofline.csv (ncu --set full).
 cpu_baseline = the oracle as it stands on the host cores, on a bounded sample of the same workload.
 
 Multi-GPU: the path does not shard (north_star: one GPU, no collectives) -> replicas only; every
@@ -38,7 +38,7 @@ METRIC = "BH accel evals/s (build+walk) N=1M theta=0.5 fp64; speedup vs direct N
 UNIT = "body-accelerations/s"
 FLOPS_PER_INTERACTION = 20.0
 FP64_NOMINAL_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12   # nominal: SMs x fp64 FMA lanes x 2 x max SM clock
-PROFILE_CSV = os.path.join(ROOT, "profiles", "r02_roofline.csv")
+PROFILE_CSV = os.path.join(ROOT, "profiles", "r03_roofline.csv")
 
 
 def workload_desc(w):
@@ -54,14 +54,30 @@ def config_dict(w, world: int):
                   "reference arm: the oracle on host cores, bounded sample of the workload"}
 
 
+def source_sha1(files: str) -> str:
+    """sha1 over the contents of the CUDA sources a kernel is compiled from (';'-separated names under csrc/), the
+    fingerprint a row of the profile CSV carries: a row whose sources have changed since its capture is stale."""
+    import hashlib
+    h = hashlib.sha1()
+    for name in files.split(";"):
+        with open(os.path.join(ROOT, "paper_1912_04197_b200", "csrc", name), "rb") as f:
+            h.update(f.read())
+    return h.hexdigest()[:16]
+
+
 def profile_row(kernel: str, config: str):
     """Profiler figures of one kernel launch (dram bytes, L2 hit rate, ...) from the committed summary of the
-    ncu --set full captures, profiles/r02_roofline.csv (its .md names the commands and the commit)."""
+    ncu --set full captures, profiles/r03_roofline.csv (its .md names the commands and the commit).  The row gets
+    "stale": True when the kernel's sources no longer hash to what they did at the capture."""
     import csv
     try:
         with open(PROFILE_CSV) as f:
             for row in csv.DictReader(f):
                 if row["kernel"] == kernel and row["config"] == config:
+                    try:
+                        row["stale"] = source_sha1(row["source_files"]) != row["source_sha1"]
+                    except (OSError, KeyError):
+                        row["stale"] = True
                     return row
     except OSError:
         pass
@@ -435,8 +451,9 @@ def run_own(args):
                 "traffic": float(prof["dram_bytes_per_launch"]) if prof else None,
                 "l2_hit_rate": float(prof["l2_hit_pct"]) / 100.0 if prof else None,
                 "fp64_pipe_active": float(prof["fp64_pipe_pct"]) / 100.0 if prof else None,
-                "profile_source": (f"profiles/r02_roofline.csv (ncu --set full at commit {prof['commit']}; profiler "
-                                   "figures, not measured by this run)") if prof else None}
+                "profile_source": (f"profiles/r03_roofline.csv (ncu --set full at commit {prof['commit']}; profiler "
+                                   "figures, not measured by this run)") if prof else None,
+                "profile_stale": bool(prof["stale"]) if prof else None}
     # build kernels against HBM: algorithmic bytes per body over the time of the SAME phases.
     # Inside a KDK step above the one-kernel builds' sizes the drift kernel takes the bounding cube (step a1): that pass
     # is timed under "kick_drift", phases["cube"] is 0, and a1's 24 B/body leave the numerator with it.
@@ -493,7 +510,8 @@ def run_own(args):
                                       "unit": "TFLOP/s", "frac": dtf / peak_meas, "frac_of_nominal": dtf / FP64_NOMINAL_TFLOPS,
                                       "traffic": float(dprof["dram_bytes_per_launch"]) if dprof else None,
                                       "l2_hit_rate": float(dprof["l2_hit_pct"]) / 100.0 if dprof else None,
-                                      "fp64_pipe_active": float(dprof["fp64_pipe_pct"]) / 100.0 if dprof else None}}
+                                      "fp64_pipe_active": float(dprof["fp64_pipe_pct"]) / 100.0 if dprof else None,
+                                      "profile_stale": bool(dprof["stale"]) if dprof else None}}
         out["speedup_vs_direct"] = direct_full_ms / (total_ms / args.steps)
 
         # ---- end to end through the C ABI with host buffers ----

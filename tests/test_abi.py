@@ -57,3 +57,19 @@ def test_missing_library_fails_loudly(monkeypatch):
     monkeypatch.setattr(binding, "LIB_PATH", "/nonexistent/libbh.so")
     with pytest.raises(RuntimeError, match="no CPU fallback"):
         binding.lib()
+
+
+def test_profile_rows_match_the_kernel_sources():
+    """profiles/r03_roofline.csv carries a fingerprint of each kernel's sources at its ncu capture; bench.py marks a row
+    stale when the sources have changed since.  No committed row may be stale: a kernel edit needs a new capture."""
+    import csv
+
+    import bench
+    with open(bench.PROFILE_CSV) as f:
+        rows = list(csv.DictReader(f))
+    assert len(rows) >= 10
+    for r in rows:
+        assert bench.source_sha1(r["source_files"]) == r["source_sha1"], (r["kernel"], r["config"], r["commit"])
+    assert bench.profile_row("walk_kernel", "c4")["stale"] is False
+    assert bench.profile_row("walk_kernel", "c9") is None
+
