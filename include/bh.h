@@ -15,6 +15,12 @@
  *   - Return value: BH_OK (0) or a negative bh_status.  No exceptions, no abort().  Data errors that
  *     only the GPU can see (non-finite coordinates, node capacity) are sticky: they are reported by
  *     the next synchronising call.  bh_last_error() gives a human-readable message.
+ *   - Devices: a context belongs to the CUDA device that was current at bh_create (its workspace, stream and
+ *     events live there).  Make that device current before every call on the context; a call that touches the
+ *     GPU with another device current returns BH_ERR_STATE.  One process may hold contexts on several devices;
+ *     what the library sets up once per kernel (shared-memory limits, occupancy) it sets up per device.
+ *     bh_last_error(NULL) returns the message of the last context-free call that failed on this host thread
+ *     (bh_create, bh_diagnostics_static).
  *   - Ownership: the caller owns every buffer it passes, including the workspace; the library
  *     allocates no device memory except a few bytes of pinned host memory at bh_create.
  *   - Range of the input.  Checked on the GPU (sticky BH_ERR_NONFINITE / BH_ERR_INVALID_ARG): every
